@@ -1,0 +1,532 @@
+"""Pins of the fp64 oracle against what the paper and the mathematics fix (CPU only).
+
+Each test names the pin (P1..P15 of SURVEY.md 8(c)-P / DESIGN.md "Oracle pins") and the passage it rests on.
+None of the expected values comes from the oracle itself or from the CUDA path: they are closed forms,
+invariants, dense direct solves assembled from the paper's printed matrix entries, or brute force.
+"""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import tdgl_oracle as O
+
+P_, O_ = O.PERIODIC, O.OPEN
+ALL_BC = [(a, b, c) for a in (P_, O_) for b in (P_, O_) for c in (P_, O_)]
+
+
+def rand_psi(p, seed, amp=1.0):
+    rng = np.random.default_rng(seed)
+    return amp * (rng.uniform(-1, 1, p.shape) + 1j * rng.uniform(-1, 1, p.shape))
+
+
+def nonzero_psi(p, seed):
+    """Zero-free field with a rough phase (modulus in [0.5, 1.5])."""
+    rng = np.random.default_rng(seed)
+    return (1.0 + 0.5 * rng.uniform(-1, 1, p.shape)) * np.exp(1j * rng.uniform(-math.pi, math.pi, p.shape))
+
+
+# ------------------------------------------------------------------------------------------------
+# P1 / P2: reaction term + Crank-Nicolson linearisation (Eq. 26 with psi_est = psi^-)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("a,eps0", [(0.3, 1.0), (1.2, 1.0), (0.7, 0.5), (0.4, -1.0)])
+def test_P1_uniform_reaction_closed_form(a, eps0):
+    # Eq. (26), B = 0, uniform real psi = a:  psi+ (1 - q) = psi- (1 + q),  q = h_t (eps - a^2)/2
+    p = O.Params(8, 6, 4, eps_tol=1e-28, max_sweeps=2000, solve_mu=False)
+    st = O.State(psi=np.full(p.shape, a, dtype=np.complex128), mu=np.zeros(p.shape))
+    O.step(p, st, np.full(p.shape, eps0), 0.0, 0.0, 0.0)
+    q = p.ht * (eps0 - a * a) / 2.0
+    assert np.max(np.abs(st.psi - a * (1 + q) / (1 - q))) < 1e-13
+
+
+@pytest.mark.parametrize("bc", [(P_, P_, P_), (P_, P_, O_), (O_, O_, O_)])
+def test_P2_uniform_fixed_point(bc):
+    # psi = sqrt(eps) at zero field is stationary (BASELINE.json north_star); residual 0, one sweep.
+    p = O.Params(8, 8, 8, bc=bc, solve_mu=True)
+    eps0 = 0.64
+    st = O.State(psi=np.full(p.shape, math.sqrt(eps0), dtype=np.complex128), mu=np.zeros(p.shape))
+    for _ in range(3):
+        O.step(p, st, np.full(p.shape, eps0), 0.0, 0.0, 0.0)
+        assert st.sweeps_last == 1
+    assert np.max(np.abs(st.psi - math.sqrt(eps0))) < 1e-15
+    assert np.max(np.abs(st.mu)) < 1e-15 and st.K == 0.0
+
+
+# ------------------------------------------------------------------------------------------------
+# P3: plane wave -> Laplacian, sign of U, CN factor (Eqs. 26, 27, 29a)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("K", [0.0, 0.37, -1.1])
+def test_P3_plane_wave_growth_factor(K):
+    p = O.Params(16, 8, 4, hx=0.5, hy=0.4, hz=0.7, g=1.3, eps_tol=1e-30, max_sweeps=5000, solve_mu=False)
+    eps0, delta = 0.8, 1e-7
+    mx, my, mz = 3, 1, 1
+    kx, ky, kz = (2 * math.pi * mx / p.length("x"), 2 * math.pi * my / p.length("y"),
+                  2 * math.pi * mz / p.length("z"))
+    k_, j_, i_ = np.meshgrid(np.arange(p.nz), np.arange(p.ny), np.arange(p.nx), indexing="ij")
+    wave = np.exp(1j * (kx * i_ * p.hx + ky * j_ * p.hy + kz * k_ * p.hz))
+    st = O.State(psi=delta * wave, mu=np.zeros(p.shape), K=K)
+    O.step(p, st, np.full(p.shape, eps0), 0.0, 0.0, 0.0, fixed_sweeps=200)   # |r| is O(delta): iterate to rounding
+    # (grad - iA~)^2 with A~ = -K e_x acts on e^{ikx} as -(k+K)^2; lattice version 2 - 2cos((k+K)h)
+    lam = ((2 - 2 * math.cos((kx + K) * p.hx)) / p.hx ** 2 + (2 - 2 * math.cos(ky * p.hy)) / p.hy ** 2
+           + (2 - 2 * math.cos(kz * p.hz)) / (p.g * p.hz) ** 2)
+    q = p.ht * (eps0 - lam) / 2.0
+    fac = (1 + q) / (1 - q)
+    assert np.max(np.abs(st.psi / (delta * wave) - fac)) < 1e-12   # nonlinearity is O(delta^2)
+
+
+# ------------------------------------------------------------------------------------------------
+# P4: J_av (Eq. 35)
+# ------------------------------------------------------------------------------------------------
+def test_P4_average_supercurrent_closed_form():
+    # psi = a e^{ikx}: continuum J = a^2 (k + K); Eq. (35) central difference gives a^2 sin((k+K)h)/h
+    p = O.Params(16, 4, 4)
+    a, K, mx = 0.9, 0.23, 2
+    kx = 2 * math.pi * mx / p.length("x")
+    i_ = np.arange(p.nx)[None, None, :]
+    psi = a * np.exp(1j * kx * i_ * p.hx) * np.ones(p.shape)
+    J = O.average_supercurrent(p, psi, O.paper_links(p, K, 0.0, 0.0))
+    assert abs(J - a * a * math.sin((kx + K) * p.hx) / p.hx) < 1e-14
+
+
+# ------------------------------------------------------------------------------------------------
+# P5: Ohmic normal state (Eq. 21 with psi = 0: d_t K = J_ext, E = J)
+# ------------------------------------------------------------------------------------------------
+def test_P5_ohmic_normal_state():
+    p = O.Params(8, 8, 4)
+    st = O.State(psi=np.zeros(p.shape, dtype=np.complex128), mu=np.zeros(p.shape))
+    Jext = 0.7
+    for n in range(1, 400):
+        O.step(p, st, np.full(p.shape, -1.0), 0.0, 0.0, Jext)
+        assert abs(st.Ex - Jext) < 1e-15
+        expect = math.fmod(n * p.dt * Jext, 2 * math.pi / p.hx)      # rewinding
+        assert abs(st.K - expect) < 1e-9
+    assert n * p.dt * Jext > 2 * math.pi / p.hx                        # the run did wrap at least once
+    assert np.max(np.abs(st.mu)) == 0.0 and np.max(np.abs(st.psi)) == 0.0
+
+
+# ------------------------------------------------------------------------------------------------
+# P6: quasi-periodic boundary, P_{i,k}, flux quantisation
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("nzq,nxq", [(4, 0), (1, 2), (-3, 1)])
+def test_P6_flux_quantisation_topological(nzq, nxq):
+    p = O.Params(12, 10, 6, hx=0.5, hy=0.6, hz=0.4)
+    Bz_req = 2 * math.pi * nzq / (p.length("x") * p.length("y")) * 1.0004   # slightly off: must snap
+    Bx_req = 2 * math.pi * nxq / (p.length("y") * p.length("z")) + 1e-4
+    Bx, Bz, nx_, nz_ = O.snap_field(p, Bx_req, Bz_req)
+    assert (nx_, nz_) == (nxq, nzq)
+    psi = nonzero_psi(p, 5)
+    links = O.paper_links(p, 0.31, Bx, Bz)
+    n = O.plaquette_windings(p, psi, links, Bz)
+    assert np.max(np.abs(n - np.rint(n))) < 1e-12          # every winding is an integer ...
+    per_slice = np.rint(n).sum(axis=(1, 2))
+    assert np.all(per_slice == nzq)                          # ... and each z-slice holds exactly n_z quanta
+    assert abs(O.vortices_per_slice(p, psi, links, Bz) - nzq) < 1e-12
+
+
+def test_P6_unsnapped_field_breaks_the_identity():
+    # negative control: without the flux constraint the phase jump is discontinuous and the count is not n_z
+    p = O.Params(12, 10, 4)
+    Bz = 2 * math.pi * 3.5 / (p.length("x") * p.length("y"))
+    psi = nonzero_psi(p, 6)
+    n = O.plaquette_windings(p, psi, O.paper_links(p, 0.0, 0.0, Bz), Bz)
+    assert np.max(np.abs(n - np.rint(n))) > 1e-3
+
+
+# ------------------------------------------------------------------------------------------------
+# P7: current conservation after the mu solve (Eqs. 17, 18)
+# ------------------------------------------------------------------------------------------------
+def _divergence(p, jx, jy, jz):
+    """Lattice divergence of link currents; at an open face the ghost link carries minus the first link
+    (mirror), so the boundary divergence is 2 j / h."""
+    out = np.zeros(p.shape)
+    for a, axis, h, j in ((0, 2, p.hx, jx), (1, 1, p.hy, jy), (2, 0, p.hz, jz)):
+        d = (j - np.roll(j, 1, axis)) / h
+        if p.bc[a] == O_:
+            first = [slice(None)] * 3
+            last = [slice(None)] * 3
+            first[axis], last[axis] = 0, -1
+            first, last = tuple(first), tuple(last)
+            jm1 = np.take(j, -2, axis=axis)
+            d[first] = 2.0 * j[first] / h
+            d[last] = -2.0 * jm1 / h
+        out += d
+    return out
+
+
+@pytest.mark.parametrize("bc", ALL_BC)
+def test_P7_current_conservation(bc):
+    p = O.Params(8, 6, 7, hx=0.5, hy=0.45, hz=0.6, g=1.2, bc=bc)
+    Bx, Bz, _, _ = O.snap_field(p, 0.07, 0.21)
+    links = O.paper_links(p, 0.4 if bc[0] == P_ else 0.0, Bx, Bz)
+    psi = rand_psi(p, 11)
+    rho = O.supercurrent_divergence(p, psi, links)
+    js = O.link_supercurrents(p, psi, links)
+    assert np.max(np.abs(_divergence(p, *js) - rho)) < 1e-12           # rho IS div j_s
+    assert abs(np.sum(O.site_weights(p) * rho)) < 1e-11                 # solvability (S6)
+    mu = O.solve_poisson(p, rho)
+    jn = []
+    for a, axis, h, gg in ((0, 2, p.hx, 1.0), (1, 1, p.hy, 1.0), (2, 0, p.hz, p.g ** 2)):
+        j = -(np.roll(mu, -1, axis) - mu) / (h * gg)
+        if bc[a] == O_:
+            sl = [slice(None)] * 3
+            sl[axis] = -1
+            j[tuple(sl)] = 0.0
+        jn.append(j)
+    total = [js[a] + jn[a] for a in range(3)]
+    assert np.max(np.abs(_divergence(p, *total))) < 1e-11              # div (j_s + j_n) = 0
+    assert abs(np.sum(O.site_weights(p) * mu)) < 1e-11                  # gauge S7
+
+
+# ------------------------------------------------------------------------------------------------
+# P8: gauge invariance
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("bc", [(P_, P_, P_), (P_, P_, O_), (P_, O_, O_), (O_, O_, O_)])
+def test_P8_gauge_invariance(bc):
+    p = O.Params(8, 8, 6, bc=bc, eps_tol=1e-6)
+    Jext = 0.05 if bc[0] == P_ else 0.0
+    Bx, Bz, _, _ = O.snap_field(p, 0.1, 0.4)
+    rng = np.random.default_rng(3)
+    chi = rng.uniform(-3, 3, p.shape)
+    eps = np.where(rng.uniform(size=p.shape) < 0.2, -1.0, 1.0)
+
+    def links_fn(K):
+        return O.paper_links(p, K, Bx, Bz)
+
+    def links_fn_g(K):
+        # psi' = psi e^{i chi};  S'+ f' = e^{i chi} S+ f  <=>  th'(m) = th(m) + chi(m) - chi(m + alpha)
+        thx, thy, thz = O.paper_links(p, K, Bx, Bz)
+        return (thx + chi - np.roll(chi, -1, 2), thy + chi - np.roll(chi, -1, 1), thz + chi - np.roll(chi, -1, 0))
+
+    psi0 = 1.0 + 0.3 * rand_psi(p, 2)
+    a = O.State(psi=psi0.copy(), mu=np.zeros(p.shape))
+    b = O.State(psi=psi0 * np.exp(1j * chi), mu=np.zeros(p.shape))
+    for n in range(12):
+        O.step(p, a, eps, Bx, Bz, Jext, links_fn=links_fn)
+        O.step(p, b, eps, Bx, Bz, Jext, links_fn=links_fn_g)
+        assert a.sweeps_last == b.sweeps_last
+        assert np.max(np.abs(b.psi - a.psi * np.exp(1j * chi))) < 1e-12
+        assert np.max(np.abs(a.mu - b.mu)) < 1e-12
+        assert abs(a.K - b.K) < 1e-12 and abs(a.Jav - b.Jav) < 1e-13
+    la, lb = links_fn(a.K), links_fn_g(b.K)
+    assert abs(O.free_energy(p, a.psi, eps, la) - O.free_energy(p, b.psi, eps, lb)) < 1e-10
+    ja, jb = O.link_supercurrents(p, a.psi, la), O.link_supercurrents(p, b.psi, lb)
+    assert max(np.max(np.abs(x - y)) for x, y in zip(ja, jb)) < 1e-12
+    assert np.max(np.abs(O.supercurrent_divergence(p, a.psi, la) - O.supercurrent_divergence(p, b.psi, lb))) < 1e-11
+
+
+# ------------------------------------------------------------------------------------------------
+# P9: the implicit step against a dense direct solve (BASELINE.json north_star)
+# ------------------------------------------------------------------------------------------------
+def dense_M(p, psi_prev, mu, eps, K, Bx, Bz):
+    """Assemble the N x N matrix of Eq. (30) entry by entry from the printed list, the
+    quasi-periodic rows and the open-face second derivatives."""
+    N = p.n_sites
+    M = np.zeros((N, N), dtype=np.complex128)
+    ht = p.ht
+    Ly = p.length("y")
+
+    def idx(i, j, k):
+        return i + p.nx * (j + p.ny * k)
+
+    for k in range(p.nz):
+        for j in range(p.ny):
+            ybar = j * p.hy - Ly / 2
+            Ux = np.exp(1j * p.hx * (K + Bz * ybar))           # U = exp(-i h A~), A~_x = -B_z ybar - K
+            Uz = np.exp(-1j * p.hz * Bx * ybar)                 # A~_z = +B_x ybar
+            for i in range(p.nx):
+                m = idx(i, j, k)
+                Pik = np.exp(1j * (i * p.hx * Ly * Bz - k * p.hz * Ly * Bx))
+                M[m, m] = 1 + (ht / 2) * (abs(psi_prev[k, j, i]) ** 2
+                                          + 2 * (1 / p.hx ** 2 + 1 / p.hy ** 2 + 1 / (p.g * p.hz) ** 2)
+                                          + 1j * p.u * mu[k, j, i] - eps[k, j, i])
+                # x
+                ax = -ht / (2 * p.hx ** 2)
+                if p.bc[0] == P_:
+                    M[m, idx((i + 1) % p.nx, j, k)] += ax * Ux
+                    M[m, idx((i - 1) % p.nx, j, k)] += ax * np.conj(Ux)
+                elif i == 0:
+                    M[m, idx(1, j, k)] += 2 * ax * Ux                       # 2(U psi_1 - psi_0)/h^2
+                elif i == p.nx - 1:
+                    M[m, idx(p.nx - 2, j, k)] += 2 * ax * np.conj(Ux)        # 2(U* psi_{N-2} - psi_{N-1})/h^2
+                else:
+                    M[m, idx(i + 1, j, k)] += ax * Ux
+                    M[m, idx(i - 1, j, k)] += ax * np.conj(Ux)
+                # y
+                ay = -ht / (2 * p.hy ** 2)
+                if p.bc[1] == P_:
+                    if j == 0:
+                        M[m, idx(i, 1 % p.ny, k)] += ay
+                        M[m, idx(i, p.ny - 1, k)] += ay * Pik
+                    elif j == p.ny - 1:
+                        M[m, idx(i, 0, k)] += ay * np.conj(Pik)
+                        M[m, idx(i, p.ny - 2, k)] += ay
+                    else:
+                        M[m, idx(i, j + 1, k)] += ay
+                        M[m, idx(i, j - 1, k)] += ay
+                elif j == 0:
+                    M[m, idx(i, 1, k)] += 2 * ay
+                elif j == p.ny - 1:
+                    M[m, idx(i, p.ny - 2, k)] += 2 * ay
+                else:
+                    M[m, idx(i, j + 1, k)] += ay
+                    M[m, idx(i, j - 1, k)] += ay
+                # z
+                az = -ht / (2 * (p.g * p.hz) ** 2)
+                if p.bc[2] == P_:
+                    M[m, idx(i, j, (k + 1) % p.nz)] += az * Uz
+                    M[m, idx(i, j, (k - 1) % p.nz)] += az * np.conj(Uz)
+                elif k == 0:
+                    M[m, idx(i, j, 1)] += 2 * az * Uz
+                elif k == p.nz - 1:
+                    M[m, idx(i, j, p.nz - 2)] += 2 * az * np.conj(Uz)
+                else:
+                    M[m, idx(i, j, k + 1)] += az * Uz
+                    M[m, idx(i, j, k - 1)] += az * np.conj(Uz)
+    return M
+
+
+@pytest.mark.parametrize("bc", [(P_, P_, P_), (P_, P_, O_), (P_, O_, P_), (O_, O_, O_)])
+def test_P9_implicit_step_dense_solve(bc):
+    p = O.Params(8, 8, 8, hx=0.5, hy=0.55, hz=0.45, g=1.1, u=1.7, bc=bc, eps_tol=1e-28, max_sweeps=5000,
+                 solve_mu=False)
+    Bx, Bz, _, _ = O.snap_field(p, 0.12, 0.35)
+    K = 0.21 if bc[0] == P_ else 0.0
+    rng = np.random.default_rng(4)
+    psi0 = 1.0 + 0.4 * rand_psi(p, 7)
+    mu0 = rng.uniform(-0.2, 0.2, p.shape)
+    eps = np.where(rng.uniform(size=p.shape) < 0.3, -1.0, 1.0)
+    M = dense_M(p, psi0, mu0, eps, K, Bx, Bz)
+    # Crank-Nicolson: M = I - (h_t/2) Lin, b = (I + (h_t/2) Lin) psi^-  =>  b = 2 psi^- - M psi^-  (Eq. 26, 31)
+    b_dense = 2 * psi0.ravel() - M @ psi0.ravel()
+    links = O.paper_links(p, K, Bx, Bz)
+    b, d = O.build_system(p, psi0, mu0, eps, links)
+    assert np.max(np.abs(b.ravel() - b_dense)) < 1e-13
+    assert np.max(np.abs(d.ravel() - np.diag(M))) < 1e-15
+    # diagonal dominance margin the paper relies on
+    off = np.sum(np.abs(M), axis=1) - np.abs(np.diag(M))
+    assert np.all(np.abs(np.diag(M)) > off)
+    x_dense = np.linalg.solve(M, b_dense)
+    st = O.State(psi=psi0.copy(), mu=mu0.copy(), K=K)
+    O.step(p, st, eps, Bx, Bz, 0.0)
+    assert np.max(np.abs(st.psi.ravel() - x_dense)) < 1e-12
+    # residual bookkeeping (S8): r^l = b - M x^l
+    x1, r0 = O.jacobi_sweep(p, psi0, b, d, links)
+    assert np.max(np.abs(r0.ravel() - (b_dense - M @ psi0.ravel()))) < 1e-13
+
+
+def test_P9_noise_enters_as_ht_zeta():
+    # Eq. (26): the Langevin term contributes h_t zeta_m to psi - psi^-  =>  M (psi_T - psi_0) = h_t zeta
+    p0 = O.Params(8, 8, 8, eps_tol=1e-28, max_sweeps=5000, solve_mu=False)
+    pT = O.Params(8, 8, 8, eps_tol=1e-28, max_sweeps=5000, solve_mu=False, temperature=1e-3, seed=99)
+    Bx, Bz, _, _ = O.snap_field(p0, 0.0, 0.4)
+    psi0 = 1.0 + 0.2 * rand_psi(p0, 1)
+    eps = np.ones(p0.shape)
+    a = O.State(psi=psi0.copy(), mu=np.zeros(p0.shape), n=5)
+    b = O.State(psi=psi0.copy(), mu=np.zeros(p0.shape), n=5)
+    O.step(p0, a, eps, Bx, Bz, 0.0)
+    O.step(pT, b, eps, Bx, Bz, 0.0)
+    M = dense_M(p0, psi0, np.zeros(p0.shape), eps, 0.0, Bx, Bz)
+    zeta = (M @ (b.psi - a.psi).ravel()) / pT.ht
+    zmax = O.zeta_max(pT)
+    assert abs(zmax - math.sqrt(0.12)) < 1e-15          # Eq. (39) at h = 0.5, dt = 0.1, T = 1e-3, u = 1
+    assert np.max(np.abs(zeta.real)) < zmax and np.max(np.abs(zeta.imag)) < zmax
+    # <|zeta|^2> = (2/3) zeta_max^2; 512 samples -> ~4 % statistical error
+    assert abs(np.mean(np.abs(zeta) ** 2) / (2.0 / 3.0 * zmax ** 2) - 1.0) < 0.15
+    # and it is exactly the generator's stream for (seed, step 5)
+    assert np.max(np.abs(zeta - O.langevin_noise(pT, 5).ravel())) < 1e-12
+
+
+# ------------------------------------------------------------------------------------------------
+# P10: Poisson problem against a dense bordered solve and eigen-checks (PAPER.md:379, S5-S7)
+# ------------------------------------------------------------------------------------------------
+def dense_laplacian(p):
+    N = p.n_sites
+    A = np.zeros((N, N))
+    n = (p.nx, p.ny, p.nz)
+    c = (1 / p.hx ** 2, 1 / p.hy ** 2, 1 / (p.g * p.hz) ** 2)
+
+    def idx(q):
+        return q[0] + p.nx * (q[1] + p.ny * q[2])
+
+    for k in range(p.nz):
+        for j in range(p.ny):
+            for i in range(p.nx):
+                q = [i, j, k]
+                m = idx(q)
+                for a in range(3):
+                    A[m, m] -= 2 * c[a]
+                    for s in (+1, -1):
+                        r = list(q)
+                        r[a] += s
+                        if p.bc[a] == P_:
+                            r[a] %= n[a]
+                        elif r[a] < 0:
+                            r[a] = 1                      # mirror ghost mu_{-1} = mu_{1} (S6)
+                        elif r[a] >= n[a]:
+                            r[a] = n[a] - 2
+                        A[m, idx(r)] += c[a]
+    return A
+
+
+@pytest.mark.parametrize("bc", ALL_BC)
+def test_P10_poisson_dense_bordered_solve(bc):
+    p = O.Params(8, 7, 6, hx=0.5, hy=0.4, hz=0.65, g=1.25, bc=bc)
+    A = dense_laplacian(p)
+    w = O.site_weights(p).ravel()
+    rng = np.random.default_rng(8)
+    rho = rng.uniform(-1, 1, p.shape)
+    rho -= np.sum(w * rho.ravel()) / np.sum(w)                    # compatible right side
+    # the stencil operator is that matrix
+    f = rng.uniform(-1, 1, p.shape)
+    assert np.max(np.abs(O.laplacian_real(p, f).ravel() - A @ f.ravel())) < 1e-12
+    N = p.n_sites
+    B = np.zeros((N + 1, N + 1))
+    B[:N, :N] = A
+    B[:N, N] = 1.0
+    B[N, :N] = w
+    sol = np.linalg.solve(B, np.append(rho.ravel(), 0.0))
+    mu = O.solve_poisson(p, rho)
+    assert abs(sol[N]) < 1e-12
+    assert np.max(np.abs(mu.ravel() - sol[:N])) < 1e-11
+    assert np.max(np.abs(O.laplacian_real(p, mu) - rho)) < 1e-11
+
+
+@pytest.mark.parametrize("bc", [(P_, P_, O_), (O_, P_, P_)])
+def test_P10_eigenvectors(bc):
+    p = O.Params(8, 8, 9, bc=bc)
+    k_, j_, i_ = np.meshgrid(np.arange(p.nz), np.arange(p.ny), np.arange(p.nx), indexing="ij")
+    for axis_name, idx, n, c in (("x", i_, p.nx, p.cx), ("z", k_, p.nz, p.cz)):
+        a = "xyz".index(axis_name)
+        for q in (1, 3):
+            if bc[a] == P_:
+                v, lam = np.cos(2 * math.pi * q * idx / n), -c * (2 - 2 * math.cos(2 * math.pi * q / n))
+            else:
+                v, lam = np.cos(math.pi * q * idx / (n - 1)), -c * (2 - 2 * math.cos(math.pi * q / (n - 1)))
+            assert np.max(np.abs(O.laplacian_real(p, v) - lam * v)) < 1e-12
+
+
+# ------------------------------------------------------------------------------------------------
+# P11: open faces carry no normal supercurrent
+# ------------------------------------------------------------------------------------------------
+def test_P11_open_face_normal_current_vanishes():
+    p = O.Params(6, 7, 5, bc=(O_, O_, O_))
+    links = O.paper_links(p, 0.0, 0.13, 0.29)
+    psi = rand_psi(p, 12)
+    for th, axis in ((links[0], 2), (links[1], 1), (links[2], 0)):
+        sp, sm = O._S(psi, th, axis, O_)
+        jn = np.imag(np.conj(psi) * (sp - sm))                 # 2 h x central-difference normal current
+        first = [slice(None)] * 3
+        last = [slice(None)] * 3
+        first[axis], last[axis] = 0, -1
+        assert np.max(np.abs(jn[tuple(first)])) == 0.0 and np.max(np.abs(jn[tuple(last)])) == 0.0
+    # and the Laplacian there is the printed form 2 (U psi_1 - psi_0)/h^2
+    L = O.covariant_laplacian(p, psi, links)
+    j = 3
+    Ux = np.exp(1j * p.hx * 0.29 * (j * p.hy - p.length("y") / 2))
+    Uz = np.exp(-1j * p.hz * 0.13 * (j * p.hy - p.length("y") / 2))
+    k, i = 2, 0
+    expect = (2 * (Ux * psi[k, j, 1] - psi[k, j, 0]) / p.hx ** 2
+              + (psi[k, j + 1, 0] + psi[k, j - 1, 0] - 2 * psi[k, j, 0]) / p.hy ** 2
+              + (Uz * psi[k + 1, j, 0] + np.conj(Uz) * psi[k - 1, j, 0] - 2 * psi[k, j, 0]) / p.hz ** 2)
+    assert abs(L[k, j, i] - expect) < 1e-13
+
+
+# ------------------------------------------------------------------------------------------------
+# P12: free energy -- gradient by finite differences, and descent
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("bc", [(P_, P_, P_), (P_, P_, O_), (O_, P_, O_), (O_, O_, O_)])
+def test_P12_free_energy_gradient(bc):
+    # -dF/dpsi*_m / (w_m h^3) = eps psi - |psi|^2 psi + (grad - iA~)^2 psi  (right side of Eq. 16, zeta = 0)
+    p = O.Params(4, 5, 4, hx=0.5, hy=0.6, hz=0.45, g=1.15, bc=bc)
+    Bx, Bz, _, _ = O.snap_field(p, 0.2, 0.5)
+    links = O.paper_links(p, 0.3 if bc[0] == P_ else 0.0, Bx, Bz)
+    rng = np.random.default_rng(21)
+    eps = rng.uniform(-1, 1, p.shape)
+    psi = rand_psi(p, 22)
+    rhs = eps * psi - np.abs(psi) ** 2 * psi + O.covariant_laplacian(p, psi, links)
+    w = O.site_weights(p)
+    vol = p.hx * p.hy * p.hz
+    dlt = 1e-6
+    for m in rng.choice(p.n_sites, size=12, replace=False):
+        k, j, i = np.unravel_index(m, p.shape)
+        g = 0.0
+        for dz, fac in ((dlt, 1.0), (1j * dlt, 1j)):
+            a, b = psi.copy(), psi.copy()
+            a[k, j, i] += dz
+            b[k, j, i] -= dz
+            dF = (O.free_energy(p, a, eps, links) - O.free_energy(p, b, eps, links)) / (2 * dlt)
+            g = g + 0.5 * fac * dF                 # dF/dpsi* = (dF/dRe + i dF/dIm)/2
+        assert abs(-g / (w[k, j, i] * vol) - rhs[k, j, i]) < 1e-6      # FD round-off ~1e-7; a wrong term is O(1)
+
+
+def test_P12_free_energy_decreases():
+    p = O.Params(16, 16, 4, solve_mu=False, eps_tol=1e-12)
+    Bx, Bz, _, _ = O.snap_field(p, 0.0, 0.2)
+    st = O.State(psi=1.0 + 0.3 * rand_psi(p, 30), mu=np.zeros(p.shape))
+    eps = np.ones(p.shape)
+    links = O.paper_links(p, 0.0, Bx, Bz)
+    F = [O.free_energy(p, st.psi, eps, links)]
+    for _ in range(60):
+        O.step(p, st, eps, Bx, Bz, 0.0)
+        F.append(O.free_energy(p, st.psi, eps, links))
+    assert all(F[n + 1] <= F[n] + 1e-12 for n in range(60))
+    assert F[-1] < F[0] - 1.0
+
+
+# ------------------------------------------------------------------------------------------------
+# P13: physics sanity -- lowest-Landau-level growth rate (H_c2 = 1 in these units)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("eps0,grows", [(1.0, True), (0.05, False)])
+def test_P13_landau_level_growth_rate(eps0, grows):
+    p = O.Params(16, 16, 2, solve_mu=False, eps_tol=1e-30, max_sweeps=3000)
+    Bx, Bz, _, nzq = O.snap_field(p, 0.0, 0.1)
+    assert nzq == 1
+    st = O.State(psi=1e-12 * rand_psi(p, 40), mu=np.zeros(p.shape))
+    eps = np.full(p.shape, eps0)
+    norms = []
+    for _ in range(160):
+        O.step(p, st, eps, Bx, Bz, 0.0, fixed_sweeps=80)      # |psi| ~ 1e-12: an absolute tolerance is useless
+        norms.append(np.linalg.norm(st.psi))
+    rate = math.log(norms[-1] / norms[-11]) / (10 * p.dt)
+    # linearised Eq. (16): d_t psi = (eps - E) psi, lowest eigenvalue of -(grad - iA)^2 is E = B_z (+O(B^2 h^2))
+    assert abs(rate - (eps0 - Bz)) < 5e-3
+    assert (rate > 0) == grows
+
+
+# ------------------------------------------------------------------------------------------------
+# P15 (soft): sweep counts the paper quotes ("about 4-6 iterations", tests/golden/paper_values.txt)
+# ------------------------------------------------------------------------------------------------
+def test_P15_sweep_counts_are_in_the_quoted_range():
+    lo, hi = None, None
+    for line in open(__file__.rsplit("/", 1)[0] + "/golden/paper_values.txt"):
+        if line.startswith("jacobi_sweeps_steady_flow"):
+            lo, hi = (int(v) for v in line.split()[1:3])
+    p = O.Params(32, 32, 8, eps_tol=1e-6)
+    Bx, Bz, _, _ = O.snap_field(p, 0.0, 0.1)
+    st = O.State(psi=1.0 + 0.01 * rand_psi(p, 50), mu=np.zeros(p.shape))
+    O.run(p, st, np.ones(p.shape), Bx, Bz, 0.05, 250)
+    late = st.sweep_log[150:]
+    assert lo - 1 <= np.mean(late) <= hi + 1, np.mean(late)
+    assert not st.hit_max_sweeps
+
+
+# ------------------------------------------------------------------------------------------------
+# a0: inclusion pattern
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("bc", [(P_, P_, P_), (P_, P_, O_), (O_, O_, O_)])
+def test_epsilon_bounding_box_equals_brute_force(bc):
+    p = O.Params(16, 12, 10, bc=bc)
+    rng = np.random.default_rng(60)
+    sph = np.stack([rng.uniform(0, 8, 9), rng.uniform(0, 6, 9), rng.uniform(0, 5, 9), rng.uniform(0.4, 2.5, 9)], 1)
+    sph[0] = (0.1, 0.2, 0.1, 2.0)          # straddles the corner: exercises the minimum image
+    sph[1] = (4.0, 3.0, 2.5, 30.0)         # larger than the box
+    a = O.epsilon_from_spheres(p, sph[:1], -1.0, 1.0)
+    assert (a[0, 0, -1] == -1.0) == (bc[0] == P_)          # image across the periodic x face only
+    e1 = O.epsilon_from_spheres(p, sph[[0, 2, 3, 4, 5, 6, 7, 8]], -1.0, 1.0)
+    e2 = O.epsilon_brute_force(p, sph[[0, 2, 3, 4, 5, 6, 7, 8]], -1.0, 1.0)
+    assert np.array_equal(e1, e2)
+    assert 0.0 < np.mean(e1 < 0) < 1.0
+    assert np.all(O.epsilon_from_spheres(p, sph[1:2], -1.0, 1.0) == -1.0)
+    # a sphere of radius r centred on a site covers exactly the lattice points with d^2 <= r^2
+    one = O.epsilon_from_spheres(p, np.array([[4.0, 3.0, 2.5, 1.0]]), -1.0, 1.0)
+    assert int(np.sum(one < 0)) == 33          # |n|^2 <= 4 on the cubic lattice h = 0.5: 1+6+12+8+6
