@@ -1,0 +1,154 @@
+/* tdgl.h -- C ABI of libtdgl: the per-time-step hot path of the large-lambda TDGL solver of
+ * Sadovskyy, Koshelev, Phillips, Karpeyev, Glatz, "Stable large-scale solver for Ginzburg-Landau
+ * equations for superconductors" (arXiv:1409.8340), hand-written CUDA for sm_100a (B200).
+ *
+ * Citations: "P:NNN" = PAPER.md line NNN; "Sxx" = a reading listed in DESIGN.md ("Readings of the
+ * paper").  Everything a step computes runs in the library's own kernels; there is no CPU path.
+ *
+ * Memory model.  The CALLER owns all device memory: one workspace block handed over at create time
+ * (size from tdgl_workspace_bytes), the output buffers of tdgl_get_psi_mu and the CUDA stream.  The
+ * library never allocates device memory.  `tdgl_t` is a small host object freed by tdgl_destroy.
+ * Pointers named *_dev are DEVICE pointers, pointers named *_host are HOST pointers that are only
+ * read / written during the call.
+ *
+ * Data layout.  Site (i, j, k) of an nx x ny x nz mesh has the multi-index m = i + nx*(j + ny*k)
+ * (x fastest).  psi is an array of N = nx*ny*nz interleaved (re, im) fp32 pairs, mu and eps
+ * are fp32 arrays of N values.  nx must be even (rows are moved as 16-byte vectors).
+ *
+ * Errors.  Every call returns an int: 0 = TDGL_OK, negative = error (nothing was done), positive =
+ * warning (the call completed).  No exceptions, no aborts, nothing is printed.
+ */
+#ifndef TDGL_H
+#define TDGL_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define TDGL_OK            0
+#define TDGL_EINVAL      (-1)   /* bad size / mesh / bc / pointer / struct_size                         */
+#define TDGL_ENOMEM      (-2)   /* workspace too small or not 256-byte aligned                          */
+#define TDGL_EINCOMPAT   (-3)   /* open x with Jx != 0, or By != 0 (yz gauge not built)         */
+#define TDGL_ECUDA       (-4)   /* a CUDA runtime call failed; tdgl_last_cuda_error() has the code      */
+#define TDGL_WMAXSWEEPS    1    /* some step hit max_sweeps before max|r|^2 < eps_tol (S10)             */
+
+#define TDGL_BC_PERIODIC   0    /* (quasi-)periodic                                          */
+#define TDGL_BC_OPEN       1    /* open: n.(grad - iA)psi = 0, n.grad(mu) = 0            */
+
+#define TDGL_FLAG_SOLVE_MU 1u   /* mu and K are active (S15).  Off: mu == 0, K == 0             */
+#define TDGL_FLAG_HOST_LOOP 2u  /* test/diagnostic: host-driven sweep loop instead of the CUDA-graph
+                                   WHILE node (identical arithmetic)                                     */
+
+typedef struct tdgl tdgl_t;
+
+/* Problem statement of the paper (Fig. 1): mesh, time step, boundary type per axis,
+ * Jacobi tolerance (Eq. 34), noise temperature (Eq. 39).  Plain C POD. */
+typedef struct {
+  uint32_t struct_size;      /* = sizeof(tdgl_params)                                                  */
+  int32_t  nx, ny, nz;       /* mesh points per axis, each >= 2, nx even                               */
+  float    hx, hy, hz;       /* mesh size in xi_0                                                      */
+  float    dt;               /* real time step; h_t = dt/u (P:257 fn. 3, S1)                           */
+  float    u;                /* relaxation-time ratio, > 0 (S1: 1)                                     */
+  float    g;                /* anisotropy, z terms / g^2                                      */
+  int32_t  bc[3];            /* per axis x,y,z: TDGL_BC_PERIODIC / TDGL_BC_OPEN                        */
+  float    eps_tol;          /* threshold on max_m |r_m|^2, Eq. (34)                                   */
+  int32_t  max_sweeps;       /* cap on Jacobi sweeps per step (S10), >= 1                              */
+  int32_t  fixed_sweeps;     /* > 0: exactly this many sweeps per step, no test (S9 replay)            */
+  float    temperature;      /* reduced T-bar of Eq. (39) (S12); 0 = no Langevin term                  */
+  uint64_t seed;             /* Philox4x32-10 key (S11)                                                */
+  float    init_amp;         /* psi0 = 1 + init_amp (N(0,1) + i N(0,1)), Philox stream 1 (S13)         */
+  uint32_t flags;            /* TDGL_FLAG_*                                                            */
+  void    *workspace_dev;    /* DEVICE memory, 256-byte aligned, >= tdgl_workspace_bytes()             */
+  uint64_t workspace_bytes;
+  void    *stream;           /* cudaStream_t the work is enqueued on (NULL = legacy default stream)    */
+} tdgl_params;
+
+/* A spherical inclusion: centre and radius in xi_0, domain coordinates (site i sits at x = i*hx). */
+typedef struct { float cx, cy, cz, r; } tdgl_sphere;
+
+typedef struct {
+  double  t;                  /* steps * dt                                                            */
+  double  K;                  /* gauge variable of Eq. (13)-(15), rewound                      */
+  double  Ex;                 /* E_x = d_t K of the last step (Eq. 15); V = Ex * Lx                    */
+  double  Jav;                /* J_av of the last step, Eq. (35)                                       */
+  double  Ex_mean;            /* mean of Ex over the steps since the last tdgl_set_field_current       */
+  double  free_energy;        /* discrete GL functional                      */
+  double  mean_abs2;          /* <|psi|^2>                                                             */
+  double  vortices_per_slice; /* signed sum of z-plaquette windings / nz                               */
+  double  max_resid2;         /* max_m |r_m|^2 at the deciding sweep of the last step                  */
+  float   Bx_eff, Bz_eff;     /* field after flux-quantum snapping                        */
+  int64_t steps;              /* steps taken since create                                              */
+  int64_t sweeps_total;       /* Jacobi sweeps since create                                            */
+  int32_t sweeps_last;        /* sweeps of the last step                                               */
+  int32_t status;             /* latched TDGL_WMAXSWEEPS, else 0                                       */
+} tdgl_obs;
+
+/* Bytes of device workspace tdgl_create needs for these params (0 if the params are invalid).
+ * About 44 bytes per site (two psi buffers, b, d: 8 B each; mu, eps, one scratch: 4 B each). */
+uint64_t tdgl_workspace_bytes(const tdgl_params *p_host);
+
+/* Validates the params, carves the workspace, builds the transform tables and sets the initial
+ * state psi0 (S13), mu = 0, K = 0, eps = 1, B = 0, J = 0.  Asynchronous on `stream`.
+ * Errors: TDGL_EINVAL, TDGL_ENOMEM, TDGL_ECUDA. */
+int tdgl_create(const tdgl_params *p_host, tdgl_t **out);
+int tdgl_destroy(tdgl_t *h);
+
+/* eps_m = eps_in if site m lies within distance r of any sphere centre (minimum image on periodic
+ * axes), else eps_out (P:245, P:511 (i), S19).  `spheres_host` is copied during the call; n may be 0.
+ * The workspace scratch array holds the device copy, so n <= N/4. */
+int tdgl_set_pinning(tdgl_t *h, const tdgl_sphere *spheres_host, int64_t n, float eps_in, float eps_out);
+
+/* Applied field (xz Landau gauge, Eq. 24a) and transport current J_ext along x (Eq. 21).
+ * B_z is snapped to 2 pi n_z/(Lx Ly) iff x and y are periodic, B_x to 2 pi n_x/(Ly Lz) iff y and z are
+ * (P:467, S16); the effective values are reported by tdgl_observables.  Resets Ex_mean.
+ * Errors: TDGL_EINCOMPAT if By != 0, or Jx != 0 with open x. */
+int tdgl_set_field_current(tdgl_t *h, float Bx, float By, float Bz, float Jx);
+
+/* nsteps time steps in the paper's order "psi, then E, then mu": the implicit
+ * Crank-Nicolson step (26) solved by Jacobi sweeps (33) to criterion (34), J_av (35) and the K update
+ * (21), then rho = div j_s and the Poisson solve for mu (18).  Asynchronous on `stream`. */
+int tdgl_step(tdgl_t *h, int32_t nsteps);
+
+/* Device-to-device copy of the current state into caller buffers (either may be NULL):
+ * psi_dev: N (re, im) fp32 pairs; mu_dev: N fp32.  Asynchronous on `stream`. */
+int tdgl_get_psi_mu(tdgl_t *h, void *psi_dev, void *mu_dev);
+
+/* Runs the reductions (a8) and fills *out_host.  Synchronises the stream. */
+int tdgl_observables(tdgl_t *h, tdgl_obs *out_host);
+
+const char *tdgl_strerror(int code);
+int tdgl_last_cuda_error(const tdgl_t *h);
+
+/* ---- extensions used by the tests and the bench (not part of the paper's problem statement) ---- */
+
+/* Replace the state: psi_dev (N float pairs), mu_dev (N floats, may be NULL = keep) and K. */
+int tdgl_set_state(tdgl_t *h, const void *psi_dev, const void *mu_dev, double K);
+/* Change the solver controls between steps (S9 replay: fixed_sweeps > 0 runs exactly that many). */
+int tdgl_set_solver(tdgl_t *h, float eps_tol, int32_t max_sweeps, int32_t fixed_sweeps);
+/* Per-step replay of prescribed sweep counts: counts_host[s] sweeps in the s-th step from now on, for
+ * n steps; after that the solver goes back to its own test.  n = 0 clears. n <= 65536. */
+int tdgl_set_sweep_schedule(tdgl_t *h, const int32_t *counts_host, int32_t n);
+/* Sweep counts and deciding max|r|^2 of the last n steps (oldest first) into host arrays
+ * (either may be NULL).  n <= min(steps, 65536).  Synchronises the stream. */
+int tdgl_get_sweep_log(tdgl_t *h, int32_t *counts_host, float *resid2_host, int32_t n);
+/* Copy eps (N fp32) / the per-site Langevin term zeta of step index `step` (N float pairs) to caller
+ * device buffers: bit-exactness checks of the inclusion kernel (a0) and of the Philox stream (a2). */
+int tdgl_get_eps(tdgl_t *h, void *eps_dev);
+int tdgl_debug_noise(tdgl_t *h, int64_t step, void *zeta_dev);
+/* Single operators for kernel-level parity: one Poisson solve mu = Delta_h^{-1} rho (rho_dev and
+ * mu_dev: N fp32, may alias), and rho = div j_s of the current state with the current K. */
+int tdgl_debug_poisson(tdgl_t *h, const void *rho_dev, void *mu_dev);
+int tdgl_debug_rho(tdgl_t *h, void *rho_dev);
+/* Number of kernels the library has launched on this handle since create (bench: gpu_launches). */
+int64_t tdgl_launch_count(const tdgl_t *h);
+/* CUDA-event timing of the Jacobi sweep kernel: when enabled, every launch of the plain sweep kernel
+ * in HOST_LOOP mode is bracketed by events on the stream; read back the accumulated milliseconds and
+ * launch count.  Used by bench.py for the roofline figure. */
+int tdgl_sweep_timing(tdgl_t *h, int32_t enable, double *ms_total_host, int64_t *launches_host);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TDGL_H */

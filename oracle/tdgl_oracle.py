@@ -110,6 +110,7 @@ class State:
     max_resid2: float = 0.0
     sweep_log: List[int] = field(default_factory=list)
     resid_log: List[float] = field(default_factory=list)   # max|r|^2 at the deciding sweep of each step
+    resid_trace: List[List[float]] = field(default_factory=list)   # max|r|^2 of every sweep of each step (S9 check)
     hit_max_sweeps: bool = False
 
 
@@ -324,7 +325,7 @@ def jacobi_sweep(p: Params, x, b, d, links):
     return xn, r
 
 
-def solve_psi(p: Params, psi, b, d, links, fixed_sweeps: Optional[int] = None):
+def solve_psi(p: Params, psi, b, d, links, fixed_sweeps: Optional[int] = None, trace: Optional[list] = None):
     """Jacobi iteration from x^0 = psi^- until max_m |r^l_m|^2 < eps_tol (Eq. 34, P:320) or the cap (S10);
     keeps x^{l+1}; sweeps = l + 1 (S8).  `fixed_sweeps`: run exactly that many sweeps, no test (S9 replay)."""
     x = psi
@@ -334,6 +335,8 @@ def solve_psi(p: Params, psi, b, d, links, fixed_sweeps: Optional[int] = None):
         x, r = jacobi_sweep(p, x, b, d, links)
         sweeps += 1
         r2 = float(np.max(r.real ** 2 + r.imag ** 2))
+        if trace is not None:
+            trace.append(r2)          # logging only
         if fixed_sweeps is not None:
             if sweeps >= fixed_sweeps:
                 break
@@ -418,7 +421,8 @@ def step(p: Params, st: State, eps, Bx: float, Bz: float, Jext: float,
     links = links_fn(st.K)
     zeta = langevin_noise(p, st.n) if p.temperature > 0.0 else None          # step 1
     b, d = build_system(p, st.psi, st.mu, eps, links, zeta)                   # steps 2, 3
-    psi, sweeps, r2 = solve_psi(p, st.psi, b, d, links, fixed_sweeps)         # step 4
+    trace: List[float] = []
+    psi, sweeps, r2 = solve_psi(p, st.psi, b, d, links, fixed_sweeps, trace)  # step 4
     K, Ex, Jav = st.K, 0.0, 0.0
     if p.solve_mu and p.bc[0] == PERIODIC:                                    # step 5 (S3)
         Jav = average_supercurrent(p, psi, links)      # new psi, old K
@@ -434,6 +438,7 @@ def step(p: Params, st: State, eps, Bx: float, Bz: float, Jext: float,
     st.sweeps_total += sweeps
     st.sweep_log.append(sweeps)
     st.resid_log.append(r2)
+    st.resid_trace.append(trace)
     if fixed_sweeps is None and sweeps >= p.max_sweeps and not r2 < p.eps_tol:
         st.hit_max_sweeps = True
     return st

@@ -1,0 +1,224 @@
+// Set-up and on-request kernels: initial state (S13), inclusion pattern (a0), field tables (a1),
+// observables (a8), control-block setters, Langevin-term dump for the Philox bit-exactness test.
+#include "tdgl_dev.cuh"
+#include "philox.cuh"
+
+// psi0 = 1 + amp (N(0,1) + i N(0,1)): Box-Muller on Philox stream 1 words (S13); mu = 0; eps = 1.
+__global__ void k_init_state(const __grid_constant__ Dev dv, float amp) {
+  for (long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x; m < dv.N; m += (long long)gridDim.x * blockDim.x) {
+    const PhiloxOut p = philox4x32_10((uint32_t)m, (uint32_t)((unsigned long long)m >> 32), 0u, 1u, dv.seed_lo, dv.seed_hi);
+    const double u1 = u32_to_01(p.x0), u2 = u32_to_01(p.x1);
+    const double rad = sqrt(-2.0 * log(u1));
+    double s, c;
+    sincospi(2.0 * u2, &s, &c);
+    dv.psi[0][m] = make_float2((float)(1.0 + (double)amp * rad * c), (float)((double)amp * rad * s));
+    dv.mu[m] = 0.f;
+    dv.eps[m] = 1.f;
+  }
+}
+
+__global__ void k_ctl_reset(const __grid_constant__ Dev dv, float eps_tol, int max_sweeps, int fixed_sweeps) {
+  Ctl *c = dv.ctl;
+  c->K = 0.0; c->Ex = 0.0; c->Jav = 0.0; c->Ex_sum = 0.0; c->Ex_cnt = 0; c->n = 0; c->sweeps_total = 0;
+  c->sweeps = 0; c->done = 0; c->xbuf = 0; c->status = 0; c->sweeps_last = 0; c->resid_last = 0.f;
+  c->ticket = 0u; c->ticket2 = 0u;
+  c->eps_tol = eps_tol; c->max_sweeps = max_sweeps; c->fixed_sweeps = fixed_sweeps;
+  c->sched_n = 0; c->sched_pos = 0; c->Jext = 0.0; c->Bx = 0.0; c->Bz = 0.0;
+}
+__global__ void k_ctl_solver(const __grid_constant__ Dev dv, float eps_tol, int max_sweeps, int fixed_sweeps) {
+  dv.ctl->eps_tol = eps_tol; dv.ctl->max_sweeps = max_sweeps; dv.ctl->fixed_sweeps = fixed_sweeps;
+}
+__global__ void k_ctl_sched(const __grid_constant__ Dev dv, int n) { dv.ctl->sched_n = n; dv.ctl->sched_pos = 0; }
+__global__ void k_ctl_state(const __grid_constant__ Dev dv, double K) { dv.ctl->K = K; dv.ctl->xbuf = 0; }
+
+// a1: the K-independent phase tables of the xz Landau gauge (Eq. 24a, 27):
+//   U_z(j) = exp(-i h_z B_x ybar_j),  Pi[i] = exp(i i h_x L_y B_z),  Pk[k] = exp(i k h_z L_y B_x),
+//   P_{i,k} = Pi[i] conj(Pk[k]).  fp64 trigonometry, fp32 tables.
+__global__ void k_set_field(const __grid_constant__ Dev dv, double Bx, double Bz, double Jext) {
+  const int tid = threadIdx.x, nth = blockDim.x;
+  if (tid == 0) {
+    dv.ctl->Bx = Bx; dv.ctl->Bz = Bz; dv.ctl->Jext = Jext; dv.ctl->Ex_sum = 0.0; dv.ctl->Ex_cnt = 0;
+  }
+  double s, c;
+  for (int j = tid; j < dv.ny; j += nth) {
+    const double ybar = j * dv.hy - 0.5 * dv.Ly;
+    sincos(-dv.hz * Bx * ybar, &s, &c);
+    dv.Uz[j] = make_float2((float)c, (float)s);
+  }
+  for (int i = tid; i < dv.nx; i += nth) {
+    sincos((double)i * dv.hx * dv.Ly * Bz, &s, &c);
+    dv.Pi[i] = make_float2((float)c, (float)s);
+  }
+  for (int k = tid; k < dv.nz; k += nth) {
+    sincos((double)k * dv.hz * dv.Ly * Bx, &s, &c);
+    dv.Pk[k] = make_float2((float)c, (float)s);
+  }
+}
+
+__global__ void k_fill_f32(float *p, long long n, float v) {
+  for (long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x; m < n; m += (long long)gridDim.x * blockDim.x) p[m] = v;
+}
+
+// a0: one CTA per sphere writes eps_in inside its bounding box (idempotent scatter; never N x n_s).
+// Inside test (P:245, 511 (i), S19): d_x^2 + d_y^2 + d_z^2 <= r^2 with d the minimum-image distance on
+// periodic axes, evaluated in fp64 with every product and sum rounded separately (no contraction), so
+// the mask does not depend on how the compiler fuses operations.
+__global__ void __launch_bounds__(128) k_spheres(const __grid_constant__ Dev dv, const float4 *__restrict__ sph, float eps_in) {
+  const float4 s = sph[blockIdx.x];
+  const int n[3] = {dv.nx, dv.ny, dv.nz};
+  const int bc[3] = {dv.bcx, dv.bcy, dv.bcz};
+  const double h[3] = {dv.hx, dv.hy, dv.hz};
+  const double cc[3] = {(double)s.x, (double)s.y, (double)s.z};
+  const double r = (double)s.w;
+  const double r2 = __dmul_rn(r, r);
+  int lo[3], ext[3];
+  for (int a = 0; a < 3; ++a) {
+    int l = (int)floor((cc[a] - r) / h[a]) - 1, u = (int)ceil((cc[a] + r) / h[a]) + 1;
+    if (bc[a] == 1) { l = max(l, 0); u = min(u, n[a] - 1); }
+    else if (u - l + 1 >= n[a]) { l = 0; u = n[a] - 1; }
+    lo[a] = l;
+    ext[a] = max(0, u - l + 1);
+  }
+  const long long cnt = (long long)ext[0] * ext[1] * ext[2];
+  for (long long t = threadIdx.x; t < cnt; t += blockDim.x) {
+    const int qx = (int)(t % ext[0]);
+    const long long rest = t / ext[0];
+    const int qy = (int)(rest % ext[1]), qz = (int)(rest / ext[1]);
+    const int q[3] = {lo[0] + qx, lo[1] + qy, lo[2] + qz};
+    int idx[3];
+    double d2[3];
+    for (int a = 0; a < 3; ++a) {
+      int ii = q[a] % n[a];
+      if (ii < 0) ii += n[a];
+      idx[a] = ii;
+      double d = __dsub_rn(__dmul_rn((double)ii, h[a]), cc[a]);
+      if (bc[a] == 0) {
+        const double L = __dmul_rn((double)n[a], h[a]);
+        d = __dsub_rn(d, __dmul_rn(L, rint(__ddiv_rn(d, L))));
+      }
+      d2[a] = __dmul_rn(d, d);
+    }
+    if (__dadd_rn(__dadd_rn(d2[0], d2[1]), d2[2]) <= r2)
+      dv.eps[idx[0] + (long long)dv.nx * (idx[1] + (long long)dv.ny * idx[2])] = eps_in;
+  }
+}
+
+// zeta_m of step `step` (Eq. 39; S11) exactly as the init kernel draws it.
+__global__ void k_noise(const __grid_constant__ Dev dv, long long step, float2 *out) {
+  for (long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x; m < dv.N; m += (long long)gridDim.x * blockDim.x) {
+    const PhiloxOut p = philox4x32_10((uint32_t)m, (uint32_t)((unsigned long long)m >> 32), (uint32_t)step, 0u, dv.seed_lo, dv.seed_hi);
+    out[m] = make_float2(dv.zeta_max * u32_to_pm1(p.x0), dv.zeta_max * u32_to_pm1(p.x1));
+  }
+}
+
+// a8: observables.  Per-CTA fp64 partial sums of
+//   [0] sum |psi|^2   [1] sum w (-eps |psi|^2 + |psi|^4/2)   [2] sum_alpha c_alpha sum_links w_link |S+ psi - psi|^2
+//   [3] sum of rounded plaquette windings
+// Free energy and winding definitions: DESIGN.md "Observables" (the paper only names F_GL).
+__device__ __forceinline__ float face_w(int idx, int n, int open) { return (open && (idx == 0 || idx == n - 1)) ? 0.5f : 1.f; }
+
+__global__ void __launch_bounds__(256) k_obs_partial(const __grid_constant__ Dev dv) {
+  const float2 *__restrict__ x = dv.psi[dv.ctl->xbuf];
+  const int nx = dv.nx, ny = dv.ny, nz = dv.nz;
+  const float twopi = 6.283185307179586f;
+  const float flux = (float)(dv.ctl->Bz * dv.hx * dv.hy);
+  double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+  for (long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x; m < dv.N; m += (long long)gridDim.x * blockDim.x) {
+    const int i = (int)(m % nx);
+    const long long row = m / nx;
+    const int j = (int)(row % ny), k = (int)(row / ny);
+    const float2 c = x[m];
+    const float wx = face_w(i, nx, dv.bcx), wy = face_w(j, ny, dv.bcy), wz = face_w(k, nz, dv.bcz);
+    const float ab = c.x * c.x + c.y * c.y;
+    a0 += ab;
+    a1 += (double)(wx * wy * wz * (-dv.eps[m] * ab + 0.5f * ab * ab));
+    const int ip = (i + 1 == nx) ? 0 : i + 1, jp = (j + 1 == ny) ? 0 : j + 1, kp = (k + 1 == nz) ? 0 : k + 1;
+    const bool hasx = dv.bcx == 0 || i + 1 < nx, hasy = dv.bcy == 0 || j + 1 < ny, hasz = dv.bcz == 0 || k + 1 < nz;
+    const long long base = (long long)nx * ((long long)ny * k);
+    const float2 Pk = dv.Pk[k];
+    // forward neighbours with their link variables
+    const float2 e = cmul(dv.Ux[j], x[base + (long long)nx * j + ip]);
+    float2 nn = x[base + (long long)nx * jp + i];
+    if (dv.bcy == 0 && j + 1 == ny) nn = cmulc(cmulc(Pk, dv.Pi[i]), nn);          // conj(P_{i,k}) psi_{i,0,k}
+    const float2 t = cmul(dv.Uz[j], x[(long long)nx * ((long long)ny * kp + j) + i]);
+    float g = 0.f;
+    if (hasx) g += dv.cx * wy * wz * ((e.x - c.x) * (e.x - c.x) + (e.y - c.y) * (e.y - c.y));
+    if (hasy) g += dv.cy * wx * wz * ((nn.x - c.x) * (nn.x - c.x) + (nn.y - c.y) * (nn.y - c.y));
+    if (hasz) g += dv.cz * wx * wy * ((t.x - c.x) * (t.x - c.x) + (t.y - c.y) * (t.y - c.y));
+    a2 += (double)g;
+    if (hasx && hasy) {
+      // winding of the z-plaquette with corner (i, j):  g_x(i,j) + g_y(i+1,j) - g_x(i,j+1) - g_y(i,j) + B_z h_x h_y
+      const float2 ce = x[base + (long long)nx * j + ip];                            // psi(i+1, j)
+      const float2 cn = x[base + (long long)nx * jp + i];                            // psi(i, j+1)
+      float2 cne = x[base + (long long)nx * jp + ip];                                // psi(i+1, j+1)
+      const int ipp = (ip + 1 == nx) ? 0 : ip + 1;
+      (void)ipp;
+      const float2 gx0 = cmulc(c, e);                                                // psi* U_x(j) psi(i+1,j)
+      const float2 gx1 = cmulc(cn, cmul(dv.Ux[jp], cne));                            // at row j+1 (its own U_x)
+      const float2 gy0 = cmulc(c, nn);                                               // psi* S+_y psi at (i,j)
+      float2 ney = cne;
+      if (dv.bcy == 0 && j + 1 == ny) ney = cmulc(cmulc(Pk, dv.Pi[ip]), cne);        // jump at column i+1
+      const float2 gy1 = cmulc(ce, ney);
+      const float circ = atan2f(gx0.y, gx0.x) + atan2f(gy1.y, gy1.x) - atan2f(gx1.y, gx1.x) - atan2f(gy0.y, gy0.x);
+      a3 += (double)rintf((circ + flux) / twopi);
+    }
+  }
+  __shared__ double sh[4][8];
+  for (int o = 16; o > 0; o >>= 1) {
+    a0 += __shfl_down_sync(0xffffffffu, a0, o);
+    a1 += __shfl_down_sync(0xffffffffu, a1, o);
+    a2 += __shfl_down_sync(0xffffffffu, a2, o);
+    a3 += __shfl_down_sync(0xffffffffu, a3, o);
+  }
+  if ((threadIdx.x & 31) == 0) {
+    sh[0][threadIdx.x >> 5] = a0; sh[1][threadIdx.x >> 5] = a1; sh[2][threadIdx.x >> 5] = a2; sh[3][threadIdx.x >> 5] = a3;
+  }
+  __syncthreads();
+  if (threadIdx.x < 4) {
+    double s = 0.0;
+    for (int w = 0; w < 8; ++w) s += sh[threadIdx.x][w];
+    dv.part[(size_t)threadIdx.x * TDGL_NPART + blockIdx.x] = s;
+  }
+}
+
+__global__ void k_obs_final(const __grid_constant__ Dev dv, int npart) {
+  __shared__ double sh[256];
+  for (int q = 0; q < 4; ++q) {
+    double s = 0.0;
+    for (int p = threadIdx.x; p < npart; p += 256) s += dv.part[(size_t)q * TDGL_NPART + p];
+    sh[threadIdx.x] = s;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+      if (threadIdx.x < o) sh[threadIdx.x] += sh[threadIdx.x + o];
+      __syncthreads();
+    }
+    if (threadIdx.x == 0) dv.ctl->obs[q] = sh[0];
+    __syncthreads();
+  }
+}
+
+// host-side launchers
+static unsigned grid_for(long long n, int block, int cap) {
+  long long g = (n + block - 1) / block;
+  return (unsigned)(g < 1 ? 1 : (g > cap ? cap : g));
+}
+void launch_init_state(const Dev &dv, float amp, cudaStream_t st) { k_init_state<<<grid_for(dv.N, 256, 148 * 16), 256, 0, st>>>(dv, amp); }
+void launch_ctl_reset(const Dev &dv, float tol, int maxs, int fixed, cudaStream_t st) { k_ctl_reset<<<1, 1, 0, st>>>(dv, tol, maxs, fixed); }
+void launch_ctl_solver(const Dev &dv, float tol, int maxs, int fixed, cudaStream_t st) { k_ctl_solver<<<1, 1, 0, st>>>(dv, tol, maxs, fixed); }
+void launch_ctl_sched(const Dev &dv, int n, cudaStream_t st) { k_ctl_sched<<<1, 1, 0, st>>>(dv, n); }
+void launch_ctl_state(const Dev &dv, double K, cudaStream_t st) { k_ctl_state<<<1, 1, 0, st>>>(dv, K); }
+void launch_set_field(const Dev &dv, double Bx, double Bz, double J, cudaStream_t st) { k_set_field<<<1, 256, 0, st>>>(dv, Bx, Bz, J); }
+void launch_fill(float *p, long long n, float v, cudaStream_t st) { k_fill_f32<<<grid_for(n, 256, 148 * 16), 256, 0, st>>>(p, n, v); }
+void launch_spheres(const Dev &dv, const float4 *sph, long long n, float eps_in, cudaStream_t st) {
+  for (long long off = 0; off < n; off += 1 << 20) {
+    const unsigned g = (unsigned)((n - off) < (1 << 20) ? (n - off) : (1 << 20));
+    k_spheres<<<g, 128, 0, st>>>(dv, sph + off, eps_in);
+  }
+}
+void launch_noise(const Dev &dv, long long step, float2 *out, cudaStream_t st) { k_noise<<<grid_for(dv.N, 256, 148 * 16), 256, 0, st>>>(dv, step, out); }
+int launch_obs(const Dev &dv, cudaStream_t st) {
+  const int nb = (int)grid_for(dv.N, 256, TDGL_NPART);
+  k_obs_partial<<<nb, 256, 0, st>>>(dv);
+  k_obs_final<<<1, 256, 0, st>>>(dv, nb);
+  return 2;
+}

@@ -1,0 +1,506 @@
+// C ABI of libtdgl (include/tdgl.h): parameter validation, workspace carving, the per-step launch
+// sequence (host loop or CUDA graph with a WHILE node around the Jacobi sweep), read-back.
+#include "../../include/tdgl.h"
+#include "tdgl_dev.cuh"
+#include <cmath>
+#include <cstring>
+#include <new>
+#include <vector>
+
+// launchers defined in the kernel files
+void launch_march(int mode, const Dev &dv, dim3 grid, dim3 block, size_t smem, cudaStream_t st);
+size_t march_smem_bytes(dim3 block);
+cudaError_t march_configure(size_t smem);
+void launch_jav(const Dev &dv, int nblocks, cudaStream_t st);
+void launch_step_begin(const Dev &dv, cudaStream_t st);
+void launch_step_finish(const Dev &dv, int npart, cudaStream_t st);
+cudaError_t poisson_configure(int nx, int ny, int nz);
+void launch_build_tables(float *lam, float2 *tw, double *tab, int n, int open, double c, cudaStream_t st);
+int poisson_solve(const Dev &dv, float *data, bool thomas_open_z, cudaStream_t st);
+void launch_init_state(const Dev &dv, float amp, cudaStream_t st);
+void launch_ctl_reset(const Dev &dv, float tol, int maxs, int fixed, cudaStream_t st);
+void launch_ctl_solver(const Dev &dv, float tol, int maxs, int fixed, cudaStream_t st);
+void launch_ctl_sched(const Dev &dv, int n, cudaStream_t st);
+void launch_ctl_state(const Dev &dv, double K, cudaStream_t st);
+void launch_set_field(const Dev &dv, double Bx, double Bz, double J, cudaStream_t st);
+void launch_fill(float *p, long long n, float v, cudaStream_t st);
+void launch_spheres(const Dev &dv, const float4 *sph, long long n, float eps_in, cudaStream_t st);
+void launch_noise(const Dev &dv, long long step, float2 *out, cudaStream_t st);
+int launch_obs(const Dev &dv, cudaStream_t st);
+
+#define MODE_SWEEP 0
+#define MODE_INIT 1
+#define MODE_RHO 2
+
+struct tdgl {
+  tdgl_params p;
+  Dev dv;
+  cudaStream_t stream;
+  dim3 mgrid, mblock;
+  size_t msmem;
+  int jav_blocks;
+  int last_cuda;
+  int64_t launches;            // host-counted kernel launches (graph launches are counted from the log)
+  int64_t graph_steps;
+  int fixed_per_step;          // kernels per step apart from the plain sweeps
+  double Bx_eff, Bz_eff;
+  // graph mode
+  bool use_graph;
+  cudaGraph_t graph;
+  cudaGraphExec_t exec;
+  cudaStream_t cap_stream;
+  // host loop
+  int *h_flag;                 // pinned: [0] done, [1] sweeps
+  int pred_sweeps;
+  // sweep timing
+  bool timing;
+  double t_ms;
+  int64_t t_launches;
+  cudaEvent_t ev0, ev1;
+};
+
+static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+static bool params_ok(const tdgl_params *p) {
+  if (!p || p->struct_size != sizeof(tdgl_params)) return false;
+  if (p->nx < 2 || p->ny < 2 || p->nz < 2 || (p->nx & 1)) return false;
+  if ((long long)p->nx * p->ny * p->nz > (1ll << 40)) return false;
+  if (!(p->hx > 0.f) || !(p->hy > 0.f) || !(p->hz > 0.f) || !(p->dt > 0.f) || !(p->u > 0.f) || !(p->g > 0.f)) return false;
+  for (int a = 0; a < 3; ++a)
+    if (p->bc[a] != TDGL_BC_PERIODIC && p->bc[a] != TDGL_BC_OPEN) return false;
+  if (!(p->eps_tol >= 0.f) || p->max_sweeps < 1 || p->max_sweeps > TDGL_MAX_RESID_SLOTS || p->fixed_sweeps < 0 ||
+      p->fixed_sweeps > TDGL_MAX_RESID_SLOTS) return false;
+  if (!(p->temperature >= 0.f)) return false;
+  return true;
+}
+
+// workspace carving; with base == nullptr only the size is computed
+static size_t carve(const tdgl_params *p, char *base, Dev *dv) {
+  const size_t N = (size_t)p->nx * p->ny * p->nz;
+  size_t off = 0;
+  auto take = [&](size_t bytes) { char *q = base ? base + off : nullptr; off = align_up(off + bytes, 256); return q; };
+  char *q;
+  q = take(sizeof(Ctl)); if (dv) dv->ctl = (Ctl *)q;
+  q = take(p->ny * sizeof(float2)); if (dv) dv->Ux = (float2 *)q;
+  q = take(p->ny * sizeof(float2)); if (dv) dv->Uz = (float2 *)q;
+  q = take(p->nx * sizeof(float2)); if (dv) dv->Pi = (float2 *)q;
+  q = take(p->nz * sizeof(float2)); if (dv) dv->Pk = (float2 *)q;
+  const int ns[3] = {p->nx, p->ny, p->nz};
+  for (int a = 0; a < 3; ++a) {
+    q = take(ns[a] * sizeof(float)); if (dv) dv->lam[a] = (float *)q;
+    q = take(ns[a] * sizeof(float2)); if (dv) dv->tw[a] = (float2 *)q;
+    q = take(2 * (size_t)ns[a] * sizeof(double)); if (dv) dv->tab[a] = (double *)q;
+  }
+  q = take((size_t)TDGL_NPART * 4 * sizeof(double)); if (dv) dv->part = (double *)q;
+  q = take(TDGL_LOGCAP * sizeof(int)); if (dv) dv->sweep_log = (int *)q;
+  q = take(TDGL_LOGCAP * sizeof(float)); if (dv) dv->resid_log = (float *)q;
+  q = take(TDGL_LOGCAP * sizeof(int)); if (dv) dv->sched = (int *)q;
+  q = take(N * sizeof(float2)); if (dv) dv->psi[0] = (float2 *)q;
+  q = take(N * sizeof(float2)); if (dv) dv->psi[1] = (float2 *)q;
+  q = take(N * sizeof(float2)); if (dv) dv->b = (float2 *)q;
+  q = take(N * sizeof(float2)); if (dv) dv->d = (float2 *)q;
+  q = take(N * sizeof(float)); if (dv) dv->mu = (float *)q;
+  q = take(N * sizeof(float)); if (dv) dv->eps = (float *)q;
+  q = take(N * sizeof(float)); if (dv) dv->scratch = (float *)q;
+  return off;
+}
+
+static int cuda_fail(tdgl_t *h, cudaError_t e) {
+  if (h) h->last_cuda = (int)e;
+  return TDGL_ECUDA;
+}
+#define CK(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(h, e_); } while (0)
+#define CKL() do { cudaError_t e_ = cudaGetLastError(); if (e_ != cudaSuccess) return cuda_fail(h, e_); } while (0)
+
+extern "C" uint64_t tdgl_workspace_bytes(const tdgl_params *p) {
+  if (!params_ok(p)) return 0;
+  return (uint64_t)carve(p, nullptr, nullptr);
+}
+
+// the kernels of one step after the psi solve: J_av + K (a5), rho (a6), mu (a7)
+static int enqueue_after_solve(tdgl_t *h, cudaStream_t st) {
+  int n = 0;
+  const bool kact = h->dv.solve_mu && h->dv.bcx == 0;
+  if (kact) { launch_jav(h->dv, h->jav_blocks, st); ++n; }
+  launch_step_finish(h->dv, h->jav_blocks, st); ++n;
+  if (h->dv.solve_mu) {
+    launch_march(MODE_RHO, h->dv, h->mgrid, h->mblock, h->msmem, st); ++n;
+    n += poisson_solve(h->dv, h->dv.mu, true, st);
+  }
+  return n;
+}
+
+static int build_graph(tdgl_t *h) {
+  CK(cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking));
+  CK(cudaGraphCreate(&h->graph, 0));
+  cudaGraphConditionalHandle handle;
+  CK(cudaGraphConditionalHandleCreate(&handle, h->graph, 0, 0));
+  h->dv.cond_handle = (unsigned long long)handle;
+  h->dv.use_cond = 1;
+  cudaStream_t cs = h->cap_stream;
+  // segment A: begin + fused init/first sweep
+  CK(cudaStreamBeginCaptureToGraph(cs, h->graph, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal));
+  launch_step_begin(h->dv, cs);
+  launch_march(MODE_INIT, h->dv, h->mgrid, h->mblock, h->msmem, cs);
+  cudaStreamCaptureStatus status;
+  const cudaGraphNode_t *deps = nullptr;
+  size_t ndeps = 0;
+  CK(cudaStreamGetCaptureInfo(cs, &status, nullptr, nullptr, &deps, &ndeps));
+  std::vector<cudaGraphNode_t> tail(deps, deps + ndeps);
+  cudaGraph_t g2;
+  CK(cudaStreamEndCapture(cs, &g2));
+  // WHILE node: one plain sweep per iteration; the sweep's last CTA sets the condition
+  cudaGraphNodeParams np = {cudaGraphNodeTypeConditional};
+  np.type = cudaGraphNodeTypeConditional;
+  np.conditional.handle = handle;
+  np.conditional.type = cudaGraphCondTypeWhile;
+  np.conditional.size = 1;
+  cudaGraphNode_t cond;
+  CK(cudaGraphAddNode(&cond, h->graph, tail.data(), tail.size(), &np));
+  cudaGraph_t body = np.conditional.phGraph_out[0];
+  CK(cudaStreamBeginCaptureToGraph(cs, body, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal));
+  launch_march(MODE_SWEEP, h->dv, h->mgrid, h->mblock, h->msmem, cs);
+  CK(cudaStreamEndCapture(cs, &g2));
+  // segment B: everything after the psi solve
+  CK(cudaStreamBeginCaptureToGraph(cs, h->graph, &cond, nullptr, 1, cudaStreamCaptureModeThreadLocal));
+  h->fixed_per_step = 2 + enqueue_after_solve(h, cs);
+  CK(cudaStreamEndCapture(cs, &g2));
+  CK(cudaGraphInstantiate(&h->exec, h->graph, 0));
+  return TDGL_OK;
+}
+
+extern "C" int tdgl_create(const tdgl_params *p, tdgl_t **out) {
+  if (!out) return TDGL_EINVAL;
+  *out = nullptr;
+  if (!params_ok(p)) return TDGL_EINVAL;
+  const size_t need = carve(p, nullptr, nullptr);
+  if (!p->workspace_dev || ((uintptr_t)p->workspace_dev & 255) || p->workspace_bytes < need) return TDGL_ENOMEM;
+  tdgl_t *h = new (std::nothrow) tdgl();
+  if (!h) return TDGL_ENOMEM;
+  memset(h, 0, sizeof(*h));
+  h->p = *p;
+  h->stream = (cudaStream_t)p->stream;
+  Dev &dv = h->dv;
+  memset(&dv, 0, sizeof(dv));
+  carve(p, (char *)p->workspace_dev, &dv);
+  dv.nx = p->nx; dv.ny = p->ny; dv.nz = p->nz;
+  dv.bcx = p->bc[0]; dv.bcy = p->bc[1]; dv.bcz = p->bc[2];
+  dv.N = (long long)p->nx * p->ny * p->nz;
+  dv.hx = p->hx; dv.hy = p->hy; dv.hz = p->hz; dv.dt = p->dt;
+  const double cx = 1.0 / (dv.hx * dv.hx), cy = 1.0 / (dv.hy * dv.hy), cz = 1.0 / ((double)p->g * p->g * dv.hz * dv.hz);
+  dv.cx = (float)cx; dv.cy = (float)cy; dv.cz = (float)cz;
+  dv.csum2 = (float)(2.0 * (cx + cy + cz));
+  dv.ht2 = (float)(0.5 * dv.dt / (double)p->u);
+  dv.u = p->u;
+  dv.Lx = (p->nx - (p->bc[0] ? 1 : 0)) * dv.hx;
+  dv.Ly = (p->ny - (p->bc[1] ? 1 : 0)) * dv.hy;
+  dv.Lz = (p->nz - (p->bc[2] ? 1 : 0)) * dv.hz;
+  // Eq. (39), S12: zeta_max = (3 T u / (2 dt hx hy hz))^{1/2}
+  dv.zeta_max = p->temperature > 0.f
+                    ? (float)std::sqrt(3.0 * (double)p->temperature * (double)p->u / (2.0 * dv.dt * dv.hx * dv.hy * dv.hz))
+                    : 0.f;
+  dv.seed_lo = (unsigned)(p->seed & 0xffffffffull);
+  dv.seed_hi = (unsigned)(p->seed >> 32);
+  dv.solve_mu = (p->flags & TDGL_FLAG_SOLVE_MU) ? 1 : 0;
+
+  // launch geometry of the marching kernels: 512 threads, bx thread columns of two sites, by rows
+  int bx = 64;
+  while (bx > 16 && bx * 2 > p->nx) bx >>= 1;
+  int by = 512 / bx;
+  while (by > 4 && by / 2 >= p->ny) by >>= 1;
+  h->mblock = dim3(bx, by, 1);
+  const unsigned gx = (p->nx + 2 * bx - 1) / (2 * bx), gy = (p->ny + by - 1) / by;
+  // z chunks: enough CTAs for ~4 waves of 2 CTAs/SM, chunks of at least 8 planes
+  int zc = p->nz;
+  const long long want = 148ll * 2 * 4;
+  while (zc > 8 && (long long)gx * gy * ((p->nz + zc - 1) / zc) < want) zc = (zc + 1) / 2;
+  dv.zc = zc;
+  h->mgrid = dim3(gx, gy, (p->nz + zc - 1) / zc);
+  h->msmem = march_smem_bytes(h->mblock);
+  {
+    long long nb = (dv.N / 2 + 255) / 256;
+    h->jav_blocks = (int)(nb < 1 ? 1 : (nb > TDGL_NPART ? TDGL_NPART : nb));
+  }
+  h->pred_sweeps = 1;
+  CK(march_configure(h->msmem));
+  CK(poisson_configure(p->nx, p->ny, p->nz));
+  CK(cudaMallocHost((void **)&h->h_flag, 64));
+  CK(cudaEventCreate(&h->ev0));
+  CK(cudaEventCreate(&h->ev1));
+
+  cudaStream_t st = h->stream;
+  launch_ctl_reset(dv, p->eps_tol, p->max_sweeps, p->fixed_sweeps, st);
+  const int ns[3] = {p->nx, p->ny, p->nz};
+  const double cs[3] = {cx, cy, cz};
+  for (int a = 0; a < 3; ++a) launch_build_tables(dv.lam[a], dv.tw[a], dv.tab[a], ns[a], p->bc[a], cs[a], st);
+  launch_init_state(dv, p->init_amp, st);
+  launch_set_field(dv, 0.0, 0.0, 0.0, st);
+  launch_step_begin(dv, st);
+  h->launches += 7;
+  CKL();
+  h->use_graph = !(p->flags & TDGL_FLAG_HOST_LOOP);
+  if (h->use_graph) {
+    int rc = build_graph(h);
+    if (rc != TDGL_OK) { int lc = h->last_cuda; tdgl_destroy(h); (void)lc; return rc; }
+  }
+  *out = h;
+  return TDGL_OK;
+}
+
+extern "C" int tdgl_destroy(tdgl_t *h) {
+  if (!h) return TDGL_EINVAL;
+  cudaStreamSynchronize(h->stream);
+  if (h->exec) cudaGraphExecDestroy(h->exec);
+  if (h->graph) cudaGraphDestroy(h->graph);
+  if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
+  if (h->h_flag) cudaFreeHost(h->h_flag);
+  if (h->ev0) cudaEventDestroy(h->ev0);
+  if (h->ev1) cudaEventDestroy(h->ev1);
+  delete h;
+  return TDGL_OK;
+}
+
+extern "C" int tdgl_set_pinning(tdgl_t *h, const tdgl_sphere *sph, int64_t n, float eps_in, float eps_out) {
+  if (!h || n < 0 || (n > 0 && !sph) || n > h->dv.N / 4) return TDGL_EINVAL;
+  launch_fill(h->dv.eps, h->dv.N, eps_out, h->stream);
+  h->launches += 1;
+  if (n > 0) {
+    CK(cudaMemcpyAsync(h->dv.scratch, sph, (size_t)n * sizeof(tdgl_sphere), cudaMemcpyHostToDevice, h->stream));
+    CK(cudaStreamSynchronize(h->stream));       // the host list may be freed on return
+    launch_spheres(h->dv, (const float4 *)h->dv.scratch, n, eps_in, h->stream);
+    h->launches += (n + (1 << 20) - 1) >> 20;
+  }
+  CKL();
+  return TDGL_OK;
+}
+
+extern "C" int tdgl_set_field_current(tdgl_t *h, float Bx, float By, float Bz, float Jx) {
+  if (!h) return TDGL_EINVAL;
+  if (By != 0.f) return TDGL_EINCOMPAT;
+  if (Jx != 0.f && h->dv.bcx == 1) return TDGL_EINCOMPAT;
+  double bx = Bx, bz = Bz;
+  const double twopi = 2.0 * 3.14159265358979323846;
+  if (h->dv.bcx == 0 && h->dv.bcy == 0) {
+    const double a = h->dv.Lx * h->dv.Ly;
+    const double q = std::nearbyint(bz * a / twopi);
+    bz = twopi * q / a;
+  }
+  if (h->dv.bcy == 0 && h->dv.bcz == 0) {
+    const double a = h->dv.Ly * h->dv.Lz;
+    const double q = std::nearbyint(bx * a / twopi);
+    bx = twopi * q / a;
+  }
+  h->Bx_eff = bx;
+  h->Bz_eff = bz;
+  launch_set_field(h->dv, bx, bz, (double)Jx, h->stream);
+  launch_step_begin(h->dv, h->stream);           // refresh U_x(j) for the new field
+  h->launches += 2;
+  CKL();
+  return TDGL_OK;
+}
+
+static int step_host_loop(tdgl_t *h) {
+  cudaStream_t st = h->stream;
+  const Dev &dv = h->dv;
+  launch_step_begin(dv, st);
+  launch_march(MODE_INIT, dv, h->mgrid, h->mblock, h->msmem, st);
+  h->launches += 2;
+  int launched = 1;
+  const int cap = TDGL_MAX_RESID_SLOTS;
+  for (;;) {
+    // speculative sweeps (they return at once when the solve is already done), then one flag read
+    int burst = h->timing ? 0 : h->pred_sweeps - launched;
+    for (int s = 0; s < burst && launched < cap; ++s) {
+      launch_march(MODE_SWEEP, dv, h->mgrid, h->mblock, h->msmem, st);
+      ++launched; ++h->launches;
+    }
+    CK(cudaMemcpyAsync(h->h_flag, &dv.ctl->sweeps, 2 * sizeof(int), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    if (h->h_flag[1] || launched >= cap) break;
+    if (h->timing) CK(cudaEventRecord(h->ev0, st));
+    launch_march(MODE_SWEEP, dv, h->mgrid, h->mblock, h->msmem, st);
+    ++launched; ++h->launches;
+    if (h->timing) {
+      CK(cudaEventRecord(h->ev1, st));
+      CK(cudaEventSynchronize(h->ev1));
+      float ms = 0.f;
+      CK(cudaEventElapsedTime(&ms, h->ev0, h->ev1));
+      h->t_ms += ms;
+      h->t_launches += 1;
+    }
+  }
+  h->pred_sweeps = h->h_flag[0] < 1 ? 1 : h->h_flag[0];
+  h->launches += enqueue_after_solve(h, st);
+  CKL();
+  return TDGL_OK;
+}
+
+extern "C" int tdgl_step(tdgl_t *h, int32_t nsteps) {
+  if (!h || nsteps < 0) return TDGL_EINVAL;
+  for (int s = 0; s < nsteps; ++s) {
+    if (h->use_graph) {
+      CK(cudaGraphLaunch(h->exec, h->stream));
+      h->graph_steps += 1;
+    } else {
+      int rc = step_host_loop(h);
+      if (rc != TDGL_OK) return rc;
+    }
+  }
+  return TDGL_OK;
+}
+
+extern "C" int tdgl_get_psi_mu(tdgl_t *h, void *psi_dev, void *mu_dev) {
+  if (!h) return TDGL_EINVAL;
+  if (psi_dev) {
+    // which buffer holds psi is device state: read it (4 bytes) before the copy
+    CK(cudaMemcpyAsync(h->h_flag + 4, &h->dv.ctl->xbuf, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
+    CK(cudaMemcpyAsync(psi_dev, h->dv.psi[h->h_flag[4] & 1], (size_t)h->dv.N * sizeof(float2), cudaMemcpyDeviceToDevice, h->stream));
+  }
+  if (mu_dev) CK(cudaMemcpyAsync(mu_dev, h->dv.mu, (size_t)h->dv.N * sizeof(float), cudaMemcpyDeviceToDevice, h->stream));
+  return TDGL_OK;
+}
+
+extern "C" int tdgl_observables(tdgl_t *h, tdgl_obs *out) {
+  if (!h || !out) return TDGL_EINVAL;
+  h->launches += launch_obs(h->dv, h->stream);
+  CKL();
+  Ctl c;
+  CK(cudaMemcpyAsync(&c, h->dv.ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, h->stream));
+  CK(cudaStreamSynchronize(h->stream));
+  memset(out, 0, sizeof(*out));
+  out->t = (double)c.n * h->dv.dt;
+  out->K = c.K; out->Ex = c.Ex; out->Jav = c.Jav;
+  out->Ex_mean = c.Ex_cnt > 0 ? c.Ex_sum / (double)c.Ex_cnt : 0.0;
+  out->mean_abs2 = c.obs[0] / (double)h->dv.N;
+  out->free_energy = (c.obs[1] + c.obs[2]) * h->dv.hx * h->dv.hy * h->dv.hz;
+  out->vortices_per_slice = c.obs[3] / (double)h->dv.nz;
+  out->max_resid2 = c.resid_last;
+  out->Bx_eff = (float)h->Bx_eff; out->Bz_eff = (float)h->Bz_eff;
+  out->steps = c.n; out->sweeps_total = c.sweeps_total; out->sweeps_last = c.sweeps_last;
+  out->status = c.status ? TDGL_WMAXSWEEPS : 0;
+  return c.status ? TDGL_WMAXSWEEPS : TDGL_OK;
+}
+
+extern "C" const char *tdgl_strerror(int code) {
+  switch (code) {
+    case TDGL_OK: return "ok";
+    case TDGL_EINVAL: return "invalid argument (size, mesh, boundary type, pointer or struct_size)";
+    case TDGL_ENOMEM: return "workspace too small or misaligned";
+    case TDGL_EINCOMPAT: return "incompatible request (open x with a current, or By != 0)";
+    case TDGL_ECUDA: return "CUDA runtime error";
+    case TDGL_WMAXSWEEPS: return "warning: Jacobi iteration hit max_sweeps";
+    default: return "unknown code";
+  }
+}
+extern "C" int tdgl_last_cuda_error(const tdgl_t *h) { return h ? h->last_cuda : 0; }
+
+extern "C" int tdgl_set_state(tdgl_t *h, const void *psi_dev, const void *mu_dev, double K) {
+  if (!h || !psi_dev) return TDGL_EINVAL;
+  CK(cudaMemcpyAsync(h->dv.psi[0], psi_dev, (size_t)h->dv.N * sizeof(float2), cudaMemcpyDeviceToDevice, h->stream));
+  if (mu_dev) CK(cudaMemcpyAsync(h->dv.mu, mu_dev, (size_t)h->dv.N * sizeof(float), cudaMemcpyDeviceToDevice, h->stream));
+  launch_ctl_state(h->dv, K, h->stream);
+  launch_step_begin(h->dv, h->stream);
+  h->launches += 2;
+  CKL();
+  return TDGL_OK;
+}
+
+extern "C" int tdgl_set_solver(tdgl_t *h, float eps_tol, int32_t max_sweeps, int32_t fixed_sweeps) {
+  if (!h || !(eps_tol >= 0.f) || max_sweeps < 1 || max_sweeps > TDGL_MAX_RESID_SLOTS || fixed_sweeps < 0 ||
+      fixed_sweeps > TDGL_MAX_RESID_SLOTS) return TDGL_EINVAL;
+  launch_ctl_solver(h->dv, eps_tol, max_sweeps, fixed_sweeps, h->stream);
+  h->launches += 1;
+  h->p.max_sweeps = max_sweeps;
+  CKL();
+  return TDGL_OK;
+}
+
+extern "C" int tdgl_set_sweep_schedule(tdgl_t *h, const int32_t *counts, int32_t n) {
+  if (!h || n < 0 || n > TDGL_LOGCAP || (n > 0 && !counts)) return TDGL_EINVAL;
+  for (int s = 0; s < n; ++s)
+    if (counts[s] < 1 || counts[s] > TDGL_MAX_RESID_SLOTS) return TDGL_EINVAL;
+  if (n > 0) {
+    CK(cudaMemcpyAsync(h->dv.sched, counts, (size_t)n * sizeof(int), cudaMemcpyHostToDevice, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
+  }
+  launch_ctl_sched(h->dv, n, h->stream);
+  h->launches += 1;
+  CKL();
+  return TDGL_OK;
+}
+
+extern "C" int tdgl_get_sweep_log(tdgl_t *h, int32_t *counts, float *resid2, int32_t n) {
+  if (!h || n < 0 || n > TDGL_LOGCAP) return TDGL_EINVAL;
+  long long steps = 0;
+  CK(cudaMemcpyAsync(&steps, &h->dv.ctl->n, sizeof(long long), cudaMemcpyDeviceToHost, h->stream));
+  CK(cudaStreamSynchronize(h->stream));
+  if (n > steps) return TDGL_EINVAL;
+  std::vector<int> lc(TDGL_LOGCAP);
+  std::vector<float> lr(TDGL_LOGCAP);
+  CK(cudaMemcpyAsync(lc.data(), h->dv.sweep_log, TDGL_LOGCAP * sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+  CK(cudaMemcpyAsync(lr.data(), h->dv.resid_log, TDGL_LOGCAP * sizeof(float), cudaMemcpyDeviceToHost, h->stream));
+  CK(cudaStreamSynchronize(h->stream));
+  for (int s = 0; s < n; ++s) {
+    const long long step = steps - n + s;
+    if (counts) counts[s] = lc[step % TDGL_LOGCAP];
+    if (resid2) resid2[s] = lr[step % TDGL_LOGCAP];
+  }
+  return TDGL_OK;
+}
+
+extern "C" int tdgl_get_eps(tdgl_t *h, void *eps_dev) {
+  if (!h || !eps_dev) return TDGL_EINVAL;
+  CK(cudaMemcpyAsync(eps_dev, h->dv.eps, (size_t)h->dv.N * sizeof(float), cudaMemcpyDeviceToDevice, h->stream));
+  return TDGL_OK;
+}
+
+extern "C" int tdgl_debug_noise(tdgl_t *h, int64_t step, void *zeta_dev) {
+  if (!h || !zeta_dev) return TDGL_EINVAL;
+  launch_noise(h->dv, step, (float2 *)zeta_dev, h->stream);
+  h->launches += 1;
+  CKL();
+  return TDGL_OK;
+}
+
+extern "C" int tdgl_debug_poisson(tdgl_t *h, const void *rho_dev, void *mu_dev) {
+  if (!h || !rho_dev || !mu_dev) return TDGL_EINVAL;
+  if (rho_dev != mu_dev)
+    CK(cudaMemcpyAsync(mu_dev, rho_dev, (size_t)h->dv.N * sizeof(float), cudaMemcpyDeviceToDevice, h->stream));
+  h->launches += poisson_solve(h->dv, (float *)mu_dev, true, h->stream);
+  CKL();
+  return TDGL_OK;
+}
+
+extern "C" int tdgl_debug_rho(tdgl_t *h, void *rho_dev) {
+  if (!h || !rho_dev) return TDGL_EINVAL;
+  Dev d2 = h->dv;
+  d2.mu = (float *)rho_dev;                       // the rho kernel writes where mu lives
+  launch_march(MODE_RHO, d2, h->mgrid, h->mblock, h->msmem, h->stream);
+  h->launches += 1;
+  CKL();
+  return TDGL_OK;
+}
+
+extern "C" int64_t tdgl_launch_count(const tdgl_t *h) {
+  if (!h) return 0;
+  int64_t n = h->launches;
+  if (h->use_graph && h->graph_steps > 0) {
+    long long tot = 0, steps = 0;
+    cudaStreamSynchronize(h->stream);
+    cudaMemcpy(&tot, &h->dv.ctl->sweeps_total, sizeof(long long), cudaMemcpyDeviceToHost);
+    cudaMemcpy(&steps, &h->dv.ctl->n, sizeof(long long), cudaMemcpyDeviceToHost);
+    // per graph step: fixed_per_step kernels (begin, init+sweep 1, ...) + the further sweeps
+    n += h->graph_steps * (int64_t)h->fixed_per_step + (tot - steps);
+  }
+  return n;
+}
+
+extern "C" int tdgl_sweep_timing(tdgl_t *h, int32_t enable, double *ms_total, int64_t *launches) {
+  if (!h) return TDGL_EINVAL;
+  if (ms_total) *ms_total = h->t_ms;
+  if (launches) *launches = h->t_launches;
+  h->timing = enable != 0;
+  if (enable) { h->t_ms = 0.0; h->t_launches = 0; }
+  return TDGL_OK;
+}

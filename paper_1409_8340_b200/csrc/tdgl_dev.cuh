@@ -1,0 +1,72 @@
+// Device-side view of one TDGL problem: grid constants, workspace pointers and the control block.
+// Shared by every kernel of libtdgl.  Citations: P:NNN = PAPER.md line, Sxx = DESIGN.md reading.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#define TDGL_LOGCAP 65536            // ring of per-step sweep counts / residuals
+#define TDGL_MAX_RESID_SLOTS 1024    // >= max_sweeps
+#define TDGL_NPART 2048              // partial sums of the two-stage fp64 reductions
+
+// Control block, resident in the workspace; written by kernels only (the host reads it back).
+struct Ctl {
+  double K;                 // gauge variable, Eq. (13)-(15)
+  double Ex, Jav;           // last step
+  double Ex_sum;            // running sum since set_field_current
+  long long Ex_cnt;
+  long long n;              // step index = Philox counter word 2 (S11)
+  long long sweeps_total;
+  int sweeps;               // sweeps done in the current step
+  int done;                 // psi solve of the current step finished
+  int xbuf;                 // which psi buffer holds the latest iterate
+  int status;               // latched TDGL_WMAXSWEEPS
+  int sweeps_last;
+  float resid_last;
+  unsigned int ticket;      // last-block election of the sweep kernel
+  unsigned int ticket2;     // ... of the reduction kernels
+  // solver controls (changed by tdgl_set_solver / tdgl_set_sweep_schedule)
+  float eps_tol;
+  int max_sweeps;
+  int fixed_sweeps;
+  int sched_n, sched_pos;   // prescribed per-step counts in sched[]
+  double Jext;
+  double Bx, Bz;            // effective field
+  unsigned int resid_bits[TDGL_MAX_RESID_SLOTS];   // max |r|^2 of sweep l as uint bits (>= 0 floats order like uints)
+  double obs[8];            // observables scratch
+};
+
+struct Dev {
+  int nx, ny, nz;
+  int bcx, bcy, bcz;        // 0 periodic, 1 open
+  long long N;
+  float cx, cy, cz;         // 1/hx^2, 1/hy^2, 1/(g hz)^2
+  float ht2;                // h_t / 2
+  float u;
+  float csum2;              // 2 (cx + cy + cz)
+  float zeta_max;           // Eq. (39); 0 = no noise
+  double hx, hy, hz, dt, Lx, Ly, Lz;
+  unsigned int seed_lo, seed_hi;
+  int solve_mu;
+  int zc;                   // planes per z-chunk of the marching kernels
+  // workspace
+  Ctl *ctl;
+  float2 *psi[2];
+  float2 *b, *d;
+  float *mu, *eps, *scratch;
+  float2 *Ux, *Uz;          // per-row link variables U_x(j), U_z(j)  (Eq. 27)
+  float2 *Pi, *Pk;          // quasi-periodic jump P_{i,k} = Pi[i] conj(Pk[k])
+  float *lam[3];            // eigenvalues of the 1-D operators per axis
+  float2 *tw[3];            // FFT twiddles exp(-2 pi i m/n) per axis (power-of-two periodic axes)
+  double *tab[3];           // generic transform tables: cas(2 pi m/n) or cos(pi m/(n-1))
+  double *part;             // TDGL_NPART*4 partial sums
+  int *sweep_log; float *resid_log; int *sched;
+  unsigned long long cond_handle;   // cudaGraphConditionalHandle of the WHILE node (graph mode)
+  int use_cond;
+};
+
+__device__ __forceinline__ float2 cmul(float2 a, float2 b) {
+  return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+}
+__device__ __forceinline__ float2 cmulc(float2 a, float2 b) {   // conj(a) * b
+  return make_float2(a.x * b.x + a.y * b.y, a.x * b.y - a.y * b.x);
+}

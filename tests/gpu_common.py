@@ -1,0 +1,52 @@
+"""Helpers shared by the `-m gpu` parity tests: build the oracle's Params and the CUDA Solver from the
+same seeded configuration (tdgl_inputs.py) and drive both."""
+from __future__ import annotations
+
+import numpy as np
+
+import tdgl_inputs as I
+from oracle import tdgl_oracle as O
+
+
+def f32(x: float) -> float:
+    """The fp32 value the C ABI receives, widened: the oracle is fed the very same number."""
+    return float(np.float32(x))
+
+
+def oracle_params(cfg: I.Config, eps_tol=1e-6, max_sweeps=100, solve_mu=True, temperature=None, hxyz=None, g=1.0):
+    hx, hy, hz = hxyz if hxyz is not None else (cfg.h, cfg.h, cfg.h)
+    return O.Params(cfg.nx, cfg.ny, cfg.nz, hx=f32(hx), hy=f32(hy), hz=f32(hz), dt=f32(cfg.dt), u=1.0, g=f32(g),
+                    bc=tuple(cfg.bc), eps_tol=f32(eps_tol), max_sweeps=max_sweeps,
+                    temperature=f32(cfg.temperature if temperature is None else temperature), seed=cfg.seed,
+                    solve_mu=solve_mu)
+
+
+def make_solver(cfg: I.Config, eps_tol=1e-6, max_sweeps=100, solve_mu=True, temperature=None, host_loop=False,
+                fixed_sweeps=0, hxyz=None, g=1.0):
+    from paper_1409_8340_b200 import Solver
+    return Solver(cfg.nx, cfg.ny, cfg.nz, bc=cfg.bc, h=cfg.h, dt=cfg.dt, g=g, eps_tol=eps_tol, max_sweeps=max_sweeps,
+                  fixed_sweeps=fixed_sweeps, temperature=cfg.temperature if temperature is None else temperature,
+                  seed=cfg.seed, init_amp=cfg.init_amp, solve_mu=solve_mu, host_loop=host_loop, hxyz=hxyz)
+
+
+def setup_pair(cfg: I.Config, psi0=None, mu0=None, K0=0.0, with_pinning=True, **kw):
+    """Returns (oracle params, oracle state, eps, (Bx, Bz) effective, solver) with identical inputs."""
+    import torch
+    p = oracle_params(cfg, **{k: v for k, v in kw.items() if k not in ("host_loop", "fixed_sweeps")})
+    s = make_solver(cfg, **kw)
+    spheres = I.sphere_list(cfg) if with_pinning else np.zeros((0, 4), np.float32)
+    eps = O.epsilon_from_spheres(p, spheres, cfg.eps_in, cfg.eps_out)
+    s.set_pinning(spheres, cfg.eps_in, cfg.eps_out)
+    bx_req, bz_req = cfg.requested_field()
+    Bx, Bz, _, _ = O.snap_field(p, f32(bx_req), f32(bz_req))
+    s.set_field_current(Bx=bx_req, Bz=bz_req, Jx=cfg.Jx)
+    if psi0 is None:
+        psi0 = I.initial_psi(cfg)
+    mu_np = np.zeros(p.shape, np.float32) if mu0 is None else mu0
+    st = O.State(psi=psi0.astype(np.complex128), mu=mu_np.astype(np.float64), K=float(K0))
+    s.set_state(torch.from_numpy(psi0), torch.from_numpy(mu_np), float(K0))
+    return p, st, eps, (Bx, Bz), s
+
+
+def rel_l2(a, b):
+    return float(np.linalg.norm((a - b).ravel()) / max(np.linalg.norm(b.ravel()), 1e-300))

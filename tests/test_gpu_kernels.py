@@ -1,0 +1,261 @@
+"""`-m gpu`: kernel-level parity of the CUDA path (through the C ABI) against the fp64 oracle.
+
+Tolerances: integer / mask / Philox work is bit-exact; single fp32
+operators are compared with the oracle evaluated on the same fp32 inputs, with a bound of a few fp32
+ulps of the largest intermediate.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import tdgl_inputs as I
+from oracle import tdgl_oracle as O
+from gpu_common import f32, make_solver, oracle_params, rel_l2, setup_pair
+
+pytestmark = pytest.mark.gpu
+torch = pytest.importorskip("torch")
+
+P_, O_ = I.PERIODIC, I.OPEN
+ALL_BC = [(a, b, c) for a in (P_, O_) for b in (P_, O_) for c in (P_, O_)]
+
+
+def cfg_of(nx, ny, nz, bc, **kw):
+    return I.Config(f"t{nx}x{ny}x{nz}", nx, ny, nz, tuple(bc), **kw)
+
+
+# ---------------------------------------------------------------------------------------------------
+# a2: Philox stream, bit-exact
+# ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("seed,step", [(0, 0), (12345, 7), ((1 << 40) + 99, 123456)])
+def test_noise_bit_exact(seed, step):
+    cfg = cfg_of(34, 10, 6, (P_, P_, P_), temperature=1e-3, seed=seed)
+    p = oracle_params(cfg)
+    s = make_solver(cfg)
+    z = s.debug_noise(step).cpu().numpy()
+    ref = O.langevin_noise(p, step)
+    # uniform words are exact in fp32; the product with zeta_max is rounded once on each side
+    zm = np.float32(O.zeta_max(p))
+    ref32 = (np.float32(1) * (ref.real / O.zeta_max(p)).astype(np.float32) * zm) + 1j * (
+        (ref.imag / O.zeta_max(p)).astype(np.float32) * zm)
+    assert np.array_equal(z.real, ref32.real.astype(np.float32))
+    assert np.array_equal(z.imag, ref32.imag.astype(np.float32))
+    s.close()
+
+
+def test_initial_state_matches_oracle_box_muller():
+    cfg = cfg_of(32, 12, 6, (P_, P_, P_), seed=3)
+    p = oracle_params(cfg)
+    s = make_solver(cfg)
+    psi, mu = s.get_psi_mu()
+    ref = O.initial_state(p, f32(cfg.init_amp)).psi
+    assert np.max(np.abs(psi.cpu().numpy() - ref)) < 2e-7
+    assert float(mu.abs().max()) == 0.0
+    s.close()
+
+
+# ---------------------------------------------------------------------------------------------------
+# a0: inclusion mask, bit-identical
+# ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("bc", [(P_, P_, P_), (P_, P_, O_), (O_, O_, O_), (P_, O_, O_)])
+def test_epsilon_mask_identical(bc):
+    cfg = cfg_of(40, 28, 18, bc, incl_fraction=0.2, incl_rmin=1.0, incl_rmax=3.0, seed=5)
+    p = oracle_params(cfg)
+    s = make_solver(cfg)
+    sph = I.sphere_list(cfg)
+    assert len(sph) > 5
+    s.set_pinning(sph, -1.0, 1.0)
+    eps = s.get_eps().cpu().numpy()
+    ref = O.epsilon_from_spheres(p, sph, -1.0, 1.0)
+    assert np.array_equal(eps, ref.astype(np.float32))
+    assert 0.05 < (eps < 0).mean() < 0.5
+    s.set_pinning(np.zeros((0, 4), np.float32), -1.0, 0.5)          # empty list
+    assert np.all(s.get_eps().cpu().numpy() == np.float32(0.5))
+    s.close()
+
+
+def test_epsilon_mask_sphere_larger_than_box():
+    cfg = cfg_of(16, 16, 16, (P_, P_, O_))
+    p = oracle_params(cfg)
+    s = make_solver(cfg)
+    sph = np.array([[3.0, 4.0, 2.0, 30.0], [1.0, 1.0, 1.0, 0.2]], np.float32)
+    s.set_pinning(sph, -1.0, 1.0)
+    assert np.array_equal(s.get_eps().cpu().numpy(), O.epsilon_from_spheres(p, sph, -1.0, 1.0).astype(np.float32))
+    s.close()
+
+
+# ---------------------------------------------------------------------------------------------------
+# a6: rho = div j_s
+# ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("bc", ALL_BC)
+@pytest.mark.parametrize("shape", [(34, 13, 11), (132, 37, 9)])
+def test_rho_kernel(bc, shape):
+    nx, ny, nz = shape
+    cfg = cfg_of(nx, ny, nz, bc, Bx=0.07, Bz=0.21)
+    psi0, mu0 = I.random_state(cfg, seed=11)
+    K0 = 0.37 if bc[0] == P_ else 0.0
+    p, st, eps, (Bx, Bz), s = setup_pair(cfg, psi0=psi0, mu0=mu0, K0=K0)
+    rho = s.debug_rho().cpu().numpy()
+    ref = O.supercurrent_divergence(p, st.psi, O.paper_links(p, K0, Bx, Bz))
+    scale = np.max(np.abs(ref))
+    assert np.max(np.abs(rho - ref)) < 2e-6 * max(scale, 1.0) * 24
+    assert rel_l2(rho, ref) < 2e-6
+    s.close()
+
+
+# ---------------------------------------------------------------------------------------------------
+# a7: Poisson solve
+# ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("bc", ALL_BC)
+@pytest.mark.parametrize("shape", [(32, 16, 8), (30, 12, 10), (64, 64, 32)])
+def test_poisson_solve(bc, shape):
+    nx, ny, nz = shape
+    cfg = cfg_of(nx, ny, nz, bc)
+    p = oracle_params(cfg)
+    s = make_solver(cfg)
+    rng = np.random.default_rng(4)
+    w = O.site_weights(p)
+    rho = rng.standard_normal(p.shape)
+    rho -= np.sum(w * rho) / np.sum(w)                       # solvable right side (S6)
+    rho32 = rho.astype(np.float32)
+    mu = s.debug_poisson(torch.from_numpy(rho32)).cpu().numpy().astype(np.float64)
+    ref = O.solve_poisson(p, rho32.astype(np.float64))
+    scale = np.max(np.abs(ref))
+    assert np.max(np.abs(mu - ref)) < 2e-5 * scale
+    assert abs(np.sum(w * mu)) / np.sum(w) < 1e-5 * scale           # S7: weighted zero mode removed
+    # and it solves the equation: Delta_h mu = rho up to fp32 rounding of mu times |Delta_h|
+    res = O.laplacian_real(p, mu) - rho32
+    assert np.max(np.abs(res)) < 24 * 4e-6 * scale + 1e-4
+    s.close()
+
+
+def test_poisson_anisotropic_mesh():
+    cfg = cfg_of(32, 16, 12, (P_, P_, O_))
+    hxyz = (0.5, 0.4, 0.7)
+    p = oracle_params(cfg, hxyz=hxyz, g=1.3)
+    s = make_solver(cfg, hxyz=hxyz, g=1.3)
+    rng = np.random.default_rng(5)
+    w = O.site_weights(p)
+    rho = rng.standard_normal(p.shape)
+    rho -= np.sum(w * rho) / np.sum(w)
+    rho32 = rho.astype(np.float32)
+    mu = s.debug_poisson(torch.from_numpy(rho32)).cpu().numpy()
+    ref = O.solve_poisson(p, rho32.astype(np.float64))
+    assert np.max(np.abs(mu - ref)) < 2e-5 * np.max(np.abs(ref))
+    s.close()
+
+
+# ---------------------------------------------------------------------------------------------------
+# a3 + a4 + a5 + a6 + a7: one full step with a prescribed number of sweeps, every boundary combination
+# ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("bc", ALL_BC)
+@pytest.mark.parametrize("host_loop", [False, True])
+def test_one_step_fixed_sweeps(bc, host_loop):
+    cfg = cfg_of(36, 14, 10, bc, Bx=0.05, Bz=0.3, Jx=0.02 if bc[0] == P_ else 0.0, temperature=1e-3,
+                 incl_fraction=0.15, incl_rmin=1.0, incl_rmax=2.0, seed=2)
+    psi0, mu0 = I.random_state(cfg, seed=21, amp=0.8)
+    K0 = 0.11 if bc[0] == P_ else 0.0
+    p, st, eps, (Bx, Bz), s = setup_pair(cfg, psi0=psi0, mu0=mu0, K0=K0, host_loop=host_loop, fixed_sweeps=5)
+    s.step(2)
+    psi, mu = s.get_psi_mu()
+    psi, mu = psi.cpu().numpy(), mu.cpu().numpy()
+    for _ in range(2):
+        O.step(p, st, eps, Bx, Bz, f32(cfg.Jx), fixed_sweeps=5)
+    ob = s.observables()
+    assert ob.steps == 2 and ob.sweeps_last == 5 and ob.sweeps_total == 10
+    assert np.max(np.abs(psi - st.psi)) < 5e-6
+    assert np.max(np.abs(mu - st.mu)) < 2e-5 * max(1.0, np.max(np.abs(st.mu)))
+    assert abs(ob.K - st.K) < 1e-7 and abs(ob.Ex - st.Ex) < 1e-7 and abs(ob.Jav - st.Jav) < 1e-7
+    # the residual the kernel reduced is the oracle's
+    assert abs(ob.max_resid2 - st.max_resid2) <= 2e-3 * st.max_resid2 + 1e-12
+    s.close()
+
+
+def test_convergence_test_and_cap():
+    """Eq. (34): stop at the first sweep whose input residual is below eps_tol; S10: cap + warning."""
+    cfg = cfg_of(32, 16, 8, (P_, P_, P_), Bz=0.2)
+    psi0, _ = I.random_state(cfg, seed=3, amp=0.7)
+    p, st, eps, (Bx, Bz), s = setup_pair(cfg, psi0=psi0)
+    s.step(1)
+    O.step(p, st, eps, Bx, Bz, 0.0)
+    ob = s.observables()
+    assert ob.sweeps_last == st.sweeps_last and ob.status == 0
+    tr = st.resid_trace[0]
+    assert tr[-1] < p.eps_tol <= tr[-2]
+    s.set_solver(1e-30, 3, 0)
+    s.step(1)
+    from paper_1409_8340_b200 import lib, TdglObs
+    import ctypes
+    o = TdglObs()
+    rc = lib().tdgl_observables(s.h, ctypes.byref(o))
+    assert rc == 1 and o.status == 1 and o.sweeps_last == 3           # TDGL_WMAXSWEEPS
+    s.close()
+
+
+def test_graph_and_host_loop_are_bit_identical():
+    cfg = cfg_of(64, 32, 16, (P_, P_, O_), Bz=0.2, Jx=0.02, temperature=1e-3, incl_fraction=0.1, incl_rmin=1.5,
+                 incl_rmax=1.5)
+    out = []
+    for host_loop in (False, True):
+        p, st, eps, B, s = setup_pair(cfg, host_loop=host_loop)
+        s.step(12)
+        psi, mu = s.get_psi_mu()
+        c, r = s.sweep_log(12)
+        out.append((psi.cpu().numpy(), mu.cpu().numpy(), c, r, s.launch_count()))
+        s.close()
+    assert np.array_equal(out[0][0], out[1][0]) and np.array_equal(out[0][1], out[1][1])
+    assert np.array_equal(out[0][2], out[1][2]) and np.array_equal(out[0][3], out[1][3])
+    assert out[0][4] > 12 * 8
+
+
+# ---------------------------------------------------------------------------------------------------
+# a8: observables
+# ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("bc", [(P_, P_, P_), (P_, P_, O_), (O_, O_, O_), (P_, O_, P_)])
+def test_observables(bc):
+    cfg = cfg_of(32, 24, 10, bc, Bx=0.04, nz_flux=3 if bc[0] == P_ and bc[1] == P_ else None, Bz=0.2,
+                 incl_fraction=0.1, incl_rmin=1.0, incl_rmax=2.0)
+    rng = np.random.default_rng(8)
+    shape = (cfg.nz, cfg.ny, cfg.nx)
+    psi0 = ((1.0 + 0.4 * rng.uniform(-1, 1, shape)) * np.exp(1j * rng.uniform(-math.pi, math.pi, shape))).astype(np.complex64)
+    p, st, eps, (Bx, Bz), s = setup_pair(cfg, psi0=psi0, K0=0.2 if bc[0] == P_ else 0.0)
+    ob = s.observables()
+    links = O.paper_links(p, st.K, Bx, Bz)
+    F = O.free_energy(p, st.psi, eps, links)
+    assert abs(ob.free_energy - F) < 2e-6 * abs(F) + 1e-6 * p.n_sites
+    assert abs(ob.mean_abs2 - O.mean_abs2(st.psi)) < 1e-6
+    assert abs(ob.vortices_per_slice - O.vortices_per_slice(p, st.psi, links, Bz)) < 1e-9
+    if bc[0] == P_ and bc[1] == P_:
+        assert ob.vortices_per_slice == 3.0                              # flux quantisation
+    assert abs(ob.Bz_eff - Bz) < 1e-7 and abs(ob.Bx_eff - Bx) < 1e-7
+    s.close()
+
+
+# ---------------------------------------------------------------------------------------------------
+# boundary: error behaviour
+# ---------------------------------------------------------------------------------------------------
+def test_error_codes():
+    import ctypes as C
+    from paper_1409_8340_b200 import TdglParams, lib, tdgl_workspace_bytes
+    from paper_1409_8340_b200.binding import TdglError
+    p = TdglParams()
+    p.nx, p.ny, p.nz = 31, 8, 8                                          # odd nx
+    p.hx = p.hy = p.hz = 0.5
+    p.dt, p.u, p.g, p.eps_tol, p.max_sweeps = 0.1, 1.0, 1.0, 1e-6, 10
+    assert tdgl_workspace_bytes(p) == 0
+    h = C.c_void_p()
+    assert lib().tdgl_create(C.byref(p), C.byref(h)) == -1               # TDGL_EINVAL
+    p.nx = 32
+    need = tdgl_workspace_bytes(p)
+    assert need > 32 * 8 * 8 * 44
+    buf = torch.empty(need // 2, dtype=torch.uint8, device="cuda")
+    p.workspace_dev, p.workspace_bytes = (buf.data_ptr() + 255) // 256 * 256, need // 2 - 256
+    assert lib().tdgl_create(C.byref(p), C.byref(h)) == -2               # TDGL_ENOMEM
+    s = make_solver(cfg_of(32, 8, 8, (O_, P_, P_)))
+    with pytest.raises(TdglError) as e:
+        s.set_field_current(Bz=0.1, Jx=0.01)                             # open x + current
+    assert e.value.code == -3
+    with pytest.raises(TdglError) as e:
+        s.set_field_current(By=0.1)
+    assert e.value.code == -3
+    s.close()
