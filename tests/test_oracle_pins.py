@@ -530,3 +530,28 @@ def test_epsilon_bounding_box_equals_brute_force(bc):
     # a sphere of radius r centred on a site covers exactly the lattice points with d^2 <= r^2
     one = O.epsilon_from_spheres(p, np.array([[4.0, 3.0, 2.5, 1.0]]), -1.0, 1.0)
     assert int(np.sum(one < 0)) == 33          # |n|^2 <= 4 on the cubic lattice h = 0.5: 1+6+12+8+6
+
+
+# ------------------------------------------------------------------------------------------------
+# single-sweep amplification of the checkerboard mode
+# ------------------------------------------------------------------------------------------------
+def test_single_sweep_checkerboard_amplification_factor():
+    # Eq. (33) with x^0 = psi^-: one sweep gives x^1 = [psi (2 - d) + h_t nsum(psi)]/d.  For a small
+    # checkerboard psi = delta (-1)^(i+j+k): nsum = -2 (c_x + c_y + c_z) psi and d = 1 + (h_t/2)(2 sum c - eps),
+    # so the per-step factor is [(2 - d) - 2 h_t sum c]/d = -1.186 at h = 0.5, h_t = 0.1, eps = 1, although
+    # the exact Crank-Nicolson factor (1 + q)/(1 - q), q = (h_t/2)(eps - 4 sum c) = -2.35, is -0.403.
+    p = O.Params(8, 8, 8, solve_mu=False)
+    k_, j_, i_ = np.meshgrid(np.arange(8), np.arange(8), np.arange(8), indexing="ij")
+    cb = (-1.0) ** (i_ + j_ + k_)
+    eps = np.ones(p.shape)
+    sc = p.cx + p.cy + p.cz
+    d = 1 + p.ht / 2 * (2 * sc - 1.0)
+    one_sweep = ((2 - d) - 2 * p.ht * sc) / d
+    assert abs(one_sweep + 1.186) < 1e-3
+    st = O.State(psi=1e-9 * cb.astype(np.complex128), mu=np.zeros(p.shape))
+    O.step(p, st, eps, 0.0, 0.0, 0.0, fixed_sweeps=1)
+    assert np.max(np.abs(st.psi / (1e-9 * cb) - one_sweep)) < 1e-9
+    q = p.ht / 2 * (1.0 - 4 * sc)
+    st = O.State(psi=1e-9 * cb.astype(np.complex128), mu=np.zeros(p.shape))
+    O.step(p, st, eps, 0.0, 0.0, 0.0, fixed_sweeps=400)
+    assert np.max(np.abs(st.psi / (1e-9 * cb) - (1 + q) / (1 - q))) < 1e-9
