@@ -1,0 +1,325 @@
+#!/usr/bin/env python
+"""bench.py -- TDGL hot-path throughput on B200 (BASELINE.json metric) with roofline, e2e and CPU baseline.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C4] [--impl ours|reference]
+
+A bench "step" is one TDGL time step (tdgl_step(h, 1)): fused init + first Jacobi sweep, the further
+sweeps to criterion (34), J_av/K, rho, Poisson solve.  Prints ONE JSON line (rank 0).
+  value      site-iterations/s = sites x Jacobi sweeps executed / device time of the K timed steps, state
+             resident in HBM (CUDA events on the launching stream, max over ranks)
+  e2e        the same metric with, every step, the state uploaded from pinned host memory
+             (tdgl_set_state), one tdgl_step, and psi, mu and the observables read back to the host
+  roofline   the Jacobi sweep kernel: 32 B/site algorithmic bytes / mean launch duration (CUDA events
+             around every sweep launch of a host-loop run of the same workload) vs the measured HBM peak
+  cpu_baseline  the fp64 oracle (oracle/, numpy) timed on this box's host cores on a bounded sample
+N > 1 (torchrun): independent replicas, one per GPU ("replicas only"); no collective on the
+data path.  `--impl reference` times the oracle alone (rank 0).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+sys.path.insert(0, os.path.join(ROOT, "tests"))
+
+import numpy as np  # noqa: E402
+
+import tdgl_inputs as I  # noqa: E402
+
+METRIC = "TDGL site-iterations/s (whole time step) at 512x512x256 fp32"
+UNIT = "site-iterations/s"
+SWEEP_BYTES_PER_SITE = 32.0      # x^l 8 + b 8 + d 8 read, x^{l+1} 8 written
+
+
+def measured_peak():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def ncu_traffic():
+    """Per-launch DRAM bytes of the sweep kernel from the committed ncu capture, if any."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "sweep_traffic.json")) as f:
+            d = json.load(f)
+        return d
+    except Exception:
+        return None
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md)."""
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+             "clocks_event_reasons.sw_power_cap")
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def make_solver(cfg: I.Config, host_loop=False, seed_offset=0):
+    from paper_1409_8340_b200 import Solver
+    s = Solver(cfg.nx, cfg.ny, cfg.nz, bc=cfg.bc, h=cfg.h, dt=cfg.dt, eps_tol=1e-6, max_sweeps=100,
+               temperature=cfg.temperature, seed=cfg.seed + seed_offset, init_amp=cfg.init_amp, solve_mu=True,
+               host_loop=host_loop)
+    s.set_pinning(I.sphere_list(cfg), cfg.eps_in, cfg.eps_out)
+    bx, bz = cfg.requested_field()
+    s.set_field_current(Bx=bx, Bz=bz, Jx=cfg.Jx)
+    return s
+
+
+def oracle_sample(cfg: I.Config, budget_s: float = 20.0):
+    """The fp64 oracle as it stands on a bounded sample of the workload: the same physics on a z-slab of
+    the grid (full x, y extent, 16 planes), as many steps as fit the budget (>= 2)."""
+    from oracle import tdgl_oracle as O
+    from gpu_common import f32, oracle_params
+    nz = min(cfg.nz, 16)
+    sub = cfg.scaled(cfg.nx, cfg.ny, nz, f"{cfg.name} slab {cfg.nx}x{cfg.ny}x{nz}")
+    p = oracle_params(sub)
+    eps = O.epsilon_from_spheres(p, I.sphere_list(sub), sub.eps_in, sub.eps_out)
+    bx, bz = sub.requested_field()
+    Bx, Bz, _, _ = O.snap_field(p, f32(bx), f32(bz))
+    st = O.State(psi=I.initial_psi(sub).astype(np.complex128), mu=np.zeros(p.shape))
+    O.step(p, st, eps, Bx, Bz, f32(sub.Jx))                     # untimed: page-in, FFT plans
+    t0 = time.perf_counter()
+    sw0 = st.sweeps_total
+    steps = 0
+    while steps < 2 or (time.perf_counter() - t0 < budget_s and steps < 1000):
+        O.step(p, st, eps, Bx, Bz, f32(sub.Jx))
+        steps += 1
+    dt = time.perf_counter() - t0
+    sweeps = st.sweeps_total - sw0
+    return {"value": p.n_sites * sweeps / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+            "sample": f"{sub.name}, {steps} steps, {sweeps} sweeps, {dt:.1f} s (numpy fp64, single thread)",
+            "steps_per_s_on_sample": steps / dt, "ms_per_step_sample": 1e3 * dt / steps,
+            "host_cores_available": os.cpu_count()}
+
+
+def run_reference(args, cfg):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    budget = 8.0
+    vals, t_all = [], time.perf_counter()
+    for _ in range(max(1, args.warmup if args.warmup < 2 else 1)):
+        oracle_sample(cfg, 2.0)
+    res = None
+    per = []
+    for _ in range(max(1, min(args.steps, 8))):
+        res = oracle_sample(cfg, budget)
+        per.append(res["value"])
+    v = float(np.mean(per))
+    out = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": res["ms_per_step_sample"], "higher_is_better": True,
+           "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": {"workload": cfg.name, "grid": [cfg.nx, cfg.ny, cfg.nz], "note": "each bench step = one bounded oracle sample"},
+           "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": res["sample"]},
+           "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "gpu_launches": 0, "wall_s": time.perf_counter() - t_all}
+    print(json.dumps(out), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=100)
+    ap.add_argument("--config", default="C4")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    cfg = I.CONFIGS[args.config]
+    if args.impl == "reference":
+        run_reference(args, cfg)
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_1409_8340_b200 import build as B
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if rank == 0:
+        B.build()
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
+        dist.barrier()
+    torch.cuda.set_device(local_rank)
+    dev = torch.device(f"cuda:{local_rank}")
+    W = max(args.warmup, 3)
+    K = args.steps
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    # ---- resident run (graph mode) --------------------------------------------------------------
+    s = make_solver(cfg, seed_offset=rank)
+    s.step(W)
+    barrier()
+    ob0 = s.observables()
+    l0 = s.launch_count()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record()
+    s.step(K)
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    clocks = sampler.stop()
+    ob1 = s.observables()
+    launches = s.launch_count() - l0 - 2           # minus the two observables kernels
+    sweeps = ob1.sweeps_total - ob0.sweeps_total
+    t = torch.tensor([ms, float(sweeps), float(launches)], dtype=torch.float64, device=dev)
+    if world > 1:
+        tmax = t.clone(); dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        tsum = t.clone(); dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
+        ms, sweeps_all, launches_all = float(tmax[0]), float(tsum[1]), int(tsum[2])
+    else:
+        sweeps_all, launches_all = float(sweeps), int(launches)
+    N = cfg.n_sites
+    value = N * sweeps_all / (ms * 1e-3)
+    steps_per_s = world * K / (ms * 1e-3)
+
+    # ---- roofline of the sweep kernel: CUDA events around every sweep launch (host-loop run) ----
+    roof = None
+    e2e = None
+    if rank == 0 or world > 1:
+        psi, mu = s.get_psi_mu()
+        K0 = s.observables().K
+        sh = make_solver(cfg, host_loop=True, seed_offset=rank)
+        sh.set_state(psi, mu, K0)
+        sh.step(3)
+        sh.sweep_timing(True)
+        sh.step(max(3, min(K, 40)))
+        t_ms, n_l = sh.sweep_timing(False)
+        peak, how = measured_peak()
+        if n_l > 0:
+            avg_ms = t_ms / n_l
+            ach = SWEEP_BYTES_PER_SITE * N / (avg_ms * 1e-3) / 1e9
+            tr = ncu_traffic()
+            roof = {"bound": "hbm", "kernel": "k_march<SWEEP> (Jacobi sweep + max-residual)", "achieved": ach,
+                    "peak": peak, "unit": "GB/s", "frac": ach / peak, "peak_source": how,
+                    "avg_launch_ms": avg_ms, "launches_timed": int(n_l),
+                    "algorithmic_bytes_per_launch": SWEEP_BYTES_PER_SITE * N,
+                    "traffic": (tr or {}).get("dram_bytes_per_launch") if (tr or {}).get("sites") == N else None}
+        sh.close()
+        del sh
+
+        # ---- e2e: host buffers, per step H2D state -> step -> D2H state + observables ------------
+        if not args.no_e2e:
+            Ke = max(1, min(K, 30))
+            hp = torch.view_as_real(psi).cpu().pin_memory()
+            hm = mu.cpu().pin_memory()
+            dp = torch.empty_like(torch.view_as_real(psi))
+            dm = torch.empty_like(mu)
+            h2d = hp.numel() * 4 + hm.numel() * 4
+            d2h = h2d + 136
+            obx = s.observables()
+            for it in range(2 + Ke):
+                if it == 2:
+                    barrier()
+                    sw_a = s.observables().sweeps_total
+                    t0 = time.perf_counter()
+                dp.copy_(hp, non_blocking=True)
+                dm.copy_(hm, non_blocking=True)
+                s.set_state(torch.view_as_complex(dp), dm, obx.K)
+                s.step(1)
+                a, b2 = s.get_psi_mu()
+                hp.copy_(torch.view_as_real(a), non_blocking=True)
+                hm.copy_(b2, non_blocking=True)
+                obx = s.observables()                     # syncs the stream
+                torch.cuda.synchronize()
+            te = time.perf_counter() - t0
+            sw_e = obx.sweeps_total - sw_a
+            te_t = torch.tensor([te, float(sw_e)], dtype=torch.float64, device=dev)
+            if world > 1:
+                a_ = te_t.clone(); dist.all_reduce(a_, op=dist.ReduceOp.MAX)
+                b_ = te_t.clone(); dist.all_reduce(b_, op=dist.ReduceOp.SUM)
+                te, sw_e = float(a_[0]), float(b_[1])
+            e2e = {"value": N * sw_e / te, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                   "steps": Ke, "ms_per_step": 1e3 * te / Ke, "steps_per_s": world * Ke / te}
+    s.close()
+
+    if rank != 0:
+        if world > 1:
+            dist.barrier()
+            dist.destroy_process_group()
+        return
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        cpu = oracle_sample(cfg)
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "data": "synthetic", "steps_per_s": steps_per_s, "sweeps_per_step": sweeps_all / (K * world),
+        "config": {"workload": cfg.name, "grid": [cfg.nx, cfg.ny, cfg.nz], "bc": list(cfg.bc), "h": cfg.h, "dt": cfg.dt,
+                   "Bz": cfg.Bz, "Bx": cfg.Bx, "Jx": cfg.Jx, "T": cfg.temperature, "inclusion_fraction": cfg.incl_fraction,
+                   "eps_tol": 1e-6, "parallelism": "replicas only" if world > 1 else "1 GPU",
+                   "l2": "working set %.2f GB >> 126 MB L2, no flush needed" % (44.0 * N / 1e9),
+                   "loop": "CUDA graph per step, WHILE node around the sweep, no host sync"},
+        "clocks": clocks, "e2e": e2e, "gpu_launches": launches_all, "roofline": roof, "cpu_baseline": cpu,
+        "state": {"mean_abs2": ob1.mean_abs2, "Ex": ob1.Ex, "K": ob1.K, "vortices_per_slice": ob1.vortices_per_slice,
+                  "status": ob1.status},
+    }
+    print(json.dumps(out), flush=True)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -17,40 +17,22 @@
 #define MODE_INIT  1
 #define MODE_RHO   2
 
-#define NBUF 5              // ring slots; plane k+PD is fetched while plane k is computed
-#define PD (NBUF - 2)
+#define NBUF 5              // ring slots: planes k-1 .. k+2 resident, plane k+3 in flight
 
-__device__ __forceinline__ void cp_async16(void *smem, const void *g) {
-  unsigned s = (unsigned)__cvta_generic_to_shared(smem);
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(s), "l"(g) : "memory");
+__device__ __forceinline__ void cp_async16(unsigned saddr, const void *g) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(saddr), "l"(g) : "memory");
 }
-__device__ __forceinline__ void cp_async8(void *smem, const void *g) {
-  unsigned s = (unsigned)__cvta_generic_to_shared(smem);
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(s), "l"(g) : "memory");
+__device__ __forceinline__ void cp_async8(unsigned saddr, const void *g) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(saddr), "l"(g) : "memory");
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
 template <int N> __device__ __forceinline__ void cp_async_wait() {
   asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory");
 }
 
-// sum_alpha c_alpha (S+ f + S- f) at one site (Eq. 29a; open faces: S- := S+ at the first site,
-// S+ := S- at the last).  The y terms arrive with their jump phase already applied.
-__device__ __forceinline__ float2 nsum_site(float2 W, float2 E, float2 S, float2 Nn, float2 B, float2 T,
-                                            float2 Ux, float2 Uz, float cx, float cy, float cz,
-                                            bool xlo, bool xhi, bool zlo, bool zhi) {
-  float2 xp = cmul(Ux, E), xm = cmulc(Ux, W);
-  if (xlo) xm = xp;
-  if (xhi) xp = xm;
-  float2 zp = cmul(Uz, T), zm = cmulc(Uz, B);
-  if (zlo) zm = zp;
-  if (zhi) zp = zm;
-  return make_float2(cx * (xp.x + xm.x) + cy * (Nn.x + S.x) + cz * (zp.x + zm.x),
-                     cx * (xp.y + xm.y) + cy * (Nn.y + S.y) + cz * (zp.y + zm.y));
-}
-
 // The decision taken by the last CTA of a sweep (Eq. 34; S8: residual of the input iterate,
 // keep the new one; S9/S10: prescribed counts, cap).
-__device__ void sweep_decide(const Dev &dv, int l) {
+__device__ __noinline__ void sweep_decide(const Dev &dv, int l) {
   Ctl *c = dv.ctl;
   const float r2 = __uint_as_float(atomicMax(&c->resid_bits[l], 0u));
   const int sweeps = l + 1;
@@ -74,8 +56,20 @@ __device__ void sweep_decide(const Dev &dv, int l) {
   __threadfence();
 }
 
-template <int MODE>
-__global__ void __launch_bounds__(512, 2) k_march(const __grid_constant__ Dev dv) {
+// BX thread columns (two sites each) x BY rows per CTA; tile = 2*BX x BY sites.
+//
+// Arithmetic per site (all modes): with W' = W, E' = E the x neighbours, S, N the y neighbours (jump
+// phase applied on the wrap rows), B, T the z neighbours,
+//   f . nsum = f cx [U_x E + U_x* W] + f cy [N + S] + f cz [U_z T + U_z* B]
+//            = (f cx U_x).re (E + W) + i (f cx U_x).im (E - W) + f cy (N + S) + (f cz U_z).re (T + B) + i (...).im (T - B)
+// with f = h_t/2 (sweep, init) or 1 (rho): 10 adds and 10 FMAs instead of four complex products.
+// Open faces (S- := S+ at the first site, S+ := S- at the last) are folded into the
+// neighbour itself: U* W' = U E  <=>  W' = U^2 E  (|U| = 1), likewise E' = U*^2 W, B' = U_z^2 T, T' = U_z*^2 B.
+template <int MODE, int BX, int BY>
+__global__ void __launch_bounds__(BX *BY, 1024 / (BX * BY)) k_march(const __grid_constant__ Dev dv) {
+  constexpr int RP = 2 * BX + 4;            // row pitch in float2: [pad, W, 2*BX centre, E, pad]
+  constexpr int SP = (BY + 2) * RP;         // slot pitch in float2
+  constexpr unsigned SPB = SP * 8u;         // slot pitch in bytes
   extern __shared__ float4 smem4[];
   float2 *sm = reinterpret_cast<float2 *>(smem4);
   Ctl *ctl = dv.ctl;
@@ -86,86 +80,104 @@ __global__ void __launch_bounds__(512, 2) k_march(const __grid_constant__ Dev dv
   }
   const int xb = ctl->xbuf;
   const float2 *__restrict__ xin = dv.psi[xb];
-  float2 *__restrict__ xout = dv.psi[xb ^ 1];
 
   const int nx = dv.nx, ny = dv.ny, nz = dv.nz;
-  const int tx = threadIdx.x, ty = threadIdx.y, bx = blockDim.x, by = blockDim.y;
-  const int lane = (ty * bx + tx) & 31;
-  const int i0 = blockIdx.x * 2 * bx, j0 = blockIdx.y * by;
+  const int tx = threadIdx.x, ty = threadIdx.y;
+  const int lane = (ty * BX + tx) & 31;
+  const int i0 = blockIdx.x * 2 * BX, j0 = blockIdx.y * BY;
   const int i = i0 + 2 * tx, j = j0 + ty;
-  const int nvx = min(bx, (nx - i0) >> 1), nvy = min(by, ny - j0);
+  const int nvx = min(BX, (nx - i0) >> 1), nvy = min(BY, ny - j0);
   const bool actx = tx < nvx, acty = ty < nvy, act = actx && acty;
   const int k0 = blockIdx.z * dv.zc, k1 = min(nz, k0 + dv.zc);     // planes [k0, k1)
-
-  // ghost sources: periodic wrap or mirror
   const bool px = dv.bcx == 0, py = dv.bcy == 0, pz = dv.bcz == 0;
-  int jS = j0 - 1, jN = j0 + nvy;
-  if (jS < 0) jS = py ? ny - 1 : 1;
-  if (jN >= ny) jN = py ? 0 : ny - 2;
-  int iW = i0 - 1, iE = i0 + 2 * nvx;
-  if (iW < 0) iW = px ? nx - 1 : 1;
-  if (iE >= nx) iE = px ? 0 : nx - 2;
-
-  const int RP = 2 * bx + 4;                 // row pitch in float2: [pad, W, 2*bx centre, E, pad]
-  const int SP = (by + 2) * RP;              // slot pitch
-  const size_t plane = (size_t)nx * ny;
+  const long long plane = (long long)nx * ny;
   const int r = ty + 1, c = 2 + 2 * tx;
+  const unsigned sbase = (unsigned)__cvta_generic_to_shared(sm);
 
-  auto load_plane = [&](int kp, int slot, bool ghosts) {
+  // Copy roles, fixed for the whole march.  Every active thread copies its own 16-byte centre vector.
+  // Ghost row j0-1 is copied by thread row 0, ghost row j0+nvy by thread row BY-1 (wrapped, or
+  // mirrored); ghost column i0-1 by thread column 0, ghost column i0+2 nvx by thread column BX-1.
+  const float2 *gC = xin + ((long long)min(j, ny - 1) * nx + min(i, nx - 2));
+  const unsigned dC = sbase + (unsigned)(r * RP + c) * 8u;
+  const float2 *gR = gC;
+  unsigned dR = 0;
+  bool hasR = false;
+  if (actx && (ty == 0 || ty == BY - 1)) {
+    int js, row;
+    if (ty == 0) { js = j0 - 1; if (js < 0) js = py ? ny - 1 : 1; row = 0; }
+    else { js = j0 + nvy; if (js >= ny) js = py ? 0 : ny - 2; row = nvy + 1; }
+    gR = xin + ((long long)js * nx + i);
+    dR = sbase + (unsigned)(row * RP + c) * 8u;
+    hasR = true;
+  }
+  const float2 *gG = gC;
+  unsigned dG = 0;
+  bool hasG = false;
+  if (acty && (tx == 0 || tx == BX - 1)) {
+    int is, col;
+    if (tx == 0) { is = i0 - 1; if (is < 0) is = px ? nx - 1 : 1; col = 1; }
+    else { is = i0 + 2 * nvx; if (is >= nx) is = px ? 0 : nx - 2; col = 2 + 2 * nvx; }
+    gG = xin + ((long long)j * nx + is);
+    dG = sbase + (unsigned)(r * RP + col) * 8u;
+    hasG = true;
+  }
+
+  // plane offset (elements) with the z wrap / mirror
+  auto zoff = [&](int kp) -> long long {
     int kw = kp;
     if (kw < 0) kw = pz ? nz - 1 : 1;
     if (kw >= nz) kw = pz ? 0 : nz - 2;
-    const float2 *src = xin + (size_t)kw * plane;
-    float2 *dst = sm + slot * SP;
-    if (act) cp_async16(dst + r * RP + c, src + (size_t)j * nx + i);
+    return (long long)kw * plane;
+  };
+  auto load_plane = [&](long long poff, unsigned slotb, bool ghosts) {
+    if (act) cp_async16(dC + slotb, gC + poff);
     if (ghosts) {
-      if (actx && ty == 0) cp_async16(dst + c, src + (size_t)jS * nx + i);
-      if (actx && ty == nvy - 1) cp_async16(dst + (nvy + 1) * RP + c, src + (size_t)jN * nx + i);
-      if (acty && tx == 0) cp_async8(dst + r * RP + 1, src + (size_t)j * nx + iW);
-      if (acty && tx == nvx - 1) cp_async8(dst + r * RP + 2 + 2 * nvx, src + (size_t)j * nx + iE);
+      if (hasR) cp_async16(dR + slotb, gR + poff);
+      if (hasG) cp_async8(dG + slotb, gG + poff);
     }
   };
 
-  // prologue: planes k0-1, k0, k0+1 in one group, then one group per further plane
-  load_plane(k0 - 1, 0, false);
-  load_plane(k0, 1, true);
-  load_plane(k0 + 1, 2, k0 + 1 < k1);
+  // prologue: planes k0-1, k0, k0+1 (slots 0, 1, 2) in one group, plane k0+2 (slot 3) in the next
+  load_plane(zoff(k0 - 1), 0u, false);
+  load_plane(zoff(k0), SPB, true);
+  load_plane(zoff(k0 + 1), 2u * SPB, k0 + 1 < k1);
   cp_async_commit();
-#pragma unroll
-  for (int p = 2; p < PD; ++p) {
-    if (k0 + p <= k1) load_plane(k0 + p, (p + 1) % NBUF, k0 + p < k1);
-    cp_async_commit();
-  }
+  if (k0 + 2 <= k1) load_plane(zoff(k0 + 2), 3u * SPB, k0 + 2 < k1);
+  cp_async_commit();
 
   const int jc = min(j, ny - 1);
-  const float2 Ux = dv.Ux[jc], Uz = dv.Uz[jc];
-  const float cx = dv.cx, cy = dv.cy, cz = dv.cz, ht2 = dv.ht2;
+  const float f = (MODE == MODE_RHO) ? 1.f : dv.ht2;
+  float2 hUx, hUz;
+  {
+    const float2 Ux = dv.Ux[jc], Uz = dv.Uz[jc];
+    hUx = make_float2(f * dv.cx * Ux.x, f * dv.cx * Ux.y);
+    hUz = make_float2(f * dv.cz * Uz.x, f * dv.cz * Uz.y);
+  }
+  const float hcy = f * dv.cy;
   const bool xlo0 = !px && i == 0, xhi1 = !px && (i + 1 == nx - 1);
   const bool ylo = py && j == 0, yhi = py && j == ny - 1;
-  float4 Pij = make_float4(1.f, 0.f, 1.f, 0.f);
-  if ((ylo || yhi) && actx) Pij = *reinterpret_cast<const float4 *>(dv.Pi + i);
+  const bool wsm = (tx == 0 || lane == 0), esm = (tx >= nvx - 1 || lane == 31);
   float rmax = 0.f;
-  long long nstep = 0;
-  if (MODE == MODE_INIT) nstep = ctl->n;
+  unsigned nstep = 0;
+  if (MODE == MODE_INIT) nstep = (unsigned)ctl->n;
 
-  const size_t rowoff = (size_t)j * nx + i;
-  float4 bv = make_float4(0, 0, 0, 0), dvv = make_float4(1, 0, 1, 0);
-  if (MODE == MODE_SWEEP && act) {
-    bv = __ldcs(reinterpret_cast<const float4 *>(dv.b + (size_t)k0 * plane + rowoff));
-    dvv = __ldcs(reinterpret_cast<const float4 *>(dv.d + (size_t)k0 * plane + rowoff));
-  }
+  // running element index of this thread's pair of sites (float2 units)
+  long long idx = (long long)k0 * plane + (long long)min(j, ny - 1) * nx + min(i, nx - 2);
+  float2 *__restrict__ xout = dv.psi[xb ^ 1];
+  // ring of 5 slots (element offsets): planes k-1, k, k+1, k+2 and the free slot that receives plane k+3
+  unsigned oB = 0u, oC = SP, oT = 2u * SP, oU = 3u * SP, oF = 4u * SP;
+  const float2 *sthr = sm + r * RP + c;       // this thread's centre position inside a slot
 
   for (int k = k0; k < k1; ++k) {
-    cp_async_wait<PD - 2>();
+    cp_async_wait<1>();                     // planes <= k+1 have landed; plane k+2 may still be in flight
     __syncthreads();
-    if (k + PD <= k1) load_plane(k + PD, (k + PD - k0 + 1) % NBUF, k + PD < k1);
+    if (k + 3 <= k1) load_plane(zoff(k + 3), oF * 8u, k + 3 < k1);
     cp_async_commit();
 
-    const size_t idx = (size_t)k * plane + rowoff;
-    float4 bn = bv, dn = dvv;
-    if (MODE == MODE_SWEEP && act && k + 1 < k1) {            // next plane's b, d: one plane ahead
-      bn = __ldcs(reinterpret_cast<const float4 *>(dv.b + idx + plane));
-      dn = __ldcs(reinterpret_cast<const float4 *>(dv.d + idx + plane));
+    float4 bv = make_float4(0, 0, 0, 0), dvv = make_float4(1, 0, 1, 0);
+    if (MODE == MODE_SWEEP && act) {                          // issued early, consumed after the stencil
+      bv = __ldcs(reinterpret_cast<const float4 *>(dv.b + idx));
+      dvv = __ldcs(reinterpret_cast<const float4 *>(dv.d + idx));
     }
     float2 muv = make_float2(0.f, 0.f), ev = make_float2(1.f, 1.f);
     if (MODE == MODE_INIT && act) {
@@ -173,24 +185,24 @@ __global__ void __launch_bounds__(512, 2) k_march(const __grid_constant__ Dev dv
       ev = __ldg(reinterpret_cast<const float2 *>(dv.eps + idx));
     }
 
-    const float2 *sC = sm + ((k - k0 + 1) % NBUF) * SP;
-    const float2 *sB = sm + ((k - k0) % NBUF) * SP;
-    const float2 *sT = sm + ((k - k0 + 2) % NBUF) * SP;
-    const float4 C = *reinterpret_cast<const float4 *>(sC + r * RP + c);
-    float4 Nn = *reinterpret_cast<const float4 *>(sC + (r + 1) * RP + c);
-    float4 Ss = *reinterpret_cast<const float4 *>(sC + (r - 1) * RP + c);
-    const float4 T = *reinterpret_cast<const float4 *>(sT + r * RP + c);
-    const float4 B = *reinterpret_cast<const float4 *>(sB + r * RP + c);
+    const float2 *sC = sthr + oC;
+    const float4 C = *reinterpret_cast<const float4 *>(sC);
+    float4 Nn = *reinterpret_cast<const float4 *>(sC + RP);
+    float4 Ss = *reinterpret_cast<const float4 *>(sC - RP);
+    float4 T = *reinterpret_cast<const float4 *>(sthr + oT);
+    float4 B = *reinterpret_cast<const float4 *>(sthr + oB);
     float2 W, E;
     W.x = __shfl_up_sync(0xffffffffu, C.z, 1);
     W.y = __shfl_up_sync(0xffffffffu, C.w, 1);
     E.x = __shfl_down_sync(0xffffffffu, C.x, 1);
     E.y = __shfl_down_sync(0xffffffffu, C.y, 1);
-    if (tx == 0 || lane == 0) W = sC[r * RP + c - 1];
-    if (tx >= nvx - 1 || lane == 31) E = sC[r * RP + c + 2];
+    if (wsm) W = sC[-1];
+    if (esm) E = sC[2];
+    const float2 c0 = make_float2(C.x, C.y), c1 = make_float2(C.z, C.w);
 
     if (ylo || yhi) {                          // quasi-periodic jump in y
       const float2 Pk = dv.Pk[k];
+      const float4 Pij = *reinterpret_cast<const float4 *>(dv.Pi + min(i, nx - 2));
       const float2 P0 = cmulc(Pk, make_float2(Pij.x, Pij.y));   // P_{i,k} = Pi[i] conj(Pk[k])
       const float2 P1 = cmulc(Pk, make_float2(Pij.z, Pij.w));
       if (ylo) {                               // psi_{i,-1,k} = P psi_{i,ny-1,k}
@@ -202,12 +214,38 @@ __global__ void __launch_bounds__(512, 2) k_march(const __grid_constant__ Dev dv
         Nn = make_float4(a.x, a.y, bq.x, bq.y);
       }
     }
-    const bool zlo = !pz && k == 0, zhi = !pz && k == nz - 1;
-    const float2 c0 = make_float2(C.x, C.y), c1 = make_float2(C.z, C.w);
-    const float2 s0 = nsum_site(W, c1, make_float2(Ss.x, Ss.y), make_float2(Nn.x, Nn.y), make_float2(B.x, B.y),
-                                make_float2(T.x, T.y), Ux, Uz, cx, cy, cz, xlo0, false, zlo, zhi);
-    const float2 s1 = nsum_site(c0, E, make_float2(Ss.z, Ss.w), make_float2(Nn.z, Nn.w), make_float2(B.z, B.w),
-                                make_float2(T.z, T.w), Ux, Uz, cx, cy, cz, false, xhi1, zlo, zhi);
+    if (xlo0 || xhi1) {
+      const float2 Ux = dv.Ux[jc];
+      if (xlo0) W = cmul(cmul(Ux, Ux), c1);                     // open x, first site: W' = U^2 E
+      if (xhi1) E = cmulc(cmul(Ux, Ux), c0);                    // open x, last site:  E' = U*^2 W
+    }
+    if (!pz && (k == 0 || k == nz - 1)) {                       // open z faces (uniform over the CTA)
+      const float2 Uz = dv.Uz[jc];
+      const float2 U2 = cmul(Uz, Uz);
+      if (k == 0) {
+        const float2 a = cmul(U2, make_float2(T.x, T.y)), bq = cmul(U2, make_float2(T.z, T.w));
+        B = make_float4(a.x, a.y, bq.x, bq.y);
+      } else {
+        const float2 a = cmulc(U2, make_float2(B.x, B.y)), bq = cmulc(U2, make_float2(B.z, B.w));
+        T = make_float4(a.x, a.y, bq.x, bq.y);
+      }
+    }
+
+    float2 b0 = make_float2(bv.x, bv.y), b1 = make_float2(bv.z, bv.w);
+    // acc = start + f nsum;  start = b (sweep) or 0 (init, rho)
+    float2 s0 = (MODE == MODE_SWEEP) ? b0 : make_float2(0.f, 0.f);
+    float2 s1 = (MODE == MODE_SWEEP) ? b1 : make_float2(0.f, 0.f);
+    // site 0: west W, east c1;  site 1: west c0, east E
+    s0.x = fmaf(hUx.x, c1.x + W.x, s0.x);  s0.x = fmaf(-hUx.y, c1.y - W.y, s0.x);
+    s0.y = fmaf(hUx.x, c1.y + W.y, s0.y);  s0.y = fmaf(hUx.y, c1.x - W.x, s0.y);
+    s1.x = fmaf(hUx.x, E.x + c0.x, s1.x);  s1.x = fmaf(-hUx.y, E.y - c0.y, s1.x);
+    s1.y = fmaf(hUx.x, E.y + c0.y, s1.y);  s1.y = fmaf(hUx.y, E.x - c0.x, s1.y);
+    s0.x = fmaf(hcy, Nn.x + Ss.x, s0.x);   s0.y = fmaf(hcy, Nn.y + Ss.y, s0.y);
+    s1.x = fmaf(hcy, Nn.z + Ss.z, s1.x);   s1.y = fmaf(hcy, Nn.w + Ss.w, s1.y);
+    s0.x = fmaf(hUz.x, T.x + B.x, s0.x);   s0.x = fmaf(-hUz.y, T.y - B.y, s0.x);
+    s0.y = fmaf(hUz.x, T.y + B.y, s0.y);   s0.y = fmaf(hUz.y, T.x - B.x, s0.y);
+    s1.x = fmaf(hUz.x, T.z + B.z, s1.x);   s1.x = fmaf(-hUz.y, T.w - B.w, s1.x);
+    s1.y = fmaf(hUz.x, T.w + B.w, s1.y);   s1.y = fmaf(hUz.y, T.z - B.z, s1.y);
 
     if (MODE == MODE_RHO) {
       // rho_m = sum_alpha c_alpha Im[psi*_m (S+ psi + S- psi)_m]
@@ -215,36 +253,37 @@ __global__ void __launch_bounds__(512, 2) k_march(const __grid_constant__ Dev dv
         *reinterpret_cast<float2 *>(dv.mu + idx) =
             make_float2(c0.x * s0.y - c0.y * s0.x, c1.x * s1.y - c1.y * s1.x);
     } else {
-      float2 b0 = make_float2(bv.x, bv.y), b1 = make_float2(bv.z, bv.w);
       float2 d0 = make_float2(dvv.x, dvv.y), d1 = make_float2(dvv.z, dvv.w);
+      float2 n0 = s0, n1 = s1;                 // numerators b + (h_t/2) nsum
       if (MODE == MODE_INIT) {
         // d_m = 1 + (h_t/2)[|psi|^2 + 2 sum c - eps + i u mu]
         // b_m = psi (2 - d) + (h_t/2)(nsum + 2 zeta)            (Eq. 31, rearranged)
+        const float ht2 = dv.ht2;
         const float a0 = c0.x * c0.x + c0.y * c0.y, a1 = c1.x * c1.x + c1.y * c1.y;
         d0 = make_float2(1.f + ht2 * (a0 + dv.csum2 - ev.x), ht2 * dv.u * muv.x);
         d1 = make_float2(1.f + ht2 * (a1 + dv.csum2 - ev.y), ht2 * dv.u * muv.y);
         float2 z0 = make_float2(0.f, 0.f), z1 = z0;
         if (dv.zeta_max > 0.f) {               // Langevin term, Eq. (39), S11
           const unsigned long long m = (unsigned long long)idx;
-          const PhiloxOut p0 = philox4x32_10((uint32_t)m, (uint32_t)(m >> 32), (uint32_t)nstep, 0u, dv.seed_lo, dv.seed_hi);
-          const PhiloxOut p1 = philox4x32_10((uint32_t)(m + 1), (uint32_t)((m + 1) >> 32), (uint32_t)nstep, 0u, dv.seed_lo, dv.seed_hi);
-          z0 = make_float2(dv.zeta_max * u32_to_pm1(p0.x0), dv.zeta_max * u32_to_pm1(p0.x1));
-          z1 = make_float2(dv.zeta_max * u32_to_pm1(p1.x0), dv.zeta_max * u32_to_pm1(p1.x1));
+          const PhiloxOut p0 = philox4x32_10((uint32_t)m, (uint32_t)(m >> 32), nstep, 0u, dv.seed_lo, dv.seed_hi);
+          const PhiloxOut p1 = philox4x32_10((uint32_t)(m + 1), (uint32_t)((m + 1) >> 32), nstep, 0u, dv.seed_lo, dv.seed_hi);
+          const float zs = 2.f * ht2 * dv.zeta_max;
+          z0 = make_float2(zs * u32_to_pm1(p0.x0), zs * u32_to_pm1(p0.x1));
+          z1 = make_float2(zs * u32_to_pm1(p1.x0), zs * u32_to_pm1(p1.x1));
         }
-        const float2 e0 = make_float2(2.f - d0.x, -d0.y), e1 = make_float2(2.f - d1.x, -d1.y);
-        const float2 q0 = cmul(c0, e0), q1 = cmul(c1, e1);
-        b0 = make_float2(q0.x + ht2 * (s0.x + 2.f * z0.x), q0.y + ht2 * (s0.y + 2.f * z0.y));
-        b1 = make_float2(q1.x + ht2 * (s1.x + 2.f * z1.x), q1.y + ht2 * (s1.y + 2.f * z1.y));
+        const float2 q0 = cmul(c0, make_float2(2.f - d0.x, -d0.y)), q1 = cmul(c1, make_float2(2.f - d1.x, -d1.y));
+        b0 = make_float2(q0.x + s0.x + z0.x, q0.y + s0.y + z0.y);
+        b1 = make_float2(q1.x + s1.x + z1.x, q1.y + s1.y + z1.y);
+        n0 = make_float2(b0.x + s0.x, b0.y + s0.y);
+        n1 = make_float2(b1.x + s1.x, b1.y + s1.y);
         if (act) {
           *reinterpret_cast<float4 *>(dv.b + idx) = make_float4(b0.x, b0.y, b1.x, b1.y);
           *reinterpret_cast<float4 *>(dv.d + idx) = make_float4(d0.x, d0.y, d1.x, d1.y);
         }
       }
       // x^{l+1}_m = (b_m + (h_t/2) nsum) / d_m   (Eq. 33);  |r^l_m|^2 = |d_m|^2 |x^{l+1}_m - x^l_m|^2  (S8)
-      const float2 n0 = make_float2(b0.x + ht2 * s0.x, b0.y + ht2 * s0.y);
-      const float2 n1 = make_float2(b1.x + ht2 * s1.x, b1.y + ht2 * s1.y);
       const float m0 = d0.x * d0.x + d0.y * d0.y, m1 = d1.x * d1.x + d1.y * d1.y;
-      const float i0v = 1.f / m0, i1v = 1.f / m1;
+      const float i0v = __fdividef(1.f, m0), i1v = __fdividef(1.f, m1);
       const float2 y0 = cmulc(d0, n0), y1 = cmulc(d1, n1);
       const float4 out = make_float4(y0.x * i0v, y0.y * i0v, y1.x * i1v, y1.y * i1v);
       if (act) {
@@ -253,15 +292,15 @@ __global__ void __launch_bounds__(512, 2) k_march(const __grid_constant__ Dev dv
         rmax = fmaxf(rmax, fmaxf((e0x * e0x + e0y * e0y) * m0, (e1x * e1x + e1y * e1y) * m1));
       }
     }
-    bv = bn;
-    dvv = dn;
+    idx += plane;
+    const unsigned t = oB; oB = oC; oC = oT; oT = oU; oU = oF; oF = t;     // rotate the ring
   }
 
   if (MODE != MODE_RHO) {
     // max-residual reduction: redux over the warp on the uint pattern (non-negative floats order like
     // uints), one shared atomic per warp, one global atomic per CTA; the last CTA decides (Eq. 34).
     __shared__ unsigned int s_max;
-    const int tid = ty * bx + tx;
+    const int tid = ty * BX + tx;
     if (tid == 0) s_max = 0u;
     __syncthreads();
     const unsigned int w = __reduce_max_sync(0xffffffffu, __float_as_uint(rmax));
@@ -383,18 +422,32 @@ __global__ void k_step_finish(const __grid_constant__ Dev dv, int npart) {
 
 // ------------------------------------------------------------------------------------------------
 // host-side launchers (called from tdgl_api.cu)
+template <int BX, int BY>
+static void launch_march_t(int mode, const Dev &dv, dim3 grid, size_t smem, cudaStream_t st) {
+  const dim3 block(BX, BY, 1);
+  if (mode == MODE_SWEEP) k_march<MODE_SWEEP, BX, BY><<<grid, block, smem, st>>>(dv);
+  else if (mode == MODE_INIT) k_march<MODE_INIT, BX, BY><<<grid, block, smem, st>>>(dv);
+  else k_march<MODE_RHO, BX, BY><<<grid, block, smem, st>>>(dv);
+}
+template <int BX, int BY>
+static cudaError_t march_configure_t(size_t smem) {
+  cudaError_t e = cudaFuncSetAttribute(k_march<MODE_SWEEP, BX, BY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(k_march<MODE_INIT, BX, BY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(k_march<MODE_RHO, BX, BY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+}
+// supported CTA shapes (thread columns x rows): 64x8, 32x16, 16x32
 void launch_march(int mode, const Dev &dv, dim3 grid, dim3 block, size_t smem, cudaStream_t st) {
-  if (mode == MODE_SWEEP) k_march<MODE_SWEEP><<<grid, block, smem, st>>>(dv);
-  else if (mode == MODE_INIT) k_march<MODE_INIT><<<grid, block, smem, st>>>(dv);
-  else k_march<MODE_RHO><<<grid, block, smem, st>>>(dv);
+  if (block.x == 64) launch_march_t<64, 8>(mode, dv, grid, smem, st);
+  else if (block.x == 32) launch_march_t<32, 16>(mode, dv, grid, smem, st);
+  else launch_march_t<16, 32>(mode, dv, grid, smem, st);
 }
 size_t march_smem_bytes(dim3 block) { return (size_t)NBUF * (block.y + 2) * (2 * block.x + 4) * sizeof(float2); }
-cudaError_t march_configure(size_t smem) {
-  cudaError_t e = cudaFuncSetAttribute(k_march<MODE_SWEEP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (e != cudaSuccess) return e;
-  e = cudaFuncSetAttribute(k_march<MODE_INIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (e != cudaSuccess) return e;
-  return cudaFuncSetAttribute(k_march<MODE_RHO>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+cudaError_t march_configure(dim3 block, size_t smem) {
+  if (block.x == 64) return march_configure_t<64, 8>(smem);
+  if (block.x == 32) return march_configure_t<32, 16>(smem);
+  return march_configure_t<16, 32>(smem);
 }
 void launch_jav(const Dev &dv, int nblocks, cudaStream_t st) { k_jav_partial<<<nblocks, 256, 0, st>>>(dv); }
 void launch_step_begin(const Dev &dv, cudaStream_t st) { k_step_begin<<<1, 256, 0, st>>>(dv); }

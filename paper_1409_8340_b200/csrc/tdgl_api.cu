@@ -10,7 +10,7 @@
 // launchers defined in the kernel files
 void launch_march(int mode, const Dev &dv, dim3 grid, dim3 block, size_t smem, cudaStream_t st);
 size_t march_smem_bytes(dim3 block);
-cudaError_t march_configure(size_t smem);
+cudaError_t march_configure(dim3 block, size_t smem);
 void launch_jav(const Dev &dv, int nblocks, cudaStream_t st);
 void launch_step_begin(const Dev &dv, cudaStream_t st);
 void launch_step_finish(const Dev &dv, int npart, cudaStream_t st);
@@ -207,7 +207,6 @@ extern "C" int tdgl_create(const tdgl_params *p, tdgl_t **out) {
   int bx = 64;
   while (bx > 16 && bx * 2 > p->nx) bx >>= 1;
   int by = 512 / bx;
-  while (by > 4 && by / 2 >= p->ny) by >>= 1;
   h->mblock = dim3(bx, by, 1);
   const unsigned gx = (p->nx + 2 * bx - 1) / (2 * bx), gy = (p->ny + by - 1) / by;
   // z chunks: enough CTAs for ~4 waves of 2 CTAs/SM, chunks of at least 8 planes
@@ -222,7 +221,7 @@ extern "C" int tdgl_create(const tdgl_params *p, tdgl_t **out) {
     h->jav_blocks = (int)(nb < 1 ? 1 : (nb > TDGL_NPART ? TDGL_NPART : nb));
   }
   h->pred_sweeps = 1;
-  CK(march_configure(h->msmem));
+  CK(march_configure(h->mblock, h->msmem));
   CK(poisson_configure(p->nx, p->ny, p->nz));
   CK(cudaMallocHost((void **)&h->h_flag, 64));
   CK(cudaEventCreate(&h->ev0));
