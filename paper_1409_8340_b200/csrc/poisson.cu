@@ -243,26 +243,51 @@ __global__ void __launch_bounds__(128) k_thomas_z(float *__restrict__ data, floa
   const double rs = (double)scale / (double)cz;
   float *x = data + col;
   float *c = cp + col;
-  double cprev = 2.0 / bq;                            // row 0: off-diagonal 2
-  double dprev = (double)x[0] * rs / bq;
-  c[0] = (float)cprev;
-  x[0] = (float)dprev;
-  for (int k = 1; k < nz; ++k) {
-    const double a = (k == nz - 1) ? 2.0 : 1.0;
-    const double den = bq - a * cprev;
-    const double rhs = (double)x[k * plane] * rs;
-    double inv, dk;
-    if (zero && k == nz - 1) { inv = 0.0; dk = 0.0; }
-    else { inv = 1.0 / den; dk = (rhs - a * dprev) * inv; }
-    cprev = inv;
-    dprev = dk;
-    c[k * plane] = (float)cprev;
-    x[k * plane] = (float)dk;
+  // forward elimination, 8 planes per batch so that 8 independent loads are in flight per thread
+  double cprev = 0.0, dprev = 0.0;
+  for (int kb = 0; kb < nz; kb += 8) {
+    float xin[8];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) xin[u] = (kb + u < nz) ? __ldcs(x + (long long)(kb + u) * plane) : 0.f;
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      const int k = kb + u;
+      if (k < nz) {
+        const double rhs = (double)xin[u] * rs;
+        double inv, dk;
+        if (k == 0) {                                   // row 0: off-diagonal 2
+          inv = 2.0 / bq;
+          dk = rhs / bq;
+        } else {
+          const double a = (k == nz - 1) ? 2.0 : 1.0;
+          if (zero && k == nz - 1) { inv = 0.0; dk = 0.0; }
+          else { inv = 1.0 / (bq - a * cprev); dk = (rhs - a * dprev) * inv; }
+        }
+        cprev = inv;
+        dprev = dk;
+        c[(long long)k * plane] = (float)inv;
+        x[(long long)k * plane] = (float)dk;
+      }
+    }
   }
-  double xn = dprev;                                   // back substitution
-  for (int k = nz - 2; k >= 0; --k) {
-    xn = (double)x[k * plane] - (double)c[k * plane] * xn;
-    x[k * plane] = (float)xn;
+  // back substitution, same batching (descending)
+  double xn = 0.0;
+  for (int kb = nz - 1; kb >= 0; kb -= 8) {
+    float xv[8], cv[8];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      const int k = kb - u;
+      xv[u] = (k >= 0) ? x[(long long)k * plane] : 0.f;
+      cv[u] = (k >= 0) ? __ldcs(c + (long long)k * plane) : 0.f;
+    }
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      const int k = kb - u;
+      if (k >= 0) {
+        xn = (k == nz - 1) ? (double)xv[u] : (double)xv[u] - (double)cv[u] * xn;
+        x[(long long)k * plane] = (float)xn;
+      }
+    }
   }
   if (zero) {
     double s = 0.0;
@@ -298,6 +323,13 @@ __global__ void k_build_tables(float *lam, float2 *tw, double *tab, int n, int o
 // ---------------------------------------------------------------------------------------------
 static bool is_pow2(int n) { return n >= 4 && (n & (n - 1)) == 0; }
 
+// register-blocked fast path (fft.cu)
+bool dht_fast_supported(int n);
+cudaError_t dht_fast_configure(int n);
+void launch_dht_x_fast(float *data, int n, long long nrows, const float2 *tw, cudaStream_t st);
+void launch_dht_s_fast(float *data, int n, long long stride, long long ostride, int ncolc, int nother, const float2 *tw,
+                       int divide, float scale, const float *lx, const float *ly, const float *lz, cudaStream_t st);
+
 struct PoissonPlan {
   int nx, ny, nz, bc[3];
   float cz, scale;
@@ -325,6 +357,8 @@ cudaError_t poisson_configure(int nx, int ny, int nz) {
     for (int kind = 0; kind < 2; ++kind) { size_t s = smem_generic(n, kind, tl_generic(n)); if (s > c) c = s; }
   }
   cudaError_t e;
+  for (int ax = 0; ax < 3; ++ax)
+    if (dht_fast_supported(ns[ax]) && (e = dht_fast_configure(ns[ax])) != cudaSuccess) return e;
   if (a && (e = cudaFuncSetAttribute(k_dht_x, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)a)) != cudaSuccess) return e;
   if (b && (e = cudaFuncSetAttribute(k_dht_strided, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)b)) != cudaSuccess) return e;
   return cudaFuncSetAttribute(k_transform_generic, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c);
@@ -341,6 +375,15 @@ static int transform_axis(const Dev &dv, float *data, int axis, bool divide, flo
   const int n = ns[axis];
   const bool open = bcs[axis] == 1;
   const long long plane = (long long)dv.nx * dv.ny;
+  if (!open && dht_fast_supported(n)) {
+    if (axis == 0) {
+      launch_dht_x_fast(data, n, (long long)dv.ny * dv.nz, dv.tw[0], st);
+    } else {
+      launch_dht_s_fast(data, n, axis == 1 ? dv.nx : plane, axis == 1 ? plane : dv.nx, dv.nx / 2,
+                        axis == 1 ? dv.nz : dv.ny, dv.tw[axis], divide ? 1 : 0, scale, dv.lam[0], dv.lam[1], dv.lam[2], st);
+    }
+    return 1;
+  }
   if (!open && is_pow2(n)) {
     if (axis == 0) {
       const long long nrows = (long long)dv.ny * dv.nz;
