@@ -47,10 +47,15 @@ def measured_peak():
 
 
 def ncu_traffic():
-    """Per-launch DRAM bytes of the sweep kernel from the committed ncu capture, if any."""
+    """Per-launch DRAM bytes of the sweep kernel from the committed ncu capture (profiles/sweep_traffic.txt)."""
     try:
-        with open(os.path.join(ROOT, "profiles", "sweep_traffic.json")) as f:
-            d = json.load(f)
+        d = {}
+        with open(os.path.join(ROOT, "profiles", "sweep_traffic.txt")) as f:
+            for line in f:
+                if line.startswith("#") or not line.strip():
+                    continue
+                k, v = line.split()
+                d[k] = int(v)
         return d
     except Exception:
         return None
