@@ -323,6 +323,11 @@ __global__ void k_build_tables(float *lam, float2 *tw, double *tab, int n, int o
 // ---------------------------------------------------------------------------------------------
 static bool is_pow2(int n) { return n >= 4 && (n & (n - 1)) == 0; }
 
+// Bluestein DCT-I fast path (dct.cu)
+void launch_dct_x(float *data, int n, int LB, long long nrows, const float2 *T, const float2 *C, const float2 *H,
+                  cudaStream_t st);
+void launch_dct_s(float *data, int n, int LB, long long stride, long long ostride, int ncolc, int nother,
+                  const float2 *T, const float2 *C, const float2 *H, cudaStream_t st);
 // register-blocked fast path (fft.cu)
 bool dht_fast_supported(int n);
 cudaError_t dht_fast_configure(int n);
@@ -375,6 +380,12 @@ static int transform_axis(const Dev &dv, float *data, int axis, bool divide, flo
   const int n = ns[axis];
   const bool open = bcs[axis] == 1;
   const long long plane = (long long)dv.nx * dv.ny;
+  if (open && dv.bLB[axis] && !divide) {
+    if (axis == 0) launch_dct_x(data, n, dv.bLB[0], (long long)dv.ny * dv.nz, dv.bT[0], dv.bC[0], dv.bH[0], st);
+    else launch_dct_s(data, n, dv.bLB[axis], axis == 1 ? dv.nx : plane, axis == 1 ? plane : dv.nx, dv.nx / 2,
+                      axis == 1 ? dv.nz : dv.ny, dv.bT[axis], dv.bC[axis], dv.bH[axis], st);
+    return 1;
+  }
   if (!open && dht_fast_supported(n)) {
     if (axis == 0) {
       launch_dht_x_fast(data, n, (long long)dv.ny * dv.nz, dv.tw[0], st);

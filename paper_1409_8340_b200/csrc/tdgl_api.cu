@@ -17,6 +17,9 @@ void launch_step_finish(const Dev &dv, int npart, cudaStream_t st);
 cudaError_t poisson_configure(int nx, int ny, int nz);
 void launch_build_tables(float *lam, float2 *tw, double *tab, int n, int open, double c, cudaStream_t st);
 int poisson_solve(const Dev &dv, float *data, bool thomas_open_z, cudaStream_t st);
+int dct_fast_lb(int n);
+cudaError_t dct_fast_configure(int LB);
+void launch_build_bluestein(float2 *T, float2 *C, float2 *H, int n, int LB, cudaStream_t st);
 void launch_init_state(const Dev &dv, float amp, cudaStream_t st);
 void launch_ctl_reset(const Dev &dv, float tol, int maxs, int fixed, cudaStream_t st);
 void launch_ctl_solver(const Dev &dv, float tol, int maxs, int fixed, cudaStream_t st);
@@ -90,6 +93,9 @@ static size_t carve(const tdgl_params *p, char *base, Dev *dv) {
     q = take(ns[a] * sizeof(float)); if (dv) dv->lam[a] = (float *)q;
     q = take(ns[a] * sizeof(float2)); if (dv) dv->tw[a] = (float2 *)q;
     q = take(2 * (size_t)ns[a] * sizeof(double)); if (dv) dv->tab[a] = (double *)q;
+    q = take(4096 * sizeof(float2)); if (dv) dv->bT[a] = (float2 *)q;
+    q = take(4096 * sizeof(float2)); if (dv) dv->bC[a] = (float2 *)q;
+    q = take(4096 * sizeof(float2)); if (dv) dv->bH[a] = (float2 *)q;
   }
   q = take((size_t)TDGL_NPART * 4 * sizeof(double)); if (dv) dv->part = (double *)q;
   q = take(TDGL_LOGCAP * sizeof(int)); if (dv) dv->sweep_log = (int *)q;
@@ -232,6 +238,14 @@ extern "C" int tdgl_create(const tdgl_params *p, tdgl_t **out) {
   const int ns[3] = {p->nx, p->ny, p->nz};
   const double cs[3] = {cx, cy, cz};
   for (int a = 0; a < 3; ++a) launch_build_tables(dv.lam[a], dv.tw[a], dv.tab[a], ns[a], p->bc[a], cs[a], st);
+  for (int a = 0; a < 3; ++a) {
+    dv.bLB[a] = (p->bc[a] == TDGL_BC_OPEN) ? dct_fast_lb(ns[a]) : 0;
+    if (dv.bLB[a]) {
+      CK(dct_fast_configure(dv.bLB[a]));
+      launch_build_bluestein(dv.bT[a], dv.bC[a], dv.bH[a], ns[a], dv.bLB[a], st);
+      h->launches += 1;
+    }
+  }
   launch_init_state(dv, p->init_amp, st);
   launch_set_field(dv, 0.0, 0.0, 0.0, st);
   launch_step_begin(dv, st);

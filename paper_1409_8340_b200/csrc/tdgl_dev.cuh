@@ -58,6 +58,8 @@ struct Dev {
   float *lam[3];            // eigenvalues of the 1-D operators per axis
   float2 *tw[3];            // FFT twiddles exp(-2 pi i m/n) per axis (power-of-two periodic axes)
   double *tab[3];           // generic transform tables: cas(2 pi m/n) or cos(pi m/(n-1))
+  float2 *bT[3], *bC[3], *bH[3];   // Bluestein tables of the fast DCT-I per open axis (dct.cu)
+  int bLB[3];               // its FFT length, 0 = axis not open / not supported
   double *part;             // TDGL_NPART*4 partial sums
   int *sweep_log; float *resid_log; int *sched;
   unsigned long long cond_handle;   // cudaGraphConditionalHandle of the WHILE node (graph mode)

@@ -131,7 +131,9 @@ def test_poisson_solve(bc, shape):
 
 @pytest.mark.parametrize("bc,shape", [((P_, P_, O_), (512, 256, 6)), ((P_, P_, P_), (256, 128, 64)),
                                       ((P_, P_, O_), (128, 1024, 3)), ((P_, P_, P_), (1024, 64, 128)),
-                                      ((P_, O_, P_), (64, 20, 256)), ((O_, P_, P_), (30, 512, 64))])
+                                      ((P_, O_, P_), (64, 20, 256)), ((O_, P_, P_), (30, 512, 64)),
+                                      ((O_, O_, O_), (1024, 40, 6)), ((P_, O_, O_), (64, 1000, 5)),
+                                      ((O_, O_, P_), (514, 300, 8)), ((O_, P_, O_), (1366, 64, 3))])
 def test_poisson_solve_fast_transform_sizes(bc, shape):
     """The register-blocked Hartley kernels (n = 64..1024), x pass, strided pass and the fused
     transform-divide-transform of a periodic z axis."""
