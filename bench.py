@@ -110,6 +110,24 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def reduce_over_ranks(vals, dist=None, device=None):
+    """[time, count, count, ...] of this rank -> (max over ranks of vals[0], sums over ranks of the rest).
+    Replicas only: this all-reduce of a few scalars AFTER the timed region is the only
+    communication of the N > 1 bench; nothing on the data path is exchanged."""
+    import torch
+    t = torch.tensor([float(v) for v in vals], dtype=torch.float64, device=device)
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return [float(x) for x in t]
+    tmax = t.clone(); dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    tsum = t.clone(); dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
+    return [float(tmax[0])] + [float(x) for x in tsum[1:]]
+
+
+def throughput(n_sites, sweeps_all, steps_per_rank, world, ms):
+    """(site-iterations/s, steps/s) of the whole job: units all ranks processed / max-over-ranks time."""
+    return n_sites * sweeps_all / (ms * 1e-3), world * steps_per_rank / (ms * 1e-3)
+
+
 def make_solver(cfg: I.Config, host_loop=False, seed_offset=0):
     from paper_1409_8340_b200 import Solver
     s = Solver(cfg.nx, cfg.ny, cfg.nz, bc=cfg.bc, h=cfg.h, dt=cfg.dt, eps_tol=1e-6, max_sweeps=100,
@@ -228,16 +246,10 @@ def main():
     ob1 = s.observables()
     launches = s.launch_count() - l0 - 2           # minus the two observables kernels
     sweeps = ob1.sweeps_total - ob0.sweeps_total
-    t = torch.tensor([ms, float(sweeps), float(launches)], dtype=torch.float64, device=dev)
-    if world > 1:
-        tmax = t.clone(); dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        tsum = t.clone(); dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
-        ms, sweeps_all, launches_all = float(tmax[0]), float(tsum[1]), int(tsum[2])
-    else:
-        sweeps_all, launches_all = float(sweeps), int(launches)
+    ms, sweeps_all, launches_all = reduce_over_ranks([ms, sweeps, launches], dist if world > 1 else None, dev)
+    launches_all = int(launches_all)
     N = cfg.n_sites
-    value = N * sweeps_all / (ms * 1e-3)
-    steps_per_s = world * K / (ms * 1e-3)
+    value, steps_per_s = throughput(N, sweeps_all, K, world, ms)
 
     # ---- roofline of the sweep kernel: CUDA events around every sweep launch (host-loop run) ----
     roof = None
@@ -290,11 +302,7 @@ def main():
                 torch.cuda.synchronize()
             te = time.perf_counter() - t0
             sw_e = obx.sweeps_total - sw_a
-            te_t = torch.tensor([te, float(sw_e)], dtype=torch.float64, device=dev)
-            if world > 1:
-                a_ = te_t.clone(); dist.all_reduce(a_, op=dist.ReduceOp.MAX)
-                b_ = te_t.clone(); dist.all_reduce(b_, op=dist.ReduceOp.SUM)
-                te, sw_e = float(a_[0]), float(b_[1])
+            te, sw_e = reduce_over_ranks([te, sw_e], dist if world > 1 else None, dev)
             e2e = {"value": N * sw_e / te, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                    "steps": Ke, "ms_per_step": 1e3 * te / Ke, "steps_per_s": world * Ke / te}
     s.close()
