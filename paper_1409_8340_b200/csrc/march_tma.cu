@@ -1,0 +1,501 @@
+// The z-marching 7-point link-variable stencil, TMA edition (sm_100a): Jacobi sweep + max-residual (a4,
+// Eq. 33-34), fused init + first sweep (a3, with the Philox Langevin term a2,
+// Eq. 39), rho = div j_s (a6).
+//
+// A CTA of 8 warps owns a 128 x 8 tile of the xy plane and marches through a chunk of z planes.  One
+// elected thread per plane issues bulk tensor copies (cp.async.bulk.tensor, TMA) that land a whole
+// stage in shared memory -- the psi plane k+1 of the tile (centre 128 x 8, the two ghost rows, the two
+// ghost columns; wrapped or mirrored coordinates chosen by the issuing thread) plus, for
+// the sweep, the b and d tiles of plane k -- and completes on the stage's mbarrier.  Stages form a ring;
+// two are being read while the others are in flight, so a CTA keeps 2 x 26 KB outstanding and the
+// arithmetic warps never compute a global address for a load.
+// A warp owns one row; lane l owns the site pairs (2l, 2l+1) and (64+2l, 64+2l+1): every shared-memory
+// access is a conflict-free 16-byte vector.  The thread keeps its values of planes k-1 and k in
+// registers (z marching), reads plane k+1 (own sites) from the newest stage and the y neighbours and
+// tile-edge x neighbours of plane k from the previous stage; x neighbours inside the warp come from
+// shuffles.  32 B/site/sweep of HBM traffic: x^l 8, b 8, d 8 read, x^{l+1} 8 written.
+#include "tdgl_dev.cuh"
+#include "philox.cuh"
+#include "march_tma.h"
+#include <cuda_device_runtime_api.h>
+
+#define MODE_SWEEP 0
+#define MODE_INIT  1
+#define MODE_RHO   2
+
+namespace {
+
+constexpr int TW = 128;                 // tile width (sites)
+constexpr int TH = 8;                   // tile height (rows) = warps per CTA
+constexpr int NTHREADS = 32 * TH;
+// stage layout (bytes); every block is a TMA destination (128-byte aligned)
+constexpr unsigned OFF_C = 0;           // psi centre: TH rows, pitch = 8 * min(TW, nx) bytes
+constexpr unsigned OFF_RLO = 8192;      // ghost row j0 - 1
+constexpr unsigned OFF_RHI = 9216;      // ghost row j0 + nvy
+constexpr unsigned OFF_XW = 10240;      // ghost column pair (i0-2, i0-1): TH x 16 B
+constexpr unsigned OFF_XE = 10368;      // ghost column pair (i0+nv, i0+nv+1)
+constexpr unsigned OFF_B = 10496;       // b tile (sweep only)
+constexpr unsigned OFF_D = 18688;       // d tile (sweep only)
+constexpr unsigned STAGE_PSI = 10496, STAGE_SWEEP = 26880;
+constexpr unsigned HDR = 128;           // mbarriers (8 B each) + the CTA residual word at byte 96
+
+template <int MODE> struct Cfg {
+  static constexpr int NS = (MODE == MODE_SWEEP) ? 4 : 6;                       // stages in the ring
+  static constexpr unsigned SB = (MODE == MODE_SWEEP) ? STAGE_SWEEP : STAGE_PSI; // bytes per stage
+  static constexpr unsigned SMEM = HDR + NS * SB;
+};
+
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred P1;\n"
+      "LAB_WAIT:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+      "@P1 bra DONE;\n"
+      "bra LAB_WAIT;\n"
+      "DONE:\n"
+      "}\n" ::"r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(unsigned dst, const CUtensorMap *map, int c0, int c1, int c2, unsigned bar) {
+  asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];\n"
+               ::"r"(dst), "l"(map), "r"(bar), "r"(c0), "r"(c1), "r"(c2) : "memory");
+}
+__device__ __forceinline__ float4 lds128(unsigned a) {
+  float4 v;
+  asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];\n" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a));
+  return v;
+}
+__device__ __forceinline__ float2 lds64(unsigned a) {
+  float2 v;
+  asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];\n" : "=f"(v.x), "=f"(v.y) : "r"(a));
+  return v;
+}
+__device__ __forceinline__ float rcp_approx(float x) {
+  float y;
+  asm("rcp.approx.ftz.f32 %0, %1;\n" : "=f"(y) : "f"(x));
+  return y;
+}
+__device__ __forceinline__ float2 lo(const float4 &v) { return make_float2(v.x, v.y); }
+__device__ __forceinline__ float2 hi(const float4 &v) { return make_float2(v.z, v.w); }
+__device__ __forceinline__ float4 cmul4(float2 a, const float4 &v) {      // a * both sites
+  const float2 p = cmul(a, lo(v)), q = cmul(a, hi(v));
+  return make_float4(p.x, p.y, q.x, q.y);
+}
+__device__ __forceinline__ float4 cmulc4(float2 a, const float4 &v) {     // conj(a) * both sites
+  const float2 p = cmulc(a, lo(v)), q = cmulc(a, hi(v));
+  return make_float4(p.x, p.y, q.x, q.y);
+}
+
+// per-thread link constants, already scaled:  f c_x U_x(j),  f c_z U_z(j),  f c_y   (f = h_t/2 or 1)
+struct Links { float2 ux, uz; float cy; };
+
+// s += f [ c_x (U_x E + U_x* W) + c_y (N + S) + c_z (U_z T + U_z* B) ]  for the two sites of a pair:
+//   U E + U* W = U.re (E + W) + i U.im (E - W): 10 adds and 10 FMAs per site (Eq. 29a)
+__device__ __forceinline__ void nsum_pair(const Links &L, const float4 &C, const float2 &W, const float2 &E,
+                                          const float4 &Nn, const float4 &Ss, const float4 &T, const float4 &B,
+                                          float2 &s0, float2 &s1) {
+  // site 0: west W, east C.hi;  site 1: west C.lo, east E
+  s0.x = fmaf(L.ux.x, C.z + W.x, s0.x);  s0.x = fmaf(-L.ux.y, C.w - W.y, s0.x);
+  s0.y = fmaf(L.ux.x, C.w + W.y, s0.y);  s0.y = fmaf(L.ux.y, C.z - W.x, s0.y);
+  s1.x = fmaf(L.ux.x, E.x + C.x, s1.x);  s1.x = fmaf(-L.ux.y, E.y - C.y, s1.x);
+  s1.y = fmaf(L.ux.x, E.y + C.y, s1.y);  s1.y = fmaf(L.ux.y, E.x - C.x, s1.y);
+  s0.x = fmaf(L.cy, Nn.x + Ss.x, s0.x);  s0.y = fmaf(L.cy, Nn.y + Ss.y, s0.y);
+  s1.x = fmaf(L.cy, Nn.z + Ss.z, s1.x);  s1.y = fmaf(L.cy, Nn.w + Ss.w, s1.y);
+  s0.x = fmaf(L.uz.x, T.x + B.x, s0.x);  s0.x = fmaf(-L.uz.y, T.y - B.y, s0.x);
+  s0.y = fmaf(L.uz.x, T.y + B.y, s0.y);  s0.y = fmaf(L.uz.y, T.x - B.x, s0.y);
+  s1.x = fmaf(L.uz.x, T.z + B.z, s1.x);  s1.x = fmaf(-L.uz.y, T.w - B.w, s1.x);
+  s1.y = fmaf(L.uz.x, T.w + B.w, s1.y);  s1.y = fmaf(L.uz.y, T.z - B.z, s1.y);
+}
+
+// x^{l+1} = n / d for both sites of a pair (Eq. 33) and |r^l|^2 = |d|^2 |x^{l+1} - x^l|^2 (S8)
+__device__ __forceinline__ float4 divide_pair(const float2 &n0, const float2 &n1, const float4 &d, const float4 &C,
+                                              float &rmax) {
+  const float m0 = d.x * d.x + d.y * d.y, m1 = d.z * d.z + d.w * d.w;
+  const float i0 = rcp_approx(m0), i1 = rcp_approx(m1);
+  const float2 y0 = cmulc(lo(d), n0), y1 = cmulc(hi(d), n1);
+  const float4 out = make_float4(y0.x * i0, y0.y * i0, y1.x * i1, y1.y * i1);
+  const float e0x = out.x - C.x, e0y = out.y - C.y, e1x = out.z - C.z, e1y = out.w - C.w;
+  rmax = fmaxf(rmax, fmaxf((e0x * e0x + e0y * e0y) * m0, (e1x * e1x + e1y * e1y) * m1));
+  return out;
+}
+
+// The decision taken by the last CTA of a sweep (Eq. 34; S8: residual of the input iterate,
+// keep the new one; S9/S10: prescribed counts, cap).
+__device__ __noinline__ void sweep_decide2(const Dev &dv, int l) {
+  Ctl *c = dv.ctl;
+  const float r2 = __uint_as_float(atomicMax(&c->resid_bits[l], 0u));
+  const int sweeps = l + 1;
+  c->sweeps = sweeps;
+  c->xbuf ^= 1;
+  int target = c->fixed_sweeps;
+  if (c->sched_pos < c->sched_n) target = dv.sched[c->sched_pos];
+  bool done;
+  if (target > 0) {
+    done = sweeps >= target;
+  } else {
+    done = (r2 < c->eps_tol) || sweeps >= c->max_sweeps;
+    if (!(r2 < c->eps_tol) && sweeps >= c->max_sweeps) c->status = 1;
+  }
+  if (done) {
+    c->done = 1;
+    c->sweeps_last = sweeps;
+    c->resid_last = r2;
+  }
+  if (dv.use_cond) cudaGraphSetConditional((cudaGraphConditionalHandle)dv.cond_handle, done ? 0u : 1u);
+  __threadfence();
+}
+
+template <int MODE>
+__global__ void __launch_bounds__(NTHREADS, 2) k_march_tma(const __grid_constant__ Dev dv,
+                                                           const __grid_constant__ MarchMaps mm) {
+  constexpr int NS = Cfg<MODE>::NS;
+  constexpr int DEPTH = NS - 2;                       // stages in flight beyond the two being read
+  constexpr unsigned SB = Cfg<MODE>::SB;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  Ctl *ctl = dv.ctl;
+  int l = 0;
+  if (MODE != MODE_RHO) {
+    if (ctl->done) return;
+    l = ctl->sweeps;
+  }
+  const int xb = ctl->xbuf;
+
+  const int nx = dv.nx, ny = dv.ny, nz = dv.nz;
+  const int tid = threadIdx.x, lane = tid & 31, row = tid >> 5;
+  const int i0 = blockIdx.x * TW, j0 = blockIdx.y * TH;
+  const int nv = min(TW, nx - i0), nvy = min(TH, ny - j0);          // valid sites per row, valid rows
+  const int k0 = blockIdx.z * dv.zc, k1 = min(nz, k0 + dv.zc);      // planes [k0, k1)
+  const int nk = k1 - k0;
+  const bool px = dv.bcx == 0, py = dv.bcy == 0, pz = dv.bcz == 0;
+  const long long plane = (long long)nx * ny;
+  const unsigned pitch = 8u * (unsigned)min(TW, nx);                // bytes per row of a tile in smem
+  const unsigned bh = (unsigned)min(TH, ny);
+  const unsigned sbase = smem_u32(smem_raw);
+  const unsigned stage0 = sbase + HDR;
+
+  auto zwrap = [&](int kp) -> int {                                 // plane index with wrap / mirror
+    if (kp < 0) return pz ? nz - 1 : 1;
+    if (kp >= nz) return pz ? 0 : nz - 2;
+    return kp;
+  };
+
+  // ---- producer side: coordinates of the five psi boxes of this tile (floats in x) ----------------
+  const int cx0 = 2 * i0;
+  const int yLo = (j0 > 0) ? j0 - 1 : (py ? ny - 1 : 1);
+  const int yHi = (j0 + nvy < ny) ? j0 + nvy : (py ? 0 : ny - 2);
+  const int xW = 2 * ((i0 > 0) ? i0 - 2 : nx - 2);
+  const int xE = 2 * ((i0 + nv < nx) ? i0 + nv : 0);
+  const unsigned tx_psi = pitch * bh + 2u * pitch + 2u * 16u * bh;
+  const unsigned tx_bd = 2u * pitch * bh;
+  const CUtensorMap *mC = &mm.psiC[xb], *mR = &mm.psiR[xb], *mX = &mm.psiX[xb];
+  // stage t holds psi plane k0 + t (the "k+1" plane of iteration k = k0 + t - 1) and b, d of plane k0 + t - 1
+  auto issue = [&](int t) {
+    const unsigned slot = (unsigned)t % NS;
+    const unsigned sb = stage0 + slot * SB, bar = sbase + 8u * slot;
+    const int kz = zwrap(k0 + t);
+    const bool bd = (MODE == MODE_SWEEP) && t >= 1;
+    mbar_expect_tx(bar, tx_psi + (bd ? tx_bd : 0u));
+    tma_load_3d(sb + OFF_C, mC, cx0, j0, kz, bar);
+    tma_load_3d(sb + OFF_RLO, mR, cx0, yLo, kz, bar);
+    tma_load_3d(sb + OFF_RHI, mR, cx0, yHi, kz, bar);
+    tma_load_3d(sb + OFF_XW, mX, xW, j0, kz, bar);
+    tma_load_3d(sb + OFF_XE, mX, xE, j0, kz, bar);
+    if (bd) {
+      tma_load_3d(sb + OFF_B, &mm.bC, cx0, j0, k0 + t - 1, bar);
+      tma_load_3d(sb + OFF_D, &mm.dC, cx0, j0, k0 + t - 1, bar);
+    }
+  };
+
+  if (tid == 0) {
+    for (int s = 0; s < NS; ++s) mbar_init(sbase + 8u * s, 1u);
+    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+    *reinterpret_cast<unsigned *>(smem_raw + 96) = 0u;              // CTA max-residual word
+  }
+  __syncthreads();
+  if (tid == 0)
+    for (int t = 0; t <= DEPTH && t <= nk; ++t) issue(t);
+
+  // ---- consumer side: fixed per-thread geometry ----------------------------------------------------
+  const int j = j0 + row;
+  const int jc = min(j, ny - 1);
+  const int iA = i0 + 2 * lane, iB = iA + 64;
+  const bool rowact = row < nvy;
+  const bool actA = rowact && 2 * lane < nv, actB = rowact && 64 + 2 * lane < nv;
+  const int e = nv - 1;                                              // last valid site of the tile row (odd)
+  // shared-memory offsets relative to a stage base
+  const unsigned oA = OFF_C + (unsigned)row * pitch + 16u * lane, oB = oA + 512u;
+  const unsigned oNA = (row == nvy - 1) ? OFF_RHI + 16u * lane : oA + pitch, oNB = oNA + 512u;
+  const unsigned oSA = (row == 0) ? OFF_RLO + 16u * lane : oA - pitch, oSB = oSA + 512u;
+  // x neighbours that do not come from the shuffle: tile edges, the seam between the two halves
+  const bool wA_h = lane == 0, wB_h = lane == 0;
+  const bool eA_h = (lane == 31) || (2 * lane + 1 == e), eB_h = (lane == 31) || (64 + 2 * lane + 1 == e);
+  const unsigned oWA = OFF_XW + 16u * row + 8u;                                      // site i0 - 1
+  const unsigned oWB = OFF_C + (unsigned)row * pitch + 8u * 63u;                    // site i0 + 63
+  const unsigned oEA = (2 * lane + 1 == e) ? OFF_XE + 16u * row : OFF_C + (unsigned)row * pitch + 8u * 64u;
+  const unsigned oEB = OFF_XE + 16u * row;                                           // site i0 + nv
+  // boundary roles
+  const bool ylo = py && j == 0, yhi = py && j == ny - 1;           // quasi-periodic jump rows (warp-uniform)
+  const bool xloA = !px && iA == 0, xhiA = !px && iA + 1 == nx - 1;
+  const bool xhiB = !px && iB + 1 == nx - 1;                        // (iB == 0 never happens)
+  const bool xopen = !px && (i0 == 0 || i0 + nv == nx);             // CTA-uniform
+
+  const float f = (MODE == MODE_RHO) ? 1.f : dv.ht2;
+  Links L;
+  {
+    const float2 Ux = dv.Ux[jc], Uz = dv.Uz[jc];
+    L.ux = make_float2(f * dv.cx * Ux.x, f * dv.cx * Ux.y);
+    L.uz = make_float2(f * dv.cz * Uz.x, f * dv.cz * Uz.y);
+    L.cy = f * dv.cy;
+  }
+  unsigned nstep = 0;
+  if (MODE == MODE_INIT) nstep = (unsigned)ctl->n;
+  float rmax = 0.f;
+
+  // element index of pair A in plane k0 (float2 units); clamped so that inactive threads stay in range
+  const long long rowoff = (long long)jc * nx + min(iA, nx - 2);
+  long long idx = (long long)k0 * plane + rowoff;
+  const float2 *__restrict__ xin = dv.psi[xb];
+  float2 *__restrict__ xout = dv.psi[xb ^ 1];
+
+  // planes k0 - 1 (global load, wrapped / mirrored) and k0 (stage 0) of this thread's sites
+  float4 rA[3], rB[3];
+  {
+    const long long ob = (long long)zwrap(k0 - 1) * plane + rowoff;
+    rA[0] = actA ? __ldg(reinterpret_cast<const float4 *>(xin + ob)) : make_float4(0, 0, 0, 0);
+    rB[0] = actB ? __ldg(reinterpret_cast<const float4 *>(xin + ob + 64)) : make_float4(0, 0, 0, 0);
+  }
+  mbar_wait(sbase, 0u);
+  rA[1] = lds128(stage0 + oA);
+  rB[1] = lds128(stage0 + oB);
+
+  // INIT: mu and eps of plane k, prefetched one plane ahead with plain loads (4 B/site arrays whose row
+  // stride need not be a multiple of 16 B, which rules out TMA)
+  float2 muA = make_float2(0.f, 0.f), muB = muA, epA = make_float2(1.f, 1.f), epB = epA;
+  auto load_mu_eps = [&](long long ix, float2 &ma, float2 &mb, float2 &ea, float2 &eb) {
+    if (MODE == MODE_INIT) {
+      if (actA) {
+        if (dv.solve_mu) ma = __ldcs(reinterpret_cast<const float2 *>(dv.mu + ix));
+        ea = __ldg(reinterpret_cast<const float2 *>(dv.eps + ix));
+      }
+      if (actB) {
+        if (dv.solve_mu) mb = __ldcs(reinterpret_cast<const float2 *>(dv.mu + ix + 64));
+        eb = __ldg(reinterpret_cast<const float2 *>(dv.eps + ix + 64));
+      }
+    }
+  };
+  load_mu_eps(idx, muA, muB, epA, epB);
+
+  // one plane: Bv, Cv = this thread's values of planes k-1, k; Tv receives plane k+1
+  auto do_plane = [&](int t, float4 &BvA, float4 &BvB, float4 &CvA, float4 &CvB, float4 &TvA, float4 &TvB) {
+    const int k = k0 + t - 1;
+    const unsigned slot = (unsigned)t % NS, pslot = (unsigned)(t - 1) % NS;
+    __syncthreads();                                   // every warp is done with stage t - 2: its slot is free
+    if (tid == ((t & (TH - 1)) << 5) && t + DEPTH <= nk) issue(t + DEPTH);
+    mbar_wait(sbase + 8u * slot, ((unsigned)t / NS) & 1u);
+    const unsigned cur = stage0 + slot * SB, prv = stage0 + pslot * SB;
+
+    TvA = lds128(cur + oA);
+    TvB = lds128(cur + oB);
+    float4 NA = lds128(prv + oNA), NB = lds128(prv + oNB);
+    float4 SA = lds128(prv + oSA), SB_ = lds128(prv + oSB);
+    float4 bA, bB, dA, dB;
+    if (MODE == MODE_SWEEP) {
+      bA = lds128(cur + OFF_B + oA); bB = lds128(cur + OFF_B + oB);
+      dA = lds128(cur + OFF_D + oA); dB = lds128(cur + OFF_D + oB);
+    }
+    float2 nmuA, nmuB, nepA, nepB;
+    if (MODE == MODE_INIT) {
+      nmuA = muA; nmuB = muB; nepA = epA; nepB = epB;
+      if (t < nk) load_mu_eps(idx + plane, nmuA, nmuB, nepA, nepB);
+    }
+    float2 WA, EA, WB, EB;
+    WA.x = __shfl_up_sync(0xffffffffu, CvA.z, 1);   WA.y = __shfl_up_sync(0xffffffffu, CvA.w, 1);
+    EA.x = __shfl_down_sync(0xffffffffu, CvA.x, 1); EA.y = __shfl_down_sync(0xffffffffu, CvA.y, 1);
+    WB.x = __shfl_up_sync(0xffffffffu, CvB.z, 1);   WB.y = __shfl_up_sync(0xffffffffu, CvB.w, 1);
+    EB.x = __shfl_down_sync(0xffffffffu, CvB.x, 1); EB.y = __shfl_down_sync(0xffffffffu, CvB.y, 1);
+    if (wA_h) WA = lds64(prv + oWA);
+    if (wB_h) WB = lds64(prv + oWB);
+    if (eA_h) EA = lds64(prv + oEA);
+    if (eB_h) EB = lds64(prv + oEB);
+
+    float4 TA = TvA, TB = TvB, BA = BvA, BB = BvB;
+    if (ylo || yhi) {                                  // quasi-periodic jump in y, rows 0 and ny-1 only
+      const float2 Pk = dv.Pk[k];
+      const float4 PiA = *reinterpret_cast<const float4 *>(dv.Pi + min(iA, nx - 2));
+      const float4 PiB = *reinterpret_cast<const float4 *>(dv.Pi + min(iB, nx - 2));
+      const float2 PA0 = cmulc(Pk, lo(PiA)), PA1 = cmulc(Pk, hi(PiA));     // P_{i,k} = Pi[i] conj(Pk[k])
+      const float2 PB0 = cmulc(Pk, lo(PiB)), PB1 = cmulc(Pk, hi(PiB));
+      if (ylo) {                                       // psi_{i,-1,k} = P psi_{i,ny-1,k}
+        const float2 a = cmul(PA0, lo(SA)), b2 = cmul(PA1, hi(SA)), c2 = cmul(PB0, lo(SB_)), d2 = cmul(PB1, hi(SB_));
+        SA = make_float4(a.x, a.y, b2.x, b2.y);
+        SB_ = make_float4(c2.x, c2.y, d2.x, d2.y);
+      }
+      if (yhi) {                                       // psi_{i,ny,k} = P* psi_{i,0,k}
+        const float2 a = cmulc(PA0, lo(NA)), b2 = cmulc(PA1, hi(NA)), c2 = cmulc(PB0, lo(NB)), d2 = cmulc(PB1, hi(NB));
+        NA = make_float4(a.x, a.y, b2.x, b2.y);
+        NB = make_float4(c2.x, c2.y, d2.x, d2.y);
+      }
+    }
+    if (xopen) {                                       // open x faces: W' = U^2 E, E' = U*^2 W
+      const float2 Ux = dv.Ux[jc];
+      const float2 U2 = cmul(Ux, Ux);
+      if (xloA) WA = cmul(U2, hi(CvA));
+      if (xhiA) EA = cmulc(U2, lo(CvA));
+      if (xhiB) EB = cmulc(U2, lo(CvB));
+    }
+    if (!pz && (k == 0 || k == nz - 1)) {              // open z faces, uniform over the CTA
+      const float2 Uz = dv.Uz[jc];
+      const float2 U2 = cmul(Uz, Uz);
+      if (k == 0) { BA = cmul4(U2, TA); BB = cmul4(U2, TB); }
+      else { TA = cmulc4(U2, BA); TB = cmulc4(U2, BB); }
+    }
+
+    float2 sA0 = make_float2(0.f, 0.f), sA1 = sA0, sB0 = sA0, sB1 = sA0;
+    if (MODE == MODE_SWEEP) { sA0 = lo(bA); sA1 = hi(bA); sB0 = lo(bB); sB1 = hi(bB); }
+    nsum_pair(L, CvA, WA, EA, NA, SA, TA, BA, sA0, sA1);
+    nsum_pair(L, CvB, WB, EB, NB, SB_, TB, BB, sB0, sB1);
+
+    if (MODE == MODE_RHO) {
+      // rho_m = sum_alpha c_alpha Im[psi*_m (S+ psi + S- psi)_m]
+      if (actA) *reinterpret_cast<float2 *>(dv.mu + idx) =
+          make_float2(CvA.x * sA0.y - CvA.y * sA0.x, CvA.z * sA1.y - CvA.w * sA1.x);
+      if (actB) *reinterpret_cast<float2 *>(dv.mu + idx + 64) =
+          make_float2(CvB.x * sB0.y - CvB.y * sB0.x, CvB.z * sB1.y - CvB.w * sB1.x);
+    } else {
+      float2 nA0 = sA0, nA1 = sA1, nB0 = sB0, nB1 = sB1;       // numerators b + (h_t/2) nsum
+      if (MODE == MODE_INIT) {
+        // d_m = 1 + (h_t/2)[|psi|^2 + 2 sum c - eps + i u mu]
+        // b_m = psi (2 - d) + (h_t/2)(nsum + 2 zeta)             (Eq. 31, rearranged)
+        const float ht2 = dv.ht2;
+        auto init_pair = [&](const float4 &C, float2 mu, float2 ep, long long ix, bool act, float2 &s0, float2 &s1,
+                             float2 &n0, float2 &n1, float4 &dout) {
+          const float a0 = C.x * C.x + C.y * C.y, a1 = C.z * C.z + C.w * C.w;
+          const float2 d0 = make_float2(1.f + ht2 * (a0 + dv.csum2 - ep.x), ht2 * dv.u * mu.x);
+          const float2 d1 = make_float2(1.f + ht2 * (a1 + dv.csum2 - ep.y), ht2 * dv.u * mu.y);
+          float2 z0 = make_float2(0.f, 0.f), z1 = z0;
+          if (dv.zeta_max > 0.f) {                     // Langevin term, Eq. (39), S11
+            const unsigned long long m = (unsigned long long)ix;
+            const PhiloxOut p0 = philox4x32_10((uint32_t)m, (uint32_t)(m >> 32), nstep, 0u, dv.seed_lo, dv.seed_hi);
+            const PhiloxOut p1 = philox4x32_10((uint32_t)(m + 1), (uint32_t)((m + 1) >> 32), nstep, 0u, dv.seed_lo, dv.seed_hi);
+            const float zs = 2.f * ht2 * dv.zeta_max;
+            z0 = make_float2(zs * u32_to_pm1(p0.x0), zs * u32_to_pm1(p0.x1));
+            z1 = make_float2(zs * u32_to_pm1(p1.x0), zs * u32_to_pm1(p1.x1));
+          }
+          const float2 q0 = cmul(lo(C), make_float2(2.f - d0.x, -d0.y)), q1 = cmul(hi(C), make_float2(2.f - d1.x, -d1.y));
+          const float2 b0 = make_float2(q0.x + s0.x + z0.x, q0.y + s0.y + z0.y);
+          const float2 b1 = make_float2(q1.x + s1.x + z1.x, q1.y + s1.y + z1.y);
+          n0 = make_float2(b0.x + s0.x, b0.y + s0.y);
+          n1 = make_float2(b1.x + s1.x, b1.y + s1.y);
+          dout = make_float4(d0.x, d0.y, d1.x, d1.y);
+          if (act) {
+            *reinterpret_cast<float4 *>(dv.b + ix) = make_float4(b0.x, b0.y, b1.x, b1.y);
+            *reinterpret_cast<float4 *>(dv.d + ix) = dout;
+          }
+        };
+        init_pair(CvA, muA, epA, idx, actA, sA0, sA1, nA0, nA1, dA);
+        init_pair(CvB, muB, epB, idx + 64, actB, sB0, sB1, nB0, nB1, dB);
+        muA = nmuA; muB = nmuB; epA = nepA; epB = nepB;
+      }
+      float rloc = 0.f;
+      const float4 outA = divide_pair(nA0, nA1, dA, CvA, rloc);
+      if (actA) { *reinterpret_cast<float4 *>(xout + idx) = outA; rmax = fmaxf(rmax, rloc); }
+      rloc = 0.f;
+      const float4 outB = divide_pair(nB0, nB1, dB, CvB, rloc);
+      if (actB) { *reinterpret_cast<float4 *>(xout + idx + 64) = outB; rmax = fmaxf(rmax, rloc); }
+    }
+    idx += plane;
+  };
+
+  // z march; the register ring (planes k-1, k, k+1) rotates by renaming over three unrolled planes
+  for (int t = 1; t <= nk; t += 3) {
+    do_plane(t, rA[0], rB[0], rA[1], rB[1], rA[2], rB[2]);
+    if (t + 1 <= nk) do_plane(t + 1, rA[1], rB[1], rA[2], rB[2], rA[0], rB[0]);
+    if (t + 2 <= nk) do_plane(t + 2, rA[2], rB[2], rA[0], rB[0], rA[1], rB[1]);
+  }
+
+  if (MODE != MODE_RHO) {
+    // max-residual reduction: redux over the warp on the uint pattern (non-negative floats order like
+    // uints), one shared atomic per warp, one global atomic per CTA; the last CTA decides (Eq. 34).
+    unsigned *s_max = reinterpret_cast<unsigned *>(smem_raw + 96);
+    const unsigned w = __reduce_max_sync(0xffffffffu, __float_as_uint(rmax));
+    if (lane == 0) atomicMax(s_max, w);
+    __syncthreads();
+    if (tid == 0) {
+      atomicMax(&ctl->resid_bits[l], *s_max);
+      __threadfence();
+      const unsigned nb = gridDim.x * gridDim.y * gridDim.z;
+      const unsigned tk = atomicAdd(&ctl->ticket, 1u);
+      if (tk == nb - 1) {
+        ctl->ticket = 0u;
+        sweep_decide2(dv, l);
+      }
+    }
+  }
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------------
+// host side
+// ------------------------------------------------------------------------------------------------
+// Tensor maps of an interleaved complex fp32 field seen as floats [nz][ny][2 nx] with the three box
+// shapes of a stage.  Returns 0, or a negative CUresult / -1000 if the driver entry point is missing.
+int march_tma_build_maps(const Dev &dv, MarchMaps *mm) {
+  void *fn = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
+      qres != cudaDriverEntryPointSuccess)
+    return -1000;
+  EncodeTiledFn enc = (EncodeTiledFn)fn;
+  const cuuint64_t gdim[3] = {2ull * dv.nx, (cuuint64_t)dv.ny, (cuuint64_t)dv.nz};
+  const cuuint64_t gstr[2] = {8ull * dv.nx, 8ull * dv.nx * dv.ny};
+  const cuuint32_t es[3] = {1, 1, 1};
+  const cuuint32_t bw = (cuuint32_t)(2 * (dv.nx < TW ? dv.nx : TW)), bh = (cuuint32_t)(dv.ny < TH ? dv.ny : TH);
+  const cuuint32_t boxC[3] = {bw, bh, 1}, boxR[3] = {bw, 1, 1}, boxX[3] = {4, bh, 1};
+  auto mk = [&](CUtensorMap *m, void *base, const cuuint32_t *box) -> int {
+    const CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, base, gdim, gstr, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                           CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? 0 : -(int)r;
+  };
+  int rc = 0;
+  for (int s = 0; s < 2 && !rc; ++s) {
+    if (!rc) rc = mk(&mm->psiC[s], dv.psi[s], boxC);
+    if (!rc) rc = mk(&mm->psiR[s], dv.psi[s], boxR);
+    if (!rc) rc = mk(&mm->psiX[s], dv.psi[s], boxX);
+  }
+  if (!rc) rc = mk(&mm->bC, dv.b, boxC);
+  if (!rc) rc = mk(&mm->dC, dv.d, boxC);
+  return rc;
+}
+
+cudaError_t march_tma_configure() {
+  cudaError_t e = cudaFuncSetAttribute(k_march_tma<MODE_SWEEP>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       (int)Cfg<MODE_SWEEP>::SMEM);
+  if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(k_march_tma<MODE_INIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg<MODE_INIT>::SMEM);
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(k_march_tma<MODE_RHO>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg<MODE_RHO>::SMEM);
+}
+
+void march_tma_grid(int nx, int ny, int *gx, int *gy) {
+  *gx = (nx + TW - 1) / TW;
+  *gy = (ny + TH - 1) / TH;
+}
+
+void launch_march_tma(int mode, const Dev &dv, const MarchMaps &mm, dim3 grid, cudaStream_t st) {
+  if (mode == MODE_SWEEP) k_march_tma<MODE_SWEEP><<<grid, NTHREADS, Cfg<MODE_SWEEP>::SMEM, st>>>(dv, mm);
+  else if (mode == MODE_INIT) k_march_tma<MODE_INIT><<<grid, NTHREADS, Cfg<MODE_INIT>::SMEM, st>>>(dv, mm);
+  else k_march_tma<MODE_RHO><<<grid, NTHREADS, Cfg<MODE_RHO>::SMEM, st>>>(dv, mm);
+}

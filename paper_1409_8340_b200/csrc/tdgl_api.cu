@@ -2,7 +2,9 @@
 // sequence (host loop or CUDA graph with a WHILE node around the Jacobi sweep), read-back.
 #include "../../include/tdgl.h"
 #include "tdgl_dev.cuh"
+#include "march_tma.h"
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -41,6 +43,8 @@ struct tdgl {
   cudaStream_t stream;
   dim3 mgrid, mblock;
   size_t msmem;
+  bool legacy_march;           // TDGL_MARCH_LEGACY=1: the cp.async kernel of stencil.cu (A/B comparisons only)
+  MarchMaps maps;
   int jav_blocks;
   int last_cuda;
   int64_t launches;            // host-counted kernel launches (graph launches are counted from the log)
@@ -123,6 +127,11 @@ extern "C" uint64_t tdgl_workspace_bytes(const tdgl_params *p) {
   return (uint64_t)carve(p, nullptr, nullptr);
 }
 
+static void march(tdgl_t *h, int mode, const Dev &dv, cudaStream_t st) {
+  if (h->legacy_march) launch_march(mode, dv, h->mgrid, h->mblock, h->msmem, st);
+  else launch_march_tma(mode, dv, h->maps, h->mgrid, st);
+}
+
 // the kernels of one step after the psi solve: J_av + K (a5), rho (a6), mu (a7)
 static int enqueue_after_solve(tdgl_t *h, cudaStream_t st) {
   int n = 0;
@@ -130,7 +139,7 @@ static int enqueue_after_solve(tdgl_t *h, cudaStream_t st) {
   if (kact) { launch_jav(h->dv, h->jav_blocks, st); ++n; }
   launch_step_finish(h->dv, h->jav_blocks, st); ++n;
   if (h->dv.solve_mu) {
-    launch_march(MODE_RHO, h->dv, h->mgrid, h->mblock, h->msmem, st); ++n;
+    march(h, MODE_RHO, h->dv, st); ++n;
     n += poisson_solve(h->dv, h->dv.mu, true, st);
   }
   return n;
@@ -147,7 +156,7 @@ static int build_graph(tdgl_t *h) {
   // segment A: begin + fused init/first sweep
   CK(cudaStreamBeginCaptureToGraph(cs, h->graph, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal));
   launch_step_begin(h->dv, cs);
-  launch_march(MODE_INIT, h->dv, h->mgrid, h->mblock, h->msmem, cs);
+  march(h, MODE_INIT, h->dv, cs);
   cudaStreamCaptureStatus status;
   const cudaGraphNode_t *deps = nullptr;
   size_t ndeps = 0;
@@ -165,7 +174,7 @@ static int build_graph(tdgl_t *h) {
   CK(cudaGraphAddNode(&cond, h->graph, tail.data(), tail.size(), &np));
   cudaGraph_t body = np.conditional.phGraph_out[0];
   CK(cudaStreamBeginCaptureToGraph(cs, body, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal));
-  launch_march(MODE_SWEEP, h->dv, h->mgrid, h->mblock, h->msmem, cs);
+  march(h, MODE_SWEEP, h->dv, cs);
   CK(cudaStreamEndCapture(cs, &g2));
   // segment B: everything after the psi solve
   CK(cudaStreamBeginCaptureToGraph(cs, h->graph, &cond, nullptr, 1, cudaStreamCaptureModeThreadLocal));
@@ -209,25 +218,43 @@ extern "C" int tdgl_create(const tdgl_params *p, tdgl_t **out) {
   dv.seed_hi = (unsigned)(p->seed >> 32);
   dv.solve_mu = (p->flags & TDGL_FLAG_SOLVE_MU) ? 1 : 0;
 
-  // launch geometry of the marching kernels: 512 threads, bx thread columns of two sites, by rows
-  int bx = 64;
-  while (bx > 16 && bx * 2 > p->nx) bx >>= 1;
-  int by = 512 / bx;
-  h->mblock = dim3(bx, by, 1);
-  const unsigned gx = (p->nx + 2 * bx - 1) / (2 * bx), gy = (p->ny + by - 1) / by;
+  // launch geometry of the marching kernels
+  {
+    const char *lg = std::getenv("TDGL_MARCH_LEGACY");
+    h->legacy_march = lg && lg[0] == '1';
+  }
+  unsigned gx, gy;
+  if (h->legacy_march) {       // 512 threads, bx thread columns of two sites, by rows
+    int bx = 64;
+    while (bx > 16 && bx * 2 > p->nx) bx >>= 1;
+    int by = 512 / bx;
+    h->mblock = dim3(bx, by, 1);
+    gx = (p->nx + 2 * bx - 1) / (2 * bx); gy = (p->ny + by - 1) / by;
+    h->msmem = march_smem_bytes(h->mblock);
+  } else {                     // 128 x 8 tiles, one warp per row (march_tma.cu)
+    int a, b;
+    march_tma_grid(p->nx, p->ny, &a, &b);
+    gx = (unsigned)a; gy = (unsigned)b;
+    h->mblock = dim3(256, 1, 1);
+    h->msmem = 0;
+  }
   // z chunks: enough CTAs for ~4 waves of 2 CTAs/SM, chunks of at least 8 planes
   int zc = p->nz;
   const long long want = 148ll * 2 * 4;
   while (zc > 8 && (long long)gx * gy * ((p->nz + zc - 1) / zc) < want) zc = (zc + 1) / 2;
   dv.zc = zc;
   h->mgrid = dim3(gx, gy, (p->nz + zc - 1) / zc);
-  h->msmem = march_smem_bytes(h->mblock);
   {
     long long nb = (dv.N / 2 + 255) / 256;
     h->jav_blocks = (int)(nb < 1 ? 1 : (nb > TDGL_NPART ? TDGL_NPART : nb));
   }
   h->pred_sweeps = 1;
-  CK(march_configure(h->mblock, h->msmem));
+  if (h->legacy_march) {
+    CK(march_configure(h->mblock, h->msmem));
+  } else {
+    CK(march_tma_configure());
+    if (march_tma_build_maps(dv, &h->maps) != 0) { h->last_cuda = (int)cudaErrorNotSupported; delete h; return TDGL_ECUDA; }
+  }
   CK(poisson_configure(p->nx, p->ny, p->nz));
   CK(cudaMallocHost((void **)&h->h_flag, 64));
   CK(cudaEventCreate(&h->ev0));
@@ -316,7 +343,7 @@ static int step_host_loop(tdgl_t *h) {
   cudaStream_t st = h->stream;
   const Dev &dv = h->dv;
   launch_step_begin(dv, st);
-  launch_march(MODE_INIT, dv, h->mgrid, h->mblock, h->msmem, st);
+  march(h, MODE_INIT, dv, st);
   h->launches += 2;
   int launched = 1;
   const int cap = TDGL_MAX_RESID_SLOTS;
@@ -324,14 +351,14 @@ static int step_host_loop(tdgl_t *h) {
     // speculative sweeps (they return at once when the solve is already done), then one flag read
     int burst = h->timing ? 0 : h->pred_sweeps - launched;
     for (int s = 0; s < burst && launched < cap; ++s) {
-      launch_march(MODE_SWEEP, dv, h->mgrid, h->mblock, h->msmem, st);
+      march(h, MODE_SWEEP, dv, st);
       ++launched; ++h->launches;
     }
     CK(cudaMemcpyAsync(h->h_flag, &dv.ctl->sweeps, 2 * sizeof(int), cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
     if (h->h_flag[1] || launched >= cap) break;
     if (h->timing) CK(cudaEventRecord(h->ev0, st));
-    launch_march(MODE_SWEEP, dv, h->mgrid, h->mblock, h->msmem, st);
+    march(h, MODE_SWEEP, dv, st);
     ++launched; ++h->launches;
     if (h->timing) {
       CK(cudaEventRecord(h->ev1, st));
@@ -489,7 +516,7 @@ extern "C" int tdgl_debug_rho(tdgl_t *h, void *rho_dev) {
   if (!h || !rho_dev) return TDGL_EINVAL;
   Dev d2 = h->dv;
   d2.mu = (float *)rho_dev;                       // the rho kernel writes where mu lives
-  launch_march(MODE_RHO, d2, h->mgrid, h->mblock, h->msmem, h->stream);
+  march(h, MODE_RHO, d2, h->stream);
   h->launches += 1;
   CKL();
   return TDGL_OK;
