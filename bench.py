@@ -268,7 +268,7 @@ def main():
             avg_ms = t_ms / n_l
             ach = SWEEP_BYTES_PER_SITE * N / (avg_ms * 1e-3) / 1e9
             tr = ncu_traffic()
-            roof = {"bound": "hbm", "kernel": "k_march<SWEEP> (Jacobi sweep + max-residual)", "achieved": ach,
+            roof = {"bound": "hbm", "kernel": "k_march_tma<SWEEP> (Jacobi sweep + max-residual)", "achieved": ach,
                     "peak": peak, "unit": "GB/s", "frac": ach / peak, "peak_source": how,
                     "avg_launch_ms": avg_ms, "launches_timed": int(n_l),
                     "algorithmic_bytes_per_launch": SWEEP_BYTES_PER_SITE * N,

@@ -4,15 +4,11 @@
 #include "tdgl_dev.cuh"
 #include "march_tma.h"
 #include <cmath>
-#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
 
 // launchers defined in the kernel files
-void launch_march(int mode, const Dev &dv, dim3 grid, dim3 block, size_t smem, cudaStream_t st);
-size_t march_smem_bytes(dim3 block);
-cudaError_t march_configure(dim3 block, size_t smem);
 void launch_jav(const Dev &dv, int nblocks, cudaStream_t st);
 void launch_step_begin(const Dev &dv, cudaStream_t st);
 void launch_step_finish(const Dev &dv, int npart, cudaStream_t st);
@@ -41,10 +37,8 @@ struct tdgl {
   tdgl_params p;
   Dev dv;
   cudaStream_t stream;
-  dim3 mgrid, mblock;
-  size_t msmem;
-  bool legacy_march;           // TDGL_MARCH_LEGACY=1: the cp.async kernel of stencil.cu (A/B comparisons only)
-  MarchMaps maps;
+  dim3 mgrid;                  // grid of the marching kernels: 128 x 8 tiles x z chunks
+  MarchMaps maps;              // TMA tensor maps of psi[0], psi[1], b, d
   int jav_blocks;
   int last_cuda;
   int64_t launches;            // host-counted kernel launches (graph launches are counted from the log)
@@ -128,8 +122,7 @@ extern "C" uint64_t tdgl_workspace_bytes(const tdgl_params *p) {
 }
 
 static void march(tdgl_t *h, int mode, const Dev &dv, cudaStream_t st) {
-  if (h->legacy_march) launch_march(mode, dv, h->mgrid, h->mblock, h->msmem, st);
-  else launch_march_tma(mode, dv, h->maps, h->mgrid, st);
+  launch_march_tma(mode, dv, h->maps, h->mgrid, st);
 }
 
 // the kernels of one step after the psi solve: J_av + K (a5), rho (a6), mu (a7)
@@ -218,25 +211,12 @@ extern "C" int tdgl_create(const tdgl_params *p, tdgl_t **out) {
   dv.seed_hi = (unsigned)(p->seed >> 32);
   dv.solve_mu = (p->flags & TDGL_FLAG_SOLVE_MU) ? 1 : 0;
 
-  // launch geometry of the marching kernels
-  {
-    const char *lg = std::getenv("TDGL_MARCH_LEGACY");
-    h->legacy_march = lg && lg[0] == '1';
-  }
+  // launch geometry of the marching kernels: 128 x 8 tiles, one warp per row (march_tma.cu)
   unsigned gx, gy;
-  if (h->legacy_march) {       // 512 threads, bx thread columns of two sites, by rows
-    int bx = 64;
-    while (bx > 16 && bx * 2 > p->nx) bx >>= 1;
-    int by = 512 / bx;
-    h->mblock = dim3(bx, by, 1);
-    gx = (p->nx + 2 * bx - 1) / (2 * bx); gy = (p->ny + by - 1) / by;
-    h->msmem = march_smem_bytes(h->mblock);
-  } else {                     // 128 x 8 tiles, one warp per row (march_tma.cu)
+  {
     int a, b;
     march_tma_grid(p->nx, p->ny, &a, &b);
     gx = (unsigned)a; gy = (unsigned)b;
-    h->mblock = dim3(256, 1, 1);
-    h->msmem = 0;
   }
   // z chunks: enough CTAs for ~4 waves of 2 CTAs/SM, chunks of at least 8 planes
   int zc = p->nz;
@@ -249,12 +229,8 @@ extern "C" int tdgl_create(const tdgl_params *p, tdgl_t **out) {
     h->jav_blocks = (int)(nb < 1 ? 1 : (nb > TDGL_NPART ? TDGL_NPART : nb));
   }
   h->pred_sweeps = 1;
-  if (h->legacy_march) {
-    CK(march_configure(h->mblock, h->msmem));
-  } else {
-    CK(march_tma_configure());
-    if (march_tma_build_maps(dv, &h->maps) != 0) { h->last_cuda = (int)cudaErrorNotSupported; delete h; return TDGL_ECUDA; }
-  }
+  CK(march_tma_configure());
+  if (march_tma_build_maps(dv, &h->maps) != 0) { h->last_cuda = (int)cudaErrorNotSupported; delete h; return TDGL_ECUDA; }
   CK(poisson_configure(p->nx, p->ny, p->nz));
   CK(cudaMallocHost((void **)&h->h_flag, 64));
   CK(cudaEventCreate(&h->ev0));
