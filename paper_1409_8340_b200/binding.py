@@ -8,7 +8,7 @@ from typing import Optional, Sequence
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_LIB_PATH = os.path.join(_HERE, "libtdgl.so")
+_LIB_PATH = os.environ.get("TDGL_LIB") or os.path.join(_HERE, "libtdgl.so")     # TDGL_LIB: another build of the same ABI
 
 TDGL_OK, TDGL_EINVAL, TDGL_ENOMEM, TDGL_EINCOMPAT, TDGL_ECUDA, TDGL_WMAXSWEEPS = 0, -1, -2, -3, -4, 1
 TDGL_BC_PERIODIC, TDGL_BC_OPEN = 0, 1

@@ -37,7 +37,7 @@ constexpr unsigned OFF_XE = 10368;      // ghost column pair (i0+nv, i0+nv+1)
 constexpr unsigned OFF_B = 10496;       // b tile (sweep only)
 constexpr unsigned OFF_D = 18688;       // d tile (sweep only)
 constexpr unsigned STAGE_PSI = 10496, STAGE_SWEEP = 26880;
-constexpr unsigned HDR = 128;           // mbarriers (8 B each) + the CTA residual word at byte 96
+constexpr unsigned HDR = 256;           // mbarriers (8 B each) at 0, the CTA residual word at 64, 8 J_av warp sums at 128
 
 template <int MODE> struct Cfg {
   static constexpr int NS = (MODE == MODE_SWEEP) ? 4 : 6;                       // stages in the ring
@@ -216,7 +216,7 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_march_tma(const __grid_constant
   if (tid == 0) {
     for (int s = 0; s < NS; ++s) mbar_init(sbase + 8u * s, 1u);
     asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
-    *reinterpret_cast<unsigned *>(smem_raw + 96) = 0u;              // CTA max-residual word
+    *reinterpret_cast<unsigned *>(smem_raw + 64) = 0u;              // CTA max-residual word
   }
   __syncthreads();
   if (tid == 0)
@@ -257,6 +257,13 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_march_tma(const __grid_constant
   unsigned nstep = 0;
   if (MODE == MODE_INIT) nstep = (unsigned)ctl->n;
   float rmax = 0.f;
+  // J_av (Eq. 35): x links of the NEW iterate that lie inside this tile row (stencil.cu, k_jav_edges
+  // adds the links that cross a tile edge); only with x periodic and the mu / K part active
+  const bool jact = (MODE != MODE_RHO) && dv.solve_mu && px;
+  const float2 Uraw = dv.Ux[jc];
+  const bool lkA0 = actA, lkA1 = actA && 2 * lane + 2 < nv;
+  const bool lkB0 = actB, lkB1 = actB && 64 + 2 * lane + 2 < nv && lane < 31;
+  double jacc = 0.0;
 
   // element index of pair A in plane k0 (float2 units); clamped so that inactive threads stay in range
   const long long rowoff = (long long)jc * nx + min(iA, nx - 2);
@@ -409,6 +416,22 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_march_tma(const __grid_constant
       rloc = 0.f;
       const float4 outB = divide_pair(nB0, nB1, dB, CvB, rloc);
       if (actB) { *reinterpret_cast<float4 *>(xout + idx + 64) = outB; rmax = fmaxf(rmax, rloc); }
+      if (jact) {
+        // Im[x*_m U x_{m+1}] on the links (2l,2l+1), (2l+1,2l+2), (64+2l,65+2l), (65+2l,66+2l); the east
+        // end of the second comes from lane l+1, for lane 31 it is site 64 = lane 0's second pair
+        const float nAx = __shfl_down_sync(0xffffffffu, outA.x, 1), nAy = __shfl_down_sync(0xffffffffu, outA.y, 1);
+        const float rBx = __shfl_sync(0xffffffffu, outB.x, (lane + 1) & 31), rBy = __shfl_sync(0xffffffffu, outB.y, (lane + 1) & 31);
+        const float2 nxA = (lane == 31) ? make_float2(rBx, rBy) : make_float2(nAx, nAy);
+        auto link = [&](float ar, float ai, float br, float bi) {
+          return ar * (Uraw.x * bi + Uraw.y * br) - ai * (Uraw.x * br - Uraw.y * bi);
+        };
+        float tsum = 0.f;
+        if (lkA0) tsum += link(outA.x, outA.y, outA.z, outA.w);
+        if (lkA1) tsum += link(outA.z, outA.w, nxA.x, nxA.y);
+        if (lkB0) tsum += link(outB.x, outB.y, outB.z, outB.w);
+        if (lkB1) tsum += link(outB.z, outB.w, rBx, rBy);
+        jacc += (double)tsum;
+      }
     }
     idx += plane;
   };
@@ -423,11 +446,21 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_march_tma(const __grid_constant
   if (MODE != MODE_RHO) {
     // max-residual reduction: redux over the warp on the uint pattern (non-negative floats order like
     // uints), one shared atomic per warp, one global atomic per CTA; the last CTA decides (Eq. 34).
-    unsigned *s_max = reinterpret_cast<unsigned *>(smem_raw + 96);
+    unsigned *s_max = reinterpret_cast<unsigned *>(smem_raw + 64);
+    double *s_j = reinterpret_cast<double *>(smem_raw + 128);
     const unsigned w = __reduce_max_sync(0xffffffffu, __float_as_uint(rmax));
     if (lane == 0) atomicMax(s_max, w);
+    if (jact) {
+      for (int o = 16; o > 0; o >>= 1) jacc += __shfl_down_sync(0xffffffffu, jacc, o);
+      if (lane == 0) s_j[row] = jacc;
+    }
     __syncthreads();
     if (tid == 0) {
+      if (jact) {                                        // fixed order => bit-reproducible
+        double sj = 0.0;
+        for (int q = 0; q < TH; ++q) sj += s_j[q];
+        dv.jpart[blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z)] = sj;
+      }
       atomicMax(&ctl->resid_bits[l], *s_max);
       __threadfence();
       const unsigned nb = gridDim.x * gridDim.y * gridDim.z;
@@ -488,6 +521,8 @@ cudaError_t march_tma_configure() {
   if (e != cudaSuccess) return e;
   return cudaFuncSetAttribute(k_march_tma<MODE_RHO>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg<MODE_RHO>::SMEM);
 }
+
+int march_tma_tile_w() { return TW; }
 
 void march_tma_grid(int nx, int ny, int *gx, int *gy) {
   *gx = (nx + TW - 1) / TW;

@@ -14,4 +14,5 @@ struct MarchMaps {
 int march_tma_build_maps(const Dev &dv, MarchMaps *mm);
 cudaError_t march_tma_configure();
 void march_tma_grid(int nx, int ny, int *gx, int *gy);
+int march_tma_tile_w();
 void launch_march_tma(int mode, const Dev &dv, const MarchMaps &mm, dim3 grid, cudaStream_t st);

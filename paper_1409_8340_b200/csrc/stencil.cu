@@ -4,28 +4,26 @@
 
 // ------------------------------------------------------------------------------------------------
 // a5: J_av = 1/(2 N h_x) sum_m Im[psi*_m (U_x psi_{i+1} - U_x* psi_{i-1})]   (Eq. 35)
-// Stage 1: fp64 partial sum per CTA (fixed grid => fixed summation order).
-__global__ void __launch_bounds__(256) k_jav_partial(const __grid_constant__ Dev dv) {
+// With x periodic the backward term of site m equals the forward term of site m-1, so
+//   J_av = 1/(N h_x) sum over x links of Im[psi*_m U_x(j) psi_{m+x}].
+// The links inside a 128-site tile row are summed by the marching kernel itself on the iterate it has
+// just computed (one fp64 partial per CTA, dv.jpart).  This kernel adds the links that leave the last
+// site of every tile row (wrapping to i = 0): one thread per (row, tile), fp64 partial per CTA, fixed
+// grid => fixed summation order.
+__global__ void __launch_bounds__(256) k_jav_edges(const __grid_constant__ Dev dv, int tile_w) {
   const float2 *__restrict__ x = dv.psi[dv.ctl->xbuf];
-  const int hx2 = dv.nx >> 1;
-  const long long npair = dv.N >> 1;
+  const int ntx = (dv.nx + tile_w - 1) / tile_w;
+  const long long nrows = (long long)dv.ny * dv.nz, total = nrows * ntx;
   double acc = 0.0;
-  for (long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x; p < npair;
-       p += (long long)gridDim.x * blockDim.x) {
-    const long long row = p / hx2;
-    const int i = 2 * (int)(p - row * hx2);
+  for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < total; q += (long long)gridDim.x * blockDim.x) {
+    const long long row = q / ntx;
+    const int t = (int)(q - row * ntx);
+    const int e = min(dv.nx, (t + 1) * tile_w) - 1;
     const int j = (int)(row % dv.ny);
     const float2 *xr = x + row * dv.nx;
-    const float4 C = *reinterpret_cast<const float4 *>(xr + i);
-    const float2 W = xr[i == 0 ? dv.nx - 1 : i - 1];
-    const float2 E = xr[i + 2 >= dv.nx ? 0 : i + 2];
-    const float2 U = dv.Ux[j];
-    const float2 c0 = make_float2(C.x, C.y), c1 = make_float2(C.z, C.w);
-    // site i: E = c1, W = W; site i+1: E = E, W = c0
-    const float2 up0 = cmul(U, c1), um0 = cmulc(U, W), up1 = cmul(U, E), um1 = cmulc(U, c0);
-    const float t0 = c0.x * (up0.y - um0.y) - c0.y * (up0.x - um0.x);
-    const float t1 = c1.x * (up1.y - um1.y) - c1.y * (up1.x - um1.x);
-    acc += (double)t0 + (double)t1;
+    const float2 a = xr[e], b = xr[e + 1 == dv.nx ? 0 : e + 1];
+    const float2 ub = cmul(dv.Ux[j], b);
+    acc += (double)(a.x * ub.y - a.y * ub.x);
   }
   __shared__ double sh[8];
   for (int o = 16; o > 0; o >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, o);
@@ -64,7 +62,7 @@ __global__ void k_step_begin(const __grid_constant__ Dev dv) {
 
 // After the psi solve: finish the J_av sum, E_x = J_ext - J_av (Eq. 21 with d_t A = 0, Eq. 15), forward
 // Euler for K (S3) and rewinding; refresh U_x(j) with the new K for rho (S4); log the step.
-__global__ void k_step_finish(const __grid_constant__ Dev dv, int npart) {
+__global__ void k_step_finish(const __grid_constant__ Dev dv, int ncta, int nedge) {
   Ctl *c = dv.ctl;
   __shared__ double sh[256];
   __shared__ double Knew;
@@ -72,7 +70,8 @@ __global__ void k_step_finish(const __grid_constant__ Dev dv, int npart) {
   const bool kact = dv.solve_mu && dv.bcx == 0;
   if (kact) {
     double s = 0.0;
-    for (int p = tid; p < npart; p += 256) s += dv.part[p];
+    for (int p = tid; p < ncta; p += 256) s += dv.jpart[p];       // in-tile links (marching kernel)
+    for (int p = tid; p < nedge; p += 256) s += dv.part[p];      // tile-crossing links (k_jav_edges)
     sh[tid] = s;
     __syncthreads();
     for (int o = 128; o > 0; o >>= 1) {
@@ -83,7 +82,7 @@ __global__ void k_step_finish(const __grid_constant__ Dev dv, int npart) {
   if (tid == 0) {
     double K = c->K, Ex = 0.0, Jav = 0.0;
     if (kact) {
-      Jav = sh[0] / (2.0 * (double)dv.N * dv.hx);
+      Jav = sh[0] / ((double)dv.N * dv.hx);
       Ex = c->Jext - Jav;
       K = K + dv.dt * Ex;
       const double q = 6.283185307179586476925286766559 / dv.hx;
@@ -105,6 +104,11 @@ __global__ void k_step_finish(const __grid_constant__ Dev dv, int npart) {
 
 // ------------------------------------------------------------------------------------------------
 // host-side launchers (called from tdgl_api.cu)
-void launch_jav(const Dev &dv, int nblocks, cudaStream_t st) { k_jav_partial<<<nblocks, 256, 0, st>>>(dv); }
+int jav_edge_blocks(const Dev &dv, int tile_w) {
+  const long long total = (long long)dv.ny * dv.nz * ((dv.nx + tile_w - 1) / tile_w);
+  const long long nb = (total + 255) / 256;
+  return (int)(nb < 1 ? 1 : (nb > TDGL_NPART ? TDGL_NPART : nb));
+}
+void launch_jav_edges(const Dev &dv, int tile_w, int nblocks, cudaStream_t st) { k_jav_edges<<<nblocks, 256, 0, st>>>(dv, tile_w); }
 void launch_step_begin(const Dev &dv, cudaStream_t st) { k_step_begin<<<1, 256, 0, st>>>(dv); }
-void launch_step_finish(const Dev &dv, int npart, cudaStream_t st) { k_step_finish<<<1, 256, 0, st>>>(dv, npart); }
+void launch_step_finish(const Dev &dv, int ncta, int nedge, cudaStream_t st) { k_step_finish<<<1, 256, 0, st>>>(dv, ncta, nedge); }

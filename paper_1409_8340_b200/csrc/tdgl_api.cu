@@ -9,9 +9,10 @@
 #include <vector>
 
 // launchers defined in the kernel files
-void launch_jav(const Dev &dv, int nblocks, cudaStream_t st);
+int jav_edge_blocks(const Dev &dv, int tile_w);
+void launch_jav_edges(const Dev &dv, int tile_w, int nblocks, cudaStream_t st);
 void launch_step_begin(const Dev &dv, cudaStream_t st);
-void launch_step_finish(const Dev &dv, int npart, cudaStream_t st);
+void launch_step_finish(const Dev &dv, int ncta, int nedge, cudaStream_t st);
 cudaError_t poisson_configure(int nx, int ny, int nz);
 void launch_build_tables(float *lam, float2 *tw, double *tab, int n, int open, double c, cudaStream_t st);
 int poisson_solve(const Dev &dv, float *data, bool thomas_open_z, cudaStream_t st);
@@ -62,6 +63,17 @@ struct tdgl {
 
 static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
+// launch geometry of the marching kernels (march_tma.cu): 128 x 8 tiles, one warp per row; z chunks chosen
+// so that there are enough CTAs for ~4 waves of 2 CTAs/SM, chunks of at least 8 planes
+static void march_geometry(const tdgl_params *p, unsigned *gx, unsigned *gy, unsigned *gz, int *zc_out) {
+  int a, b;
+  march_tma_grid(p->nx, p->ny, &a, &b);
+  int zc = p->nz;
+  const long long want = 148ll * 2 * 4;
+  while (zc > 8 && (long long)a * b * ((p->nz + zc - 1) / zc) < want) zc = (zc + 1) / 2;
+  *gx = (unsigned)a; *gy = (unsigned)b; *gz = (unsigned)((p->nz + zc - 1) / zc); *zc_out = zc;
+}
+
 static bool params_ok(const tdgl_params *p) {
   if (!p || p->struct_size != sizeof(tdgl_params)) return false;
   if (p->nx < 2 || p->ny < 2 || p->nz < 2 || (p->nx & 1)) return false;
@@ -96,6 +108,11 @@ static size_t carve(const tdgl_params *p, char *base, Dev *dv) {
     q = take(4096 * sizeof(float2)); if (dv) dv->bH[a] = (float2 *)q;
   }
   q = take((size_t)TDGL_NPART * 4 * sizeof(double)); if (dv) dv->part = (double *)q;
+  {
+    unsigned gx, gy, gz; int zc;
+    march_geometry(p, &gx, &gy, &gz, &zc);
+    q = take((size_t)gx * gy * gz * sizeof(double)); if (dv) dv->jpart = (double *)q;
+  }
   q = take(TDGL_LOGCAP * sizeof(int)); if (dv) dv->sweep_log = (int *)q;
   q = take(TDGL_LOGCAP * sizeof(float)); if (dv) dv->resid_log = (float *)q;
   q = take(TDGL_LOGCAP * sizeof(int)); if (dv) dv->sched = (int *)q;
@@ -129,8 +146,10 @@ static void march(tdgl_t *h, int mode, const Dev &dv, cudaStream_t st) {
 static int enqueue_after_solve(tdgl_t *h, cudaStream_t st) {
   int n = 0;
   const bool kact = h->dv.solve_mu && h->dv.bcx == 0;
-  if (kact) { launch_jav(h->dv, h->jav_blocks, st); ++n; }
-  launch_step_finish(h->dv, h->jav_blocks, st); ++n;
+  // J_av: the in-tile x links were summed by the last sweep (one partial per CTA); the links that cross a
+  // tile edge are summed here
+  if (kact) { launch_jav_edges(h->dv, march_tma_tile_w(), h->jav_blocks, st); ++n; }
+  launch_step_finish(h->dv, (int)(h->mgrid.x * h->mgrid.y * h->mgrid.z), h->jav_blocks, st); ++n;
   if (h->dv.solve_mu) {
     march(h, MODE_RHO, h->dv, st); ++n;
     n += poisson_solve(h->dv, h->dv.mu, true, st);
@@ -211,23 +230,13 @@ extern "C" int tdgl_create(const tdgl_params *p, tdgl_t **out) {
   dv.seed_hi = (unsigned)(p->seed >> 32);
   dv.solve_mu = (p->flags & TDGL_FLAG_SOLVE_MU) ? 1 : 0;
 
-  // launch geometry of the marching kernels: 128 x 8 tiles, one warp per row (march_tma.cu)
-  unsigned gx, gy;
   {
-    int a, b;
-    march_tma_grid(p->nx, p->ny, &a, &b);
-    gx = (unsigned)a; gy = (unsigned)b;
+    unsigned gx, gy, gz; int zc;
+    march_geometry(p, &gx, &gy, &gz, &zc);
+    dv.zc = zc;
+    h->mgrid = dim3(gx, gy, gz);
   }
-  // z chunks: enough CTAs for ~4 waves of 2 CTAs/SM, chunks of at least 8 planes
-  int zc = p->nz;
-  const long long want = 148ll * 2 * 4;
-  while (zc > 8 && (long long)gx * gy * ((p->nz + zc - 1) / zc) < want) zc = (zc + 1) / 2;
-  dv.zc = zc;
-  h->mgrid = dim3(gx, gy, (p->nz + zc - 1) / zc);
-  {
-    long long nb = (dv.N / 2 + 255) / 256;
-    h->jav_blocks = (int)(nb < 1 ? 1 : (nb > TDGL_NPART ? TDGL_NPART : nb));
-  }
+  h->jav_blocks = jav_edge_blocks(dv, march_tma_tile_w());
   h->pred_sweeps = 1;
   CK(march_tma_configure());
   if (march_tma_build_maps(dv, &h->maps) != 0) { h->last_cuda = (int)cudaErrorNotSupported; delete h; return TDGL_ECUDA; }

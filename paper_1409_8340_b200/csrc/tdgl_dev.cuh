@@ -61,6 +61,7 @@ struct Dev {
   float2 *bT[3], *bC[3], *bH[3];   // Bluestein tables of the fast DCT-I per open axis (dct.cu)
   int bLB[3];               // its FFT length, 0 = axis not open / not supported
   double *part;             // TDGL_NPART*4 partial sums
+  double *jpart;            // one J_av partial sum per CTA of the marching kernels (in-tile x links of the new iterate)
   int *sweep_log; float *resid_log; int *sched;
   unsigned long long cond_handle;   // cudaGraphConditionalHandle of the WHILE node (graph mode)
   int use_cond;
