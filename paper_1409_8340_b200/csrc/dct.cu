@@ -66,7 +66,7 @@ k_dct_x(float *__restrict__ data, int n, long long nrows, const float2 *__restri
   float2 *tw = reinterpret_cast<float2 *>(smem4);
   float2 *sm = tw + LB;
   const int tid = threadIdx.x;
-  for (int m = tid; m < LB; m += NT) tw[m] = twg[m];
+  fill_twiddles<LB>(tw, twg, tid, NT);
   const int j = tid % TPF, f = tid / TPF;
   const int M = 2 * (n - 1);
   const long long ra = 2 * ((long long)blockIdx.x * F + f), rb = ra + 1;
@@ -107,7 +107,7 @@ k_dct_s(float *__restrict__ data, int n, long long stride, long long ostride, in
   float2 *tw = reinterpret_cast<float2 *>(smem4);
   float2 *sm = tw + LB;
   const int tid = threadIdx.x;
-  for (int m = tid; m < LB; m += NT) tw[m] = twg[m];
+  fill_twiddles<LB>(tw, twg, tid, NT);
   const int f = tid % CC, j = tid / CC;
   const int col = blockIdx.x * CC + f;
   const bool valid = col < ncolc;

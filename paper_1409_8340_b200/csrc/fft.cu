@@ -19,7 +19,7 @@ __global__ void __launch_bounds__(256) k_dht_x_fast(float *__restrict__ data, lo
   float2 *tw = reinterpret_cast<float2 *>(smem4);
   float2 *sm = tw + N;
   const int tid = threadIdx.x;
-  for (int m = tid; m < N; m += 256) tw[m] = twg[m];
+  fill_twiddles<N>(tw, twg, tid, 256);
   const int j = tid % TPF, f = tid / TPF;
   const long long ra = 2 * ((long long)blockIdx.x * F + f), rb = ra + 1;
   const bool va = ra < nrows, vb = rb < nrows;
@@ -55,7 +55,7 @@ __global__ void __launch_bounds__(CC *N / 8) k_dht_s_fast(float *__restrict__ da
   float2 *tw = reinterpret_cast<float2 *>(smem4);
   float2 *sm = tw + N;
   const int tid = threadIdx.x;
-  for (int m = tid; m < N; m += NT) tw[m] = twg[m];
+  fill_twiddles<N>(tw, twg, tid, NT);
   const int f = tid % CC, j = tid / CC;
   const int col = blockIdx.x * CC + f;
   const long long o = blockIdx.y;

@@ -44,6 +44,23 @@ template <int N, bool XPASS, int CC> __device__ __forceinline__ int saddr(int f,
   return XPASS ? f * (N + N / 8) + p + (p >> 3) : p * CC + f;
 }
 
+// Twiddles in shared memory, one compact table per (stage, r):  ct[tw_off(NS) + (r-1) NS + k] = exp(-2 pi i r k/(NS R)),
+// k < NS.  Lanes with consecutive k read consecutive addresses (the plain table tw[r k N/(NS R)] put the even
+// multiples of a stage into a few banks: ncu showed half of all shared wavefronts of the x pass were conflicts).
+// The values are the entries of the fp64-built global table exp(-2 pi i m/N), so results are unchanged.
+__host__ __device__ constexpr int tw_off(int NS) { return NS == 8 ? 0 : NS == 64 ? 56 : 504; }
+__host__ __device__ constexpr int radix_of(int N, int NS) { return (N / NS >= 8) ? 8 : N / NS; }
+template <int N> __device__ __forceinline__ void fill_twiddles(float2 *ct, const float2 *__restrict__ twg, int tid, int nth) {
+#pragma unroll
+  for (int NS = 8; NS < N; NS *= 8) {
+    const int R = radix_of(N, NS), step = N / (NS * R);
+    for (int e = tid; e < (R - 1) * NS; e += nth) {
+      const int r = 1 + e / NS, k = e % NS;
+      ct[tw_off(NS) + e] = twg[r * k * step];
+    }
+  }
+}
+
 // One Stockham stage of radix R with Ns = product of the earlier radices; the thread owns 8/R butterflies.
 // FIRST: inputs are already in v (read from global); otherwise they are read from shared memory.
 template <int N, int R, int NS, bool XPASS, int CC, bool FIRST>
@@ -64,7 +81,7 @@ __device__ __forceinline__ void stage(float2 *v, float2 *sm, const float2 *tw, i
     const int k = jj & (NS - 1);
     if (NS > 1) {
 #pragma unroll
-      for (int r = 1; r < R; ++r) v[t * R + r] = cmul(v[t * R + r], tw[r * k * (N / (NS * R))]);
+      for (int r = 1; r < R; ++r) v[t * R + r] = cmul(v[t * R + r], tw[tw_off(NS) + (r - 1) * NS + k]);
     }
     dft<R>(v + t * R);
     const int base = (jj - k) * R + k;
