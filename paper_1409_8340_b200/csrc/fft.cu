@@ -101,7 +101,7 @@ static size_t smem_s(int n, int cc) { return (size_t)(n + (size_t)n * cc) * size
 bool dht_fast_supported(int n) { return n == 64 || n == 128 || n == 256 || n == 512 || n == 1024; }
 
 template <int N> static cudaError_t cfg_n() {
-  constexpr int CC = (N == 1024) ? 8 : 16;
+  constexpr int CC = (N >= 512) ? 8 : 16;
   cudaError_t e = cudaFuncSetAttribute(k_dht_x_fast<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_x(N));
   if (e != cudaSuccess) return e;
   return cudaFuncSetAttribute(k_dht_s_fast<N, CC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_s(N, CC));
@@ -135,7 +135,7 @@ void launch_dht_x_fast(float *data, int n, long long nrows, const float2 *tw, cu
 template <int N>
 static void run_s(float *data, long long stride, long long ostride, int ncolc, int nother, const float2 *tw, int divide,
                   float scale, const float *lx, const float *ly, const float *lz, cudaStream_t st) {
-  constexpr int CC = (N == 1024) ? 8 : 16;
+  constexpr int CC = (N >= 512) ? 8 : 16;
   dim3 grid((ncolc + CC - 1) / CC, nother);
   k_dht_s_fast<N, CC><<<grid, CC * N / 8, smem_s(N, CC), st>>>(data, stride, ostride, ncolc, tw, divide, scale, lx, ly, lz);
 }
