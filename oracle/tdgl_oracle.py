@@ -141,14 +141,26 @@ def paper_links(p: Params, K: float, Bx: float, Bz: float):
         P_{i,k} = exp(i (i h_x L_y B_z - k h_z L_y B_x)),
     i.e. the wrap link that leaves row Ny-1 in +y carries exp(i th_y) = P*_{i,k}.
     """
-    ybar = (np.arange(p.ny) * p.hy - p.length("y") / 2.0)[None, :, None]
-    thx = np.broadcast_to(p.hx * (K + Bz * ybar), p.shape).copy()
-    thz = np.broadcast_to(-p.hz * Bx * ybar, p.shape).copy()
-    thy = np.zeros(p.shape)
+    return paper_links_at(p, K, Bx, Bz, np.arange(p.nx), np.arange(p.ny), np.arange(p.nz))
+
+
+def paper_links_at(p: Params, K: float, Bx: float, Bz: float, ii, jj, kk):
+    """The link phases of `paper_links` on the sub-lattice of global indices ii x jj x kk (1-D integer
+    arrays, x, y, z): arrays of shape (len(kk), len(jj), len(ii)).  `paper_links` is this function on the
+    full index ranges; the windowed form lets a test evaluate the same formulas on samples of a grid that
+    is too large for a whole oracle step."""
+    ii, jj, kk = (np.asarray(a, dtype=np.int64) for a in (ii, jj, kk))
+    shape = (len(kk), len(jj), len(ii))
+    ybar = (jj * p.hy - p.length("y") / 2.0)[None, :, None]
+    thx = np.broadcast_to(p.hx * (K + Bz * ybar), shape).copy()
+    thz = np.broadcast_to(-p.hz * Bx * ybar, shape).copy()
+    thy = np.zeros(shape)
     if p.bc[1] == PERIODIC:
-        i = np.arange(p.nx)[None, :]
-        k = np.arange(p.nz)[:, None]
-        thy[:, p.ny - 1, :] = -(i * p.hx * p.length("y") * Bz - k * p.hz * p.length("y") * Bx)
+        i = ii[None, :]
+        k = kk[:, None]
+        wrap = -(i * p.hx * p.length("y") * Bz - k * p.hz * p.length("y") * Bx)
+        for w in np.nonzero(jj == p.ny - 1)[0]:
+            thy[:, w, :] = wrap
     return thx, thy, thz
 
 
@@ -224,9 +236,15 @@ def zeta_max(p: Params) -> float:
 def langevin_noise(p: Params, step: int):
     """zeta_m = zeta_max (r1 + i r2), r uniform in (-1, 1), independent per site and step (P:353);
     Philox stream 0, counter (m, step) (S11)."""
-    x0, x1 = philox.site_words(p.n_sites, step, 0, p.seed)
-    z = philox.uniform_pm1(x0) + 1j * philox.uniform_pm1(x1)
-    return (zeta_max(p) * z).reshape(p.shape)
+    return langevin_noise_at(p, step, np.arange(p.n_sites, dtype=np.uint64)).reshape(p.shape)
+
+
+def langevin_noise_at(p: Params, step: int, m):
+    """The Langevin term of `langevin_noise` at the global site indices m = i + nx (j + ny k) (any shape)."""
+    m = np.asarray(m, dtype=np.uint64)
+    x0, x1, _, _ = philox.philox4x32_10(m & np.uint64(0xFFFFFFFF), m >> np.uint64(32), step, 0,
+                                        p.seed & 0xFFFFFFFF, (p.seed >> 32) & 0xFFFFFFFF)
+    return zeta_max(p) * (philox.uniform_pm1(x0) + 1j * philox.uniform_pm1(x1))
 
 
 def initial_state(p: Params, init_amp: float) -> State:

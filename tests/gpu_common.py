@@ -50,3 +50,54 @@ def setup_pair(cfg: I.Config, psi0=None, mu0=None, K0=0.0, with_pinning=True, **
 
 def rel_l2(a, b):
     return float(np.linalg.norm((a - b).ravel()) / max(np.linalg.norm(b.ravel()), 1e-300))
+
+
+# ---- sampled parity at sizes where a whole oracle step is out of reach ---------------------------------
+def window_indices(origin, size, n, periodic):
+    """Global indices of a window along one axis: origin may be negative / run past n on a periodic axis
+    (indices wrap); on an open axis the window is clipped to [0, n)."""
+    q = np.arange(origin, origin + size)
+    if periodic:
+        return np.mod(q, n)
+    return q[(q >= 0) & (q < n)]
+
+
+def oracle_window_solve(p, psi0, eps, Bx, Bz, K, step, sweeps, ii, jj, kk, mu=None):
+    """The oracle's psi solve (build_system + `sweeps` Jacobi sweeps, Eq. 31/33) on the window ii x jj x kk of a
+    large grid, from the window's own inputs only.  Jacobi information travels one site per sweep, so
+    the result is the full-grid result at every site farther than `sweeps` sites from an ARTIFICIAL
+    window edge; real open faces inside the window keep the oracle's open boundary rule.  `psi0`, `eps`
+    (and `mu`) are window arrays of shape (len(kk), len(jj), len(ii)).  Returns (x, valid mask)."""
+    n = (p.nx, p.ny, p.nz)
+    idx = (ii, jj, kk)
+    bcw, lo_real, hi_real = [], [], []
+    for a in range(3):
+        op = p.bc[a] == O.OPEN
+        lo_real.append(op and idx[a][0] == 0)
+        hi_real.append(op and idx[a][-1] == n[a] - 1)
+        bcw.append(O.OPEN if (lo_real[a] or hi_real[a]) else O.PERIODIC)
+    pw = O.Params(len(ii), len(jj), len(kk), hx=p.hx, hy=p.hy, hz=p.hz, dt=p.dt, u=p.u, g=p.g, bc=tuple(bcw),
+                  eps_tol=p.eps_tol, max_sweeps=p.max_sweeps, temperature=p.temperature, seed=p.seed,
+                  solve_mu=p.solve_mu)
+    links = O.paper_links_at(p, K, Bx, Bz, ii, jj, kk)
+    zeta = None
+    if p.temperature > 0.0:
+        m = (kk[:, None, None].astype(np.uint64) * np.uint64(p.ny) + jj[None, :, None].astype(np.uint64)) \
+            * np.uint64(p.nx) + ii[None, None, :].astype(np.uint64)
+        zeta = O.langevin_noise_at(p, step, m)
+    psi0 = psi0.astype(np.complex128)
+    b, d = O.build_system(pw, psi0, np.zeros(pw.shape) if mu is None else mu.astype(np.float64), eps, links, zeta)
+    x = psi0
+    for _ in range(sweeps):
+        x, _r = O.jacobi_sweep(pw, x, b, d, links)
+    valid = np.ones(pw.shape, bool)
+    for a, axis in ((0, 2), (1, 1), (2, 0)):
+        m1 = np.ones(len(idx[a]), bool)
+        if not lo_real[a]:
+            m1[:sweeps + 1] = False
+        if not hi_real[a]:
+            m1[len(idx[a]) - sweeps - 1:] = False
+        sh = [1, 1, 1]
+        sh[axis] = len(idx[a])
+        valid &= m1.reshape(sh)
+    return x, valid
