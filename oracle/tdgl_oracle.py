@@ -93,7 +93,19 @@ class Params:
 
     @property
     def cz(self):
+        """1/(g h_z)^2; a film (N_z = 1: the paper's 2D mode) has no z links at all: c_z = 0 (S22)."""
+        if self.nz == 1:
+            return 0.0
         return 1.0 / (self.g ** 2 * self.hz ** 2)
+
+    @property
+    def cell(self):
+        """Volume of a mesh cell, h_x h_y h_z; area h_x h_y for a film (d = 2 in Eq. 38-39; S22)."""
+        return self.hx * self.hy * (self.hz if self.nz > 1 else 1.0)
+
+    def __post_init__(self):
+        if self.nz == 1 and self.bc[2] != PERIODIC:
+            raise ValueError("a film (nz = 1) has no z faces: bc[2] must be PERIODIC")
 
 
 @dataclass
@@ -229,8 +241,9 @@ def site_weights(p: Params):
 # --------------------------------------------------------------------------------------------------
 def zeta_max(p: Params) -> float:
     """Eq. (39): zeta_max = (3 T u / (2 h_t h_x h_y h_z))^{1/2}; per S1/S12 the time step in it is
-    the real step dt and T is the reduced T-bar."""
-    return math.sqrt(3.0 * p.temperature * p.u / (2.0 * p.dt * p.hx * p.hy * p.hz))
+    the real step dt and T is the reduced T-bar.  In d = 2 (film, N_z = 1) the delta function of Eq. (38)
+    discretises as delta_ij/(h_x h_y) ("d = 2, 3"), so h_z drops out (S22)."""
+    return math.sqrt(3.0 * p.temperature * p.u / (2.0 * p.dt * p.cell))
 
 
 def langevin_noise(p: Params, step: int):
@@ -503,7 +516,7 @@ def free_energy(p: Params, psi, eps, links) -> float:
             sl[axis] = -1
             wl[tuple(sl)] = 0.0
         F += c * np.sum(wl * g2)
-    return float(F * p.hx * p.hy * p.hz)
+    return float(F * p.cell)
 
 
 def plaquette_windings(p: Params, psi, links, Bz: float):
