@@ -47,7 +47,9 @@ typedef struct tdgl tdgl_t;
  * Jacobi tolerance (Eq. 34), noise temperature (Eq. 39).  Plain C POD. */
 typedef struct {
   uint32_t struct_size;      /* = sizeof(tdgl_params)                                                  */
-  int32_t  nx, ny, nz;       /* mesh points per axis, each >= 2, nx even                               */
+  int32_t  nx, ny, nz;       /* mesh points per axis; nx, ny >= 2, nx even; nz >= 2, or nz = 1 for a FILM  */
+                             /* (the paper's 2D mode: no z links, bc[2] and hz ignored except  */
+                             /* that Eq. (39) and the free energy use the cell h_x h_y; Bx must be 0)      */
   float    hx, hy, hz;       /* mesh size in xi_0                                                      */
   float    dt;               /* real time step; h_t = dt/u (P:257 fn. 3, S1)                           */
   float    u;                /* relaxation-time ratio, > 0 (S1: 1)                                     */

@@ -348,7 +348,13 @@ static size_t smem_generic(int n, int kind, int TL) {
 }
 static int nfft_x(int n) { int f = 2048 / n; return f < 1 ? 1 : (f > 32 ? 32 : f); }
 static int cc_strided(int n) { return n >= 512 ? 8 : 16; }
-static int tl_generic(int n) { return n > 512 ? 16 : 32; }
+// lines per CTA of the generic O(n^2) transform: as many as fit ~200 KB of shared memory (table + two line buffers)
+static int tl_generic(int n) {
+  const long long tab = 16ll * n;                       // <= 2 (n - 1) doubles
+  int tl = n > 512 ? 16 : 32;
+  while (tl > 1 && tab + 8ll * tl * n > 200 * 1024) tl >>= 1;
+  return tl;
+}
 
 cudaError_t poisson_configure(int nx, int ny, int nz) {
   size_t a = 0, b = 0, c = 0;
@@ -378,6 +384,7 @@ static int transform_axis(const Dev &dv, float *data, int axis, bool divide, flo
   const int ns[3] = {dv.nx, dv.ny, dv.nz};
   const int bcs[3] = {dv.bcx, dv.bcy, dv.bcz};
   const int n = ns[axis];
+  if (n == 1) return 0;                                   // a periodic axis of one point: the transform is the identity
   const bool open = bcs[axis] == 1;
   const long long plane = (long long)dv.nx * dv.ny;
   if (open && dv.bLB[axis] && !divide) {

@@ -3,6 +3,7 @@
 #include "../../include/tdgl.h"
 #include "tdgl_dev.cuh"
 #include "march_tma.h"
+#include "march_film.h"
 #include <cmath>
 #include <cstring>
 #include <new>
@@ -40,6 +41,8 @@ struct tdgl {
   cudaStream_t stream;
   dim3 mgrid;                  // grid of the marching kernels: 128 x 8 tiles x z chunks
   MarchMaps maps;              // TMA tensor maps of psi[0], psi[1], b, d
+  bool film;                   // nz = 1: the paper's 2D mode (S22), kernels of march_film.cu
+  Dev dvp;                     // the Poisson solver's view of the grid (film: y takes the role of z)
   int jav_blocks;
   int last_cuda;
   int64_t launches;            // host-counted kernel launches (graph launches are counted from the log)
@@ -66,17 +69,24 @@ static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 // launch geometry of the marching kernels (march_tma.cu): 128 x 8 tiles, one warp per row; z chunks chosen
 // so that there are enough CTAs for ~4 waves of 2 CTAs/SM, chunks of at least 8 planes
 static void march_geometry(const tdgl_params *p, unsigned *gx, unsigned *gy, unsigned *gz, int *zc_out) {
+  const long long want = 148ll * 2 * 4;
+  if (p->nz == 1) {            // film (march_film.cu): strips of 1024 sites in x, chunks of rows in y
+    const int a = march_film_strips(p->nx);
+    int yc = p->ny;
+    while (yc > 8 && (long long)a * ((p->ny + yc - 1) / yc) < want) yc = (yc + 1) / 2;
+    *gx = (unsigned)a; *gy = (unsigned)((p->ny + yc - 1) / yc); *gz = 1; *zc_out = yc;
+    return;
+  }
   int a, b;
   march_tma_grid(p->nx, p->ny, &a, &b);
   int zc = p->nz;
-  const long long want = 148ll * 2 * 4;
   while (zc > 8 && (long long)a * b * ((p->nz + zc - 1) / zc) < want) zc = (zc + 1) / 2;
   *gx = (unsigned)a; *gy = (unsigned)b; *gz = (unsigned)((p->nz + zc - 1) / zc); *zc_out = zc;
 }
 
 static bool params_ok(const tdgl_params *p) {
   if (!p || p->struct_size != sizeof(tdgl_params)) return false;
-  if (p->nx < 2 || p->ny < 2 || p->nz < 2 || (p->nx & 1)) return false;
+  if (p->nx < 2 || p->ny < 2 || p->nz < 1 || (p->nx & 1)) return false;      // nz = 1: film (2D mode, S22)
   if ((long long)p->nx * p->ny * p->nz > (1ll << 40)) return false;
   if (!(p->hx > 0.f) || !(p->hy > 0.f) || !(p->hz > 0.f) || !(p->dt > 0.f) || !(p->u > 0.f) || !(p->g > 0.f)) return false;
   for (int a = 0; a < 3; ++a)
@@ -139,7 +149,8 @@ extern "C" uint64_t tdgl_workspace_bytes(const tdgl_params *p) {
 }
 
 static void march(tdgl_t *h, int mode, const Dev &dv, cudaStream_t st) {
-  launch_march_tma(mode, dv, h->maps, h->mgrid, st);
+  if (h->film) launch_march_film(mode, dv, h->mgrid, st);
+  else launch_march_tma(mode, dv, h->maps, h->mgrid, st);
 }
 
 // the kernels of one step after the psi solve: J_av + K (a5), rho (a6), mu (a7)
@@ -152,7 +163,7 @@ static int enqueue_after_solve(tdgl_t *h, cudaStream_t st) {
   launch_step_finish(h->dv, (int)(h->mgrid.x * h->mgrid.y * h->mgrid.z), h->jav_blocks, st); ++n;
   if (h->dv.solve_mu) {
     march(h, MODE_RHO, h->dv, st); ++n;
-    n += poisson_solve(h->dv, h->dv.mu, true, st);
+    n += poisson_solve(h->dvp, h->dv.mu, true, st);
   }
   return n;
 }
@@ -210,21 +221,27 @@ extern "C" int tdgl_create(const tdgl_params *p, tdgl_t **out) {
   Dev &dv = h->dv;
   memset(&dv, 0, sizeof(dv));
   carve(p, (char *)p->workspace_dev, &dv);
+  // film (nz = 1): the paper's 2D mode: no z links, no z faces, d = 2 in Eq. (39) (S22)
+  const bool film = p->nz == 1;
+  h->film = film;
+  const int bcs[3] = {p->bc[0], p->bc[1], film ? TDGL_BC_PERIODIC : p->bc[2]};
   dv.nx = p->nx; dv.ny = p->ny; dv.nz = p->nz;
-  dv.bcx = p->bc[0]; dv.bcy = p->bc[1]; dv.bcz = p->bc[2];
+  dv.bcx = bcs[0]; dv.bcy = bcs[1]; dv.bcz = bcs[2];
   dv.N = (long long)p->nx * p->ny * p->nz;
   dv.hx = p->hx; dv.hy = p->hy; dv.hz = p->hz; dv.dt = p->dt;
-  const double cx = 1.0 / (dv.hx * dv.hx), cy = 1.0 / (dv.hy * dv.hy), cz = 1.0 / ((double)p->g * p->g * dv.hz * dv.hz);
+  const double cx = 1.0 / (dv.hx * dv.hx), cy = 1.0 / (dv.hy * dv.hy),
+               cz = film ? 0.0 : 1.0 / ((double)p->g * p->g * dv.hz * dv.hz);
   dv.cx = (float)cx; dv.cy = (float)cy; dv.cz = (float)cz;
   dv.csum2 = (float)(2.0 * (cx + cy + cz));
   dv.ht2 = (float)(0.5 * dv.dt / (double)p->u);
   dv.u = p->u;
   dv.Lx = (p->nx - (p->bc[0] ? 1 : 0)) * dv.hx;
   dv.Ly = (p->ny - (p->bc[1] ? 1 : 0)) * dv.hy;
-  dv.Lz = (p->nz - (p->bc[2] ? 1 : 0)) * dv.hz;
+  dv.Lz = (p->nz - (bcs[2] ? 1 : 0)) * dv.hz;
   // Eq. (39), S12: zeta_max = (3 T u / (2 dt hx hy hz))^{1/2}
   dv.zeta_max = p->temperature > 0.f
-                    ? (float)std::sqrt(3.0 * (double)p->temperature * (double)p->u / (2.0 * dv.dt * dv.hx * dv.hy * dv.hz))
+                    ? (float)std::sqrt(3.0 * (double)p->temperature * (double)p->u /
+                                       (2.0 * dv.dt * dv.hx * dv.hy * (film ? 1.0 : dv.hz)))
                     : 0.f;
   dv.seed_lo = (unsigned)(p->seed & 0xffffffffull);
   dv.seed_hi = (unsigned)(p->seed >> 32);
@@ -238,9 +255,14 @@ extern "C" int tdgl_create(const tdgl_params *p, tdgl_t **out) {
   }
   h->jav_blocks = jav_edge_blocks(dv, march_tma_tile_w());
   h->pred_sweeps = 1;
-  CK(march_tma_configure());
-  if (march_tma_build_maps(dv, &h->maps) != 0) { h->last_cuda = (int)cudaErrorNotSupported; delete h; return TDGL_ECUDA; }
-  CK(poisson_configure(p->nx, p->ny, p->nz));
+  if (film) {
+    CK(march_film_configure());
+  } else {
+    CK(march_tma_configure());
+    if (march_tma_build_maps(dv, &h->maps) != 0) { h->last_cuda = (int)cudaErrorNotSupported; delete h; return TDGL_ECUDA; }
+  }
+  if (film) CK(poisson_configure(p->nx, 1, p->ny));
+  else CK(poisson_configure(p->nx, p->ny, p->nz));
   CK(cudaMallocHost((void **)&h->h_flag, 64));
   CK(cudaEventCreate(&h->ev0));
   CK(cudaEventCreate(&h->ev1));
@@ -249,14 +271,24 @@ extern "C" int tdgl_create(const tdgl_params *p, tdgl_t **out) {
   launch_ctl_reset(dv, p->eps_tol, p->max_sweeps, p->fixed_sweeps, st);
   const int ns[3] = {p->nx, p->ny, p->nz};
   const double cs[3] = {cx, cy, cz};
-  for (int a = 0; a < 3; ++a) launch_build_tables(dv.lam[a], dv.tw[a], dv.tab[a], ns[a], p->bc[a], cs[a], st);
+  for (int a = 0; a < 3; ++a) launch_build_tables(dv.lam[a], dv.tw[a], dv.tab[a], ns[a], bcs[a], cs[a], st);
   for (int a = 0; a < 3; ++a) {
-    dv.bLB[a] = (p->bc[a] == TDGL_BC_OPEN) ? dct_fast_lb(ns[a]) : 0;
+    dv.bLB[a] = (bcs[a] == TDGL_BC_OPEN) ? dct_fast_lb(ns[a]) : 0;
     if (dv.bLB[a]) {
       CK(dct_fast_configure(dv.bLB[a]));
       launch_build_bluestein(dv.bT[a], dv.bC[a], dv.bH[a], ns[a], dv.bLB[a], st);
       h->launches += 1;
     }
+  }
+  // the Poisson solver's view: a film (nx, ny, 1) is solved as the grid (nx, 1, ny) -- x transform, then the y
+  // direction takes the role of z (transform + divide + transform back, or Thomas when y is open)
+  h->dvp = dv;
+  if (film) {
+    Dev &q = h->dvp;
+    q.ny = 1; q.nz = p->ny; q.bcy = TDGL_BC_PERIODIC; q.bcz = bcs[1]; q.cz = (float)cy;
+    q.lam[1] = dv.lam[2]; q.lam[2] = dv.lam[1];        // lam of the length-1 periodic axis is {0}
+    q.tw[2] = dv.tw[1]; q.tab[2] = dv.tab[1];
+    q.bT[2] = dv.bT[1]; q.bC[2] = dv.bC[1]; q.bH[2] = dv.bH[1]; q.bLB[2] = dv.bLB[1]; q.bLB[1] = 0;
   }
   launch_init_state(dv, p->init_amp, st);
   launch_set_field(dv, 0.0, 0.0, 0.0, st);
@@ -302,6 +334,7 @@ extern "C" int tdgl_set_pinning(tdgl_t *h, const tdgl_sphere *sph, int64_t n, fl
 extern "C" int tdgl_set_field_current(tdgl_t *h, float Bx, float By, float Bz, float Jx) {
   if (!h) return TDGL_EINVAL;
   if (By != 0.f) return TDGL_EINCOMPAT;
+  if (h->film && Bx != 0.f) return TDGL_EINCOMPAT;           // a film has no z links for B_x to act on
   if (Jx != 0.f && h->dv.bcx == 1) return TDGL_EINCOMPAT;
   double bx = Bx, bz = Bz;
   const double twopi = 2.0 * 3.14159265358979323846;
@@ -398,7 +431,7 @@ extern "C" int tdgl_observables(tdgl_t *h, tdgl_obs *out) {
   out->K = c.K; out->Ex = c.Ex; out->Jav = c.Jav;
   out->Ex_mean = c.Ex_cnt > 0 ? c.Ex_sum / (double)c.Ex_cnt : 0.0;
   out->mean_abs2 = c.obs[0] / (double)h->dv.N;
-  out->free_energy = (c.obs[1] + c.obs[2]) * h->dv.hx * h->dv.hy * h->dv.hz;
+  out->free_energy = (c.obs[1] + c.obs[2]) * h->dv.hx * h->dv.hy * (h->film ? 1.0 : h->dv.hz);
   out->vortices_per_slice = c.obs[3] / (double)h->dv.nz;
   out->max_resid2 = c.resid_last;
   out->Bx_eff = (float)h->Bx_eff; out->Bz_eff = (float)h->Bz_eff;
@@ -492,7 +525,7 @@ extern "C" int tdgl_debug_poisson(tdgl_t *h, const void *rho_dev, void *mu_dev) 
   if (!h || !rho_dev || !mu_dev) return TDGL_EINVAL;
   if (rho_dev != mu_dev)
     CK(cudaMemcpyAsync(mu_dev, rho_dev, (size_t)h->dv.N * sizeof(float), cudaMemcpyDeviceToDevice, h->stream));
-  h->launches += poisson_solve(h->dv, (float *)mu_dev, true, h->stream);
+  h->launches += poisson_solve(h->dvp, (float *)mu_dev, true, h->stream);
   CKL();
   return TDGL_OK;
 }
