@@ -268,7 +268,8 @@ def main():
             avg_ms = t_ms / n_l
             ach = SWEEP_BYTES_PER_SITE * N / (avg_ms * 1e-3) / 1e9
             tr = ncu_traffic()
-            roof = {"bound": "hbm", "kernel": "k_march_tma<SWEEP> (Jacobi sweep + max-residual)", "achieved": ach,
+            kname = "k_march_film<SWEEP>" if cfg.nz == 1 else "k_march_tma<SWEEP>"
+            roof = {"bound": "hbm", "kernel": kname + " (Jacobi sweep + max-residual)", "achieved": ach,
                     "peak": peak, "unit": "GB/s", "frac": ach / peak, "peak_source": how,
                     "avg_launch_ms": avg_ms, "launches_timed": int(n_l),
                     "algorithmic_bytes_per_launch": SWEEP_BYTES_PER_SITE * N,
@@ -316,7 +317,8 @@ def main():
     if world == 1 and not args.no_cpu_baseline:
         cpu = oracle_sample(cfg)
     out = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        "metric": METRIC if args.config == "C4" else METRIC.replace("512x512x256", "%dx%dx%d" % (cfg.nx, cfg.ny, cfg.nz)),
+        "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
         "data": "synthetic", "steps_per_s": steps_per_s, "sweeps_per_step": sweeps_all / (K * world),
         "config": {"workload": cfg.name, "grid": [cfg.nx, cfg.ny, cfg.nz], "bc": list(cfg.bc), "h": cfg.h, "dt": cfg.dt,

@@ -130,7 +130,7 @@ k_dct_s(float *__restrict__ data, int n, long long stride, long long ostride, in
   for (int r = 0; r < 8; ++r) {
     const int q = j + r * TPF;
     if (q < n && valid) {
-      const float2 w = cmul(Cg[q], sm[q * CC + f]);
+      const float2 w = cmul(Cg[q], sm[saddr<LB, false, CC>(f, q)]);
       *reinterpret_cast<float2 *>(base + q * stride) = make_float2(w.x * inv, -w.y * inv);
     }
   }
@@ -152,7 +152,7 @@ template <int LB> struct DctCfg {
   static constexpr int F = (TPF >= 256) ? 1 : 256 / TPF;
   static constexpr int CC = (8192 / LB > 16) ? 16 : 8192 / LB;
   static size_t smem_x() { return (size_t)(LB + F * (LB + LB / 8)) * sizeof(float2); }
-  static size_t smem_s() { return (size_t)(LB + (size_t)LB * CC) * sizeof(float2); }
+  static size_t smem_s() { return (size_t)(LB + sbuf_elems_s(LB, CC)) * sizeof(float2); }
 };
 template <int LB> static cudaError_t cfg_dct() {
   cudaError_t e = cudaFuncSetAttribute(k_dct_x<LB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)DctCfg<LB>::smem_x());

@@ -12,14 +12,14 @@
 
 // ---- x pass: contiguous rows, two rows per complex FFT, F = 2048/N pairs per CTA (256 threads) ----------
 template <int N>
-__global__ void __launch_bounds__(256) k_dht_x_fast(float *__restrict__ data, long long nrows,
-                                                    const float2 *__restrict__ twg) {
-  constexpr int F = 2048 / N, TPF = N / 8;
+__global__ void __launch_bounds__((N > 2048) ? N / 8 : 256) k_dht_x_fast(float *__restrict__ data, long long nrows,
+                                                                          const float2 *__restrict__ twg) {
+  constexpr int F = (N >= 2048) ? 1 : 2048 / N, TPF = N / 8, NT = F * TPF;
   extern __shared__ float4 smem4[];
   float2 *tw = reinterpret_cast<float2 *>(smem4);
   float2 *sm = tw + N;
   const int tid = threadIdx.x;
-  fill_twiddles<N>(tw, twg, tid, 256);
+  fill_twiddles<N>(tw, twg, tid, NT);
   const int j = tid % TPF, f = tid / TPF;
   const long long ra = 2 * ((long long)blockIdx.x * F + f), rb = ra + 1;
   const bool va = ra < nrows, vb = rb < nrows;
@@ -76,7 +76,7 @@ __global__ void __launch_bounds__(CC *N / 8) k_dht_s_fast(float *__restrict__ da
       const int q = j + r * TPF;
       const float lz = lamz[q] + ly;
       const float la = lxa + lz, lb = lxb + lz;
-      float2 z = sm[q * CC + f];
+      float2 z = sm[saddr<N, false, CC>(f, q)];
       z.x = (la != 0.f) ? z.x * (scale / la) : 0.f;
       z.y = (lb != 0.f) ? z.y * (scale / lb) : 0.f;
       v[r] = z;
@@ -89,19 +89,21 @@ __global__ void __launch_bounds__(CC *N / 8) k_dht_s_fast(float *__restrict__ da
 #pragma unroll
     for (int r = 0; r < 8; ++r) {
       const int p = j + r * TPF;
-      *reinterpret_cast<float2 *>(base + p * stride) = sm[p * CC + f];
+      *reinterpret_cast<float2 *>(base + p * stride) = sm[saddr<N, false, CC>(f, p)];
     }
   }
 }
 
 // ---- host side ---------------------------------------------------------------------------------------
-static size_t smem_x(int n) { return (size_t)(n + 2048 + 256) * sizeof(float2); }
-static size_t smem_s(int n, int cc) { return (size_t)(n + (size_t)n * cc) * sizeof(float2); }
+static size_t smem_x(int n) { const int f = n >= 2048 ? 1 : 2048 / n; return (size_t)(n + f * (n + n / 8)) * sizeof(float2); }
+static size_t smem_s(int n, int cc) { return (size_t)(n + sbuf_elems_s(n, cc)) * sizeof(float2); }
+// float2 columns per CTA of the strided pass: CC N/8 threads <= 1024
+constexpr int cc_of(int n) { return n >= 8192 ? 1 : n >= 4096 ? 2 : n >= 2048 ? 4 : n >= 512 ? 8 : 16; }
 
-bool dht_fast_supported(int n) { return n == 64 || n == 128 || n == 256 || n == 512 || n == 1024; }
+bool dht_fast_supported(int n) { return n >= 64 && n <= 8192 && (n & (n - 1)) == 0; }
 
 template <int N> static cudaError_t cfg_n() {
-  constexpr int CC = (N >= 512) ? 8 : 16;
+  constexpr int CC = cc_of(N);
   cudaError_t e = cudaFuncSetAttribute(k_dht_x_fast<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_x(N));
   if (e != cudaSuccess) return e;
   return cudaFuncSetAttribute(k_dht_s_fast<N, CC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_s(N, CC));
@@ -113,14 +115,17 @@ cudaError_t dht_fast_configure(int n) {
     case 256: return cfg_n<256>();
     case 512: return cfg_n<512>();
     case 1024: return cfg_n<1024>();
+    case 2048: return cfg_n<2048>();
+    case 4096: return cfg_n<4096>();
+    case 8192: return cfg_n<8192>();
   }
   return cudaSuccess;
 }
 
 template <int N> static void run_x(float *data, long long nrows, const float2 *tw, cudaStream_t st) {
-  constexpr int F = 2048 / N;
+  constexpr int F = (N >= 2048) ? 1 : 2048 / N;
   const long long npairs = (nrows + 1) / 2;
-  k_dht_x_fast<N><<<(unsigned)((npairs + F - 1) / F), 256, smem_x(N), st>>>(data, nrows, tw);
+  k_dht_x_fast<N><<<(unsigned)((npairs + F - 1) / F), F * (N / 8), smem_x(N), st>>>(data, nrows, tw);
 }
 void launch_dht_x_fast(float *data, int n, long long nrows, const float2 *tw, cudaStream_t st) {
   switch (n) {
@@ -129,13 +134,16 @@ void launch_dht_x_fast(float *data, int n, long long nrows, const float2 *tw, cu
     case 256: run_x<256>(data, nrows, tw, st); break;
     case 512: run_x<512>(data, nrows, tw, st); break;
     case 1024: run_x<1024>(data, nrows, tw, st); break;
+    case 2048: run_x<2048>(data, nrows, tw, st); break;
+    case 4096: run_x<4096>(data, nrows, tw, st); break;
+    case 8192: run_x<8192>(data, nrows, tw, st); break;
   }
 }
 
 template <int N>
 static void run_s(float *data, long long stride, long long ostride, int ncolc, int nother, const float2 *tw, int divide,
                   float scale, const float *lx, const float *ly, const float *lz, cudaStream_t st) {
-  constexpr int CC = (N >= 512) ? 8 : 16;
+  constexpr int CC = cc_of(N);
   dim3 grid((ncolc + CC - 1) / CC, nother);
   k_dht_s_fast<N, CC><<<grid, CC * N / 8, smem_s(N, CC), st>>>(data, stride, ostride, ncolc, tw, divide, scale, lx, ly, lz);
 }
@@ -147,5 +155,8 @@ void launch_dht_s_fast(float *data, int n, long long stride, long long ostride, 
     case 256: run_s<256>(data, stride, ostride, ncolc, nother, tw, divide, scale, lx, ly, lz, st); break;
     case 512: run_s<512>(data, stride, ostride, ncolc, nother, tw, divide, scale, lx, ly, lz, st); break;
     case 1024: run_s<1024>(data, stride, ostride, ncolc, nother, tw, divide, scale, lx, ly, lz, st); break;
+    case 2048: run_s<2048>(data, stride, ostride, ncolc, nother, tw, divide, scale, lx, ly, lz, st); break;
+    case 4096: run_s<4096>(data, stride, ostride, ncolc, nother, tw, divide, scale, lx, ly, lz, st); break;
+    case 8192: run_s<8192>(data, stride, ostride, ncolc, nother, tw, divide, scale, lx, ly, lz, st); break;
   }
 }

@@ -41,14 +41,17 @@ template <> __device__ __forceinline__ void dft<8>(float2 *v) {
 
 // shared-memory address of element p of line f
 template <int N, bool XPASS, int CC> __device__ __forceinline__ int saddr(int f, int p) {
-  return XPASS ? f * (N + N / 8) + p + (p >> 3) : p * CC + f;
+  return XPASS ? f * (N + N / 8) + p + (p >> 3) : (CC < 8 ? (p + (p >> 3)) * CC + f : p * CC + f);
 }
+// elements of the shared work buffer of a y/z pass (fewer than 8 columns per CTA: rows padded 9/8 like the x pass,
+// otherwise the stride-8 accesses of the radix-8 stages fall into a few banks)
+__host__ __device__ constexpr size_t sbuf_elems_s(int n, int cc) { return (size_t)(cc < 8 ? n + n / 8 : n) * cc; }
 
 // Twiddles in shared memory, one compact table per (stage, r):  ct[tw_off(NS) + (r-1) NS + k] = exp(-2 pi i r k/(NS R)),
 // k < NS.  Lanes with consecutive k read consecutive addresses (the plain table tw[r k N/(NS R)] put the even
 // multiples of a stage into a few banks: ncu showed half of all shared wavefronts of the x pass were conflicts).
 // The values are the entries of the fp64-built global table exp(-2 pi i m/N), so results are unchanged.
-__host__ __device__ constexpr int tw_off(int NS) { return NS == 8 ? 0 : NS == 64 ? 56 : 504; }
+__host__ __device__ constexpr int tw_off(int NS) { return NS == 8 ? 0 : NS == 64 ? 56 : NS == 512 ? 504 : 4088; }
 __host__ __device__ constexpr int radix_of(int N, int NS) { return (N / NS >= 8) ? 8 : N / NS; }
 template <int N> __device__ __forceinline__ void fill_twiddles(float2 *ct, const float2 *__restrict__ twg, int tid, int nth) {
 #pragma unroll
@@ -95,7 +98,7 @@ __device__ __forceinline__ void stage(float2 *v, float2 *sm, const float2 *tw, i
 // memory in natural order.
 template <int N, bool XPASS, int CC, bool FROM_SMEM>
 __device__ __forceinline__ void fft_regs(float2 *v, float2 *sm, const float2 *tw, int j, int f) {
-  constexpr int L = (N == 64) ? 6 : (N == 128) ? 7 : (N == 256) ? 8 : (N == 512) ? 9 : (N == 1024) ? 10 : (N == 2048) ? 11 : 12;
+  constexpr int L = (N == 64) ? 6 : (N == 128) ? 7 : (N == 256) ? 8 : (N == 512) ? 9 : (N == 1024) ? 10 : (N == 2048) ? 11 : (N == 4096) ? 12 : 13;
   if (FROM_SMEM) {
 #pragma unroll
     for (int r = 0; r < 8; ++r) v[r] = sm[saddr<N, XPASS, CC>(f, j + r * (N / 8))];
@@ -108,7 +111,8 @@ __device__ __forceinline__ void fft_regs(float2 *v, float2 *sm, const float2 *tw
   if (L >= 9) stage<N, 8, 64, XPASS, CC, false>(v, sm, tw, j, f);
   if (L == 10) stage<N, 2, 512, XPASS, CC, false>(v, sm, tw, j, f);
   if (L == 11) stage<N, 4, 512, XPASS, CC, false>(v, sm, tw, j, f);
-  if (L == 12) stage<N, 8, 512, XPASS, CC, false>(v, sm, tw, j, f);
+  if (L >= 12) stage<N, 8, 512, XPASS, CC, false>(v, sm, tw, j, f);
+  if (L == 13) stage<N, 2, 4096, XPASS, CC, false>(v, sm, tw, j, f);
 }
 
 // Untangle the spectrum of the packed pair into the two Hartley spectra, in place in shared memory.

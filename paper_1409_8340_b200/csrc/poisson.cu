@@ -321,7 +321,8 @@ __global__ void k_build_tables(float *lam, float2 *tw, double *tab, int n, int o
 // ---------------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------------
-static bool is_pow2(int n) { return n >= 4 && (n & (n - 1)) == 0; }
+// lengths of the shared-memory radix-4 fallback (powers of two below the register-blocked path's range)
+static bool is_pow2(int n) { return n >= 4 && n < 64 && (n & (n - 1)) == 0; }
 
 // Bluestein DCT-I fast path (dct.cu)
 void launch_dct_x(float *data, int n, int LB, long long nrows, const float2 *T, const float2 *C, const float2 *H,

@@ -93,6 +93,13 @@ CONFIGS = {
     # C5b: same grid, x periodic so that the transport current Jx=0.01 of BASELINE.json can flow.
     "C5b": Config("C5b", 1024, 1024, 512, (PERIODIC, OPEN, OPEN), Bz=0.2, Jx=0.01,
                   temperature=1e-3, incl_fraction=0.10, incl_rmin=1.0, incl_rmax=4.0, steps=500),
+    # The paper's own timed workloads ("disorder-free system with periodic boundary conditions
+    # with a magnetic field applied in z direction and an external current in x direction", eps_tol 1e-6), as
+    # context beside its K20Xm numbers.  The paper gives neither B nor J for them; B_z = 0.1 puts ~267 000 vortices
+    # on the 8192^2 film, the ">250 000" of its Fig. 4; J_x = 0.02 and T = 0 are ours.
+    "F2D": Config("F2D", 8192, 8192, 1, (PERIODIC, PERIODIC, PERIODIC), Bz=0.1, Jx=0.02, steps=1000),
+    # 3D counterpart of its 406^3 run (66.9e6 sites): 512 x 512 x 256 (67.1e6 sites), all periodic, eps = 1.
+    "P3D": Config("P3D", 512, 512, 256, (PERIODIC, PERIODIC, PERIODIC), Bz=0.1, Jx=0.02, steps=1000),
 }
 C3_CURRENTS = tuple(round(0.005 * (i + 1), 6) for i in range(10))   # 0.005 .. 0.05
 

@@ -73,9 +73,10 @@ def oracle_window_solve(p, psi0, eps, Bx, Bz, K, step, sweeps, ii, jj, kk, mu=No
     bcw, lo_real, hi_real = [], [], []
     for a in range(3):
         op = p.bc[a] == O.OPEN
-        lo_real.append(op and idx[a][0] == 0)
-        hi_real.append(op and idx[a][-1] == n[a] - 1)
-        bcw.append(O.OPEN if (lo_real[a] or hi_real[a]) else O.PERIODIC)
+        whole = (not op) and len(idx[a]) == n[a]             # the window spans a periodic axis: its wrap is the real one
+        lo_real.append(whole or (op and idx[a][0] == 0))
+        hi_real.append(whole or (op and idx[a][-1] == n[a] - 1))
+        bcw.append(O.OPEN if (op and (lo_real[a] or hi_real[a])) else O.PERIODIC)
     pw = O.Params(len(ii), len(jj), len(kk), hx=p.hx, hy=p.hy, hz=p.hz, dt=p.dt, u=p.u, g=p.g, bc=tuple(bcw),
                   eps_tol=p.eps_tol, max_sweeps=p.max_sweeps, temperature=p.temperature, seed=p.seed,
                   solve_mu=p.solve_mu)
