@@ -230,70 +230,84 @@ __global__ void __launch_bounds__(256) k_transform_generic(float *__restrict__ d
 // Forward: pivots and modified right side (fp64 arithmetic, fp32 storage: c' -> scratch, d' in place).
 // The (0,0) line is singular (Neumann): its last unknown is pinned to 0 and the z-weighted mean is
 // removed afterwards (S7).
-__global__ void __launch_bounds__(128) k_thomas_z(float *__restrict__ data, float *__restrict__ cp, int nx, int ny,
-                                                  int nz, float cz, float scale, const float *__restrict__ lamx,
-                                                  const float *__restrict__ lamy) {
-  const long long col = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+// Two adjacent lines (columns i, i+1: one 8-byte access) per thread: twice the loads in flight per thread and half
+// the threads, so that the whole plane is resident in one wave (ncu: the one-line version ran 1.54 waves and was
+// latency bound, 46 % of DRAM peak).
+__global__ void __launch_bounds__(64) k_thomas_z(float *__restrict__ data, float *__restrict__ cp, int nx, int ny,
+                                                 int nz, float cz, float scale, const float *__restrict__ lamx,
+                                                 const float *__restrict__ lamy) {
+  const long long pr = (long long)blockIdx.x * blockDim.x + threadIdx.x;     // pair index
   const long long plane = (long long)nx * ny;
+  const long long col = 2 * pr;
   if (col >= plane) return;
   const int j = (int)(col / nx), i = (int)(col - (long long)j * nx);
-  const double lam = (double)lamx[i] + (double)lamy[j];
-  const bool zero = (lam == 0.0);
-  const double bq = -2.0 + lam / (double)cz;          // diagonal / c_z
+  const double ly = (double)lamy[j];
+  const double lam[2] = {(double)lamx[i] + ly, (double)lamx[i + 1] + ly};
+  const bool zero[2] = {lam[0] == 0.0, lam[1] == 0.0};
+  const double bq[2] = {-2.0 + lam[0] / (double)cz, -2.0 + lam[1] / (double)cz};   // diagonal / c_z
   const double rs = (double)scale / (double)cz;
-  float *x = data + col;
-  float *c = cp + col;
-  // forward elimination, 8 planes per batch so that 8 independent loads are in flight per thread
-  double cprev = 0.0, dprev = 0.0;
+  float2 *x = reinterpret_cast<float2 *>(data + col);
+  float2 *c = reinterpret_cast<float2 *>(cp + col);
+  const long long ps = plane / 2;                                            // plane stride in float2 units
+  // forward elimination, 8 planes per batch so that 8 independent 8-byte loads are in flight per thread
+  double cprev[2] = {0.0, 0.0}, dprev[2] = {0.0, 0.0};
   for (int kb = 0; kb < nz; kb += 8) {
-    float xin[8];
+    float2 xin[8];
 #pragma unroll
-    for (int u = 0; u < 8; ++u) xin[u] = (kb + u < nz) ? __ldcs(x + (long long)(kb + u) * plane) : 0.f;
+    for (int u = 0; u < 8; ++u) xin[u] = (kb + u < nz) ? __ldcs(x + (long long)(kb + u) * ps) : make_float2(0.f, 0.f);
 #pragma unroll
     for (int u = 0; u < 8; ++u) {
       const int k = kb + u;
       if (k < nz) {
-        const double rhs = (double)xin[u] * rs;
-        double inv, dk;
-        if (k == 0) {                                   // row 0: off-diagonal 2
-          inv = 2.0 / bq;
-          dk = rhs / bq;
-        } else {
-          const double a = (k == nz - 1) ? 2.0 : 1.0;
-          if (zero && k == nz - 1) { inv = 0.0; dk = 0.0; }
-          else { inv = 1.0 / (bq - a * cprev); dk = (rhs - a * dprev) * inv; }
+        const double rhs[2] = {(double)xin[u].x * rs, (double)xin[u].y * rs};
+        float co[2], xo[2];
+#pragma unroll
+        for (int q = 0; q < 2; ++q) {
+          double inv, dk;
+          if (k == 0) {                                 // row 0: off-diagonal 2
+            inv = 2.0 / bq[q];
+            dk = rhs[q] / bq[q];
+          } else {
+            const double a = (k == nz - 1) ? 2.0 : 1.0;
+            if (zero[q] && k == nz - 1) { inv = 0.0; dk = 0.0; }
+            else { inv = 1.0 / (bq[q] - a * cprev[q]); dk = (rhs[q] - a * dprev[q]) * inv; }
+          }
+          cprev[q] = inv;
+          dprev[q] = dk;
+          co[q] = (float)inv;
+          xo[q] = (float)dk;
         }
-        cprev = inv;
-        dprev = dk;
-        c[(long long)k * plane] = (float)inv;
-        x[(long long)k * plane] = (float)dk;
+        c[(long long)k * ps] = make_float2(co[0], co[1]);
+        x[(long long)k * ps] = make_float2(xo[0], xo[1]);
       }
     }
   }
   // back substitution, same batching (descending)
-  double xn = 0.0;
+  double xn[2] = {0.0, 0.0};
   for (int kb = nz - 1; kb >= 0; kb -= 8) {
-    float xv[8], cv[8];
+    float2 xv[8], cv[8];
 #pragma unroll
     for (int u = 0; u < 8; ++u) {
       const int k = kb - u;
-      xv[u] = (k >= 0) ? x[(long long)k * plane] : 0.f;
-      cv[u] = (k >= 0) ? __ldcs(c + (long long)k * plane) : 0.f;
+      xv[u] = (k >= 0) ? x[(long long)k * ps] : make_float2(0.f, 0.f);
+      cv[u] = (k >= 0) ? __ldcs(c + (long long)k * ps) : make_float2(0.f, 0.f);
     }
 #pragma unroll
     for (int u = 0; u < 8; ++u) {
       const int k = kb - u;
       if (k >= 0) {
-        xn = (k == nz - 1) ? (double)xv[u] : (double)xv[u] - (double)cv[u] * xn;
-        x[(long long)k * plane] = (float)xn;
+        xn[0] = (k == nz - 1) ? (double)xv[u].x : (double)xv[u].x - (double)cv[u].x * xn[0];
+        xn[1] = (k == nz - 1) ? (double)xv[u].y : (double)xv[u].y - (double)cv[u].y * xn[1];
+        x[(long long)k * ps] = make_float2((float)xn[0], (float)xn[1]);
       }
     }
   }
-  if (zero) {
+  if (zero[0] || zero[1]) {                             // singular Neumann line: remove its z-weighted mean (S7)
+    float *xs = data + col + (zero[0] ? 0 : 1);
     double s = 0.0;
-    for (int k = 0; k < nz; ++k) s += ((k == 0 || k == nz - 1) ? 0.5 : 1.0) * (double)x[k * plane];
+    for (int k = 0; k < nz; ++k) s += ((k == 0 || k == nz - 1) ? 0.5 : 1.0) * (double)xs[k * plane];
     const float mean = (float)(s / (double)(nz - 1));
-    for (int k = 0; k < nz; ++k) x[k * plane] -= mean;
+    for (int k = 0; k < nz; ++k) xs[k * plane] -= mean;
   }
 }
 
@@ -450,7 +464,7 @@ int poisson_solve(const Dev &dv, float *data, bool thomas_open_z, cudaStream_t s
   if (dv.bcz == 1 && thomas_open_z) {
     const long long plane = (long long)dv.nx * dv.ny;
     const float scale = (float)(1.0 / (nrm[0] * nrm[1]));
-    k_thomas_z<<<(unsigned)((plane + 127) / 128), 128, 0, st>>>(data, dv.scratch, dv.nx, dv.ny, dv.nz, dv.cz, scale,
+    k_thomas_z<<<(unsigned)((plane / 2 + 63) / 64), 64, 0, st>>>(data, dv.scratch, dv.nx, dv.ny, dv.nz, dv.cz, scale,
                                                                  dv.lam[0], dv.lam[1]);
     launches += 1;
   } else {
