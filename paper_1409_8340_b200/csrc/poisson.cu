@@ -251,10 +251,15 @@ __global__ void __launch_bounds__(64) k_thomas_z(float *__restrict__ data, float
   const long long ps = plane / 2;                                            // plane stride in float2 units
   // forward elimination, 8 planes per batch so that 8 independent 8-byte loads are in flight per thread
   double cprev[2] = {0.0, 0.0}, dprev[2] = {0.0, 0.0};
+  float2 xnext[8];                                       // the next batch is in flight while this one is eliminated
+#pragma unroll
+  for (int u = 0; u < 8; ++u) xnext[u] = (u < nz) ? __ldcs(x + (long long)u * ps) : make_float2(0.f, 0.f);
   for (int kb = 0; kb < nz; kb += 8) {
     float2 xin[8];
 #pragma unroll
-    for (int u = 0; u < 8; ++u) xin[u] = (kb + u < nz) ? __ldcs(x + (long long)(kb + u) * ps) : make_float2(0.f, 0.f);
+    for (int u = 0; u < 8; ++u) xin[u] = xnext[u];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) xnext[u] = (kb + 8 + u < nz) ? __ldcs(x + (long long)(kb + 8 + u) * ps) : make_float2(0.f, 0.f);
 #pragma unroll
     for (int u = 0; u < 8; ++u) {
       const int k = kb + u;
@@ -284,13 +289,22 @@ __global__ void __launch_bounds__(64) k_thomas_z(float *__restrict__ data, float
   }
   // back substitution, same batching (descending)
   double xn[2] = {0.0, 0.0};
+  float2 xvn[8], cvn[8];
+#pragma unroll
+  for (int u = 0; u < 8; ++u) {
+    const int k = nz - 1 - u;
+    xvn[u] = (k >= 0) ? x[(long long)k * ps] : make_float2(0.f, 0.f);
+    cvn[u] = (k >= 0) ? __ldcs(c + (long long)k * ps) : make_float2(0.f, 0.f);
+  }
   for (int kb = nz - 1; kb >= 0; kb -= 8) {
     float2 xv[8], cv[8];
 #pragma unroll
+    for (int u = 0; u < 8; ++u) { xv[u] = xvn[u]; cv[u] = cvn[u]; }
+#pragma unroll
     for (int u = 0; u < 8; ++u) {
-      const int k = kb - u;
-      xv[u] = (k >= 0) ? x[(long long)k * ps] : make_float2(0.f, 0.f);
-      cv[u] = (k >= 0) ? __ldcs(c + (long long)k * ps) : make_float2(0.f, 0.f);
+      const int k = kb - 8 - u;
+      xvn[u] = (k >= 0) ? x[(long long)k * ps] : make_float2(0.f, 0.f);
+      cvn[u] = (k >= 0) ? __ldcs(c + (long long)k * ps) : make_float2(0.f, 0.f);
     }
 #pragma unroll
     for (int u = 0; u < 8; ++u) {
