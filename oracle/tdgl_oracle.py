@@ -176,6 +176,48 @@ def paper_links_at(p: Params, K: float, Bx: float, Bz: float, ii, jj, kk):
     return thx, thy, thz
 
 
+def snap_field_yz(p: Params, By: float, Bz: float) -> Tuple[float, float, Optional[int], Optional[int]]:
+    """Flux quantisation for a field in the yz plane (P:467 applied to the jump P_{j,k} of P:459):
+    B_z = 2 pi n_z/(L_x L_y) iff x and y are periodic, B_y = 2 pi n_y/(L_x L_z) iff x and z are periodic."""
+    nzq = nyq = None
+    if p.bc[0] == PERIODIC and p.bc[1] == PERIODIC:
+        a = p.length("x") * p.length("y")
+        nzq = int(np.rint(Bz * a / (2.0 * math.pi)))
+        Bz = 2.0 * math.pi * nzq / a
+    if p.bc[0] == PERIODIC and p.bc[2] == PERIODIC:
+        a = p.length("x") * p.length("z")
+        nyq = int(np.rint(By * a / (2.0 * math.pi)))
+        By = 2.0 * math.pi * nyq / a
+    return By, Bz, nyq, nzq
+
+
+def paper_links_yz(p: Params, K: float, By: float, Bz: float):
+    """Link phases of the yz Landau gauge, A^{yz} = xbar [0, B_z, -B_y], xbar = i h_x - L_x/2 (Eq. 24b with
+    the typo "B_u" -> B_y; Eq. 25b; discretised as Eq. 29b):
+        th_x = h_x K,   th_y(i) = -h_y B_z xbar_i,   th_z(i) = +h_z B_y xbar_i        (U = exp(-i h A~))
+    Quasi-periodic jump in x: psi_{-1,j,k} = P_{j,k} psi_{Nx-1,j,k},
+        P_{j,k} = exp(i (-j h_y L_x B_z + k h_z L_x B_y)),
+    i.e. the wrap link that leaves column Nx-1 in +x carries exp(i th_x) P*_{j,k}."""
+    return paper_links_yz_at(p, K, By, Bz, np.arange(p.nx), np.arange(p.ny), np.arange(p.nz))
+
+
+def paper_links_yz_at(p: Params, K: float, By: float, Bz: float, ii, jj, kk):
+    """`paper_links_yz` on the sub-lattice of global indices ii x jj x kk (see `paper_links_at`)."""
+    ii, jj, kk = (np.asarray(a, dtype=np.int64) for a in (ii, jj, kk))
+    shape = (len(kk), len(jj), len(ii))
+    xbar = (ii * p.hx - p.length("x") / 2.0)[None, None, :]
+    thx = np.full(shape, p.hx * K)
+    thy = np.broadcast_to(-p.hy * Bz * xbar, shape).copy()
+    thz = np.broadcast_to(p.hz * By * xbar, shape).copy()
+    if p.bc[0] == PERIODIC:
+        j = jj[None, :]
+        k = kk[:, None]
+        wrap = -(-j * p.hy * p.length("x") * Bz + k * p.hz * p.length("x") * By)
+        for w in np.nonzero(ii == p.nx - 1)[0]:
+            thx[:, :, w] += wrap
+    return thx, thy, thz
+
+
 # --------------------------------------------------------------------------------------------------
 # neighbour operators
 # --------------------------------------------------------------------------------------------------
