@@ -38,6 +38,9 @@ extern "C" {
 #define TDGL_BC_OPEN       1    /* open: n.(grad - iA)psi = 0, n.grad(mu) = 0            */
 
 #define TDGL_FLAG_SOLVE_MU 1u   /* mu and K are active (S15).  Off: mu == 0, K == 0             */
+#define TDGL_FLAG_GAUGE_YZ 4u   /* field in the yz plane: Landau gauge A = xbar [0, Bz, -By] (Eq. 24b),
+                                   quasi-periodic jump in x.  set_field_current then takes By (Bx
+                                   must be 0) and tdgl_obs.Bx_eff reports the effective B_y.  Not for films. */
 #define TDGL_FLAG_HOST_LOOP 2u  /* test/diagnostic: host-driven sweep loop instead of the CUDA-graph
                                    WHILE node (identical arithmetic)                                     */
 

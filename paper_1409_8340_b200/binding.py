@@ -12,7 +12,7 @@ _LIB_PATH = os.environ.get("TDGL_LIB") or os.path.join(_HERE, "libtdgl.so")     
 
 TDGL_OK, TDGL_EINVAL, TDGL_ENOMEM, TDGL_EINCOMPAT, TDGL_ECUDA, TDGL_WMAXSWEEPS = 0, -1, -2, -3, -4, 1
 TDGL_BC_PERIODIC, TDGL_BC_OPEN = 0, 1
-TDGL_FLAG_SOLVE_MU, TDGL_FLAG_HOST_LOOP = 1, 2
+TDGL_FLAG_SOLVE_MU, TDGL_FLAG_HOST_LOOP, TDGL_FLAG_GAUGE_YZ = 1, 2, 4
 
 EXPORTS = (
     "tdgl_workspace_bytes", "tdgl_create", "tdgl_destroy", "tdgl_set_pinning", "tdgl_set_field_current", "tdgl_step",
@@ -156,7 +156,8 @@ class Solver:
     def __init__(self, nx: int, ny: int, nz: int, bc: Sequence[int] = (0, 0, 0), h: float = 0.5, dt: float = 0.1,
                  u: float = 1.0, g: float = 1.0, eps_tol: float = 1e-6, max_sweeps: int = 100, fixed_sweeps: int = 0,
                  temperature: float = 0.0, seed: int = 0, init_amp: float = 0.01, solve_mu: bool = True,
-                 host_loop: bool = False, hxyz: Optional[Sequence[float]] = None, device: str = "cuda:0"):
+                 host_loop: bool = False, hxyz: Optional[Sequence[float]] = None, device: str = "cuda:0",
+                 gauge_yz: bool = False):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1409_8340_b200 needs a CUDA device (sm_100a); there is no CPU path")
@@ -170,7 +171,8 @@ class Solver:
         p.bc[0], p.bc[1], p.bc[2] = bc
         p.eps_tol, p.max_sweeps, p.fixed_sweeps = eps_tol, max_sweeps, fixed_sweeps
         p.temperature, p.seed, p.init_amp = temperature, seed, init_amp
-        p.flags = (TDGL_FLAG_SOLVE_MU if solve_mu else 0) | (TDGL_FLAG_HOST_LOOP if host_loop else 0)
+        p.flags = ((TDGL_FLAG_SOLVE_MU if solve_mu else 0) | (TDGL_FLAG_HOST_LOOP if host_loop else 0)
+                   | (TDGL_FLAG_GAUGE_YZ if gauge_yz else 0))
         nbytes = tdgl_workspace_bytes(p)
         if nbytes == 0:
             raise TdglError(TDGL_EINVAL, "tdgl_workspace_bytes")

@@ -40,6 +40,27 @@ __global__ void k_set_field(const __grid_constant__ Dev dv, double Bx, double Bz
     dv.ctl->Bx = Bx; dv.ctl->Bz = Bz; dv.ctl->Jext = Jext; dv.ctl->Ex_sum = 0.0; dv.ctl->Ex_cnt = 0;
   }
   double s, c;
+  if (dv.gauge_yz) {
+    // yz gauge (Eq. 24b; "Bx" carries B_y): U_y(i) = exp(-i h_y B_z xbar_i), U_z(i) = exp(+i h_z B_y xbar_i),
+    // Pj[j] = exp(-i j h_y L_x B_z), Pk[k] = exp(+i k h_z L_x B_y), P_{j,k} = Pj[j] Pk[k]
+    const double By = Bx;
+    for (int i = tid; i < dv.nx; i += nth) {
+      const double xbar = i * dv.hx - 0.5 * dv.Lx;
+      sincos(-dv.hy * Bz * xbar, &s, &c);
+      dv.Uy[i] = make_float2((float)c, (float)s);
+      sincos(dv.hz * By * xbar, &s, &c);
+      dv.Uzx[i] = make_float2((float)c, (float)s);
+    }
+    for (int j = tid; j < dv.ny; j += nth) {
+      sincos(-(double)j * dv.hy * dv.Lx * Bz, &s, &c);
+      dv.Pj[j] = make_float2((float)c, (float)s);
+    }
+    for (int k = tid; k < dv.nz; k += nth) {
+      sincos((double)k * dv.hz * dv.Lx * By, &s, &c);
+      dv.Pk[k] = make_float2((float)c, (float)s);
+    }
+    return;
+  }
   for (int j = tid; j < dv.ny; j += nth) {
     const double ybar = j * dv.hy - 0.5 * dv.Ly;
     sincos(-dv.hz * Bx * ybar, &s, &c);
@@ -137,10 +158,13 @@ __global__ void __launch_bounds__(256) k_obs_partial(const __grid_constant__ Dev
     const long long base = (long long)nx * ((long long)ny * k);
     const float2 Pk = dv.Pk[k];
     // forward neighbours with their link variables
-    const float2 e = cmul(dv.Ux[j], x[base + (long long)nx * j + ip]);
+    const bool yz = dv.gauge_yz != 0;
+    float2 e = cmul(dv.Ux[j], x[base + (long long)nx * j + ip]);
+    if (yz && dv.bcx == 0 && i + 1 == nx) e = cmulc(cmul(dv.Pj[j], Pk), e);       // yz: conj(P_{j,k}) psi_{0,j,k}
     float2 nn = x[base + (long long)nx * jp + i];
-    if (dv.bcy == 0 && j + 1 == ny) nn = cmulc(cmulc(Pk, dv.Pi[i]), nn);          // conj(P_{i,k}) psi_{i,0,k}
-    const float2 t = cmul(dv.Uz[j], x[(long long)nx * ((long long)ny * kp + j) + i]);
+    if (yz) nn = cmul(dv.Uy[i], nn);
+    else if (dv.bcy == 0 && j + 1 == ny) nn = cmulc(cmulc(Pk, dv.Pi[i]), nn);     // xz: conj(P_{i,k}) psi_{i,0,k}
+    const float2 t = cmul(yz ? dv.Uzx[i] : dv.Uz[j], x[(long long)nx * ((long long)ny * kp + j) + i]);
     float g = 0.f;
     if (hasx) g += dv.cx * wy * wz * ((e.x - c.x) * (e.x - c.x) + (e.y - c.y) * (e.y - c.y));
     if (hasy) g += dv.cy * wx * wz * ((nn.x - c.x) * (nn.x - c.x) + (nn.y - c.y) * (nn.y - c.y));
@@ -154,10 +178,13 @@ __global__ void __launch_bounds__(256) k_obs_partial(const __grid_constant__ Dev
       const int ipp = (ip + 1 == nx) ? 0 : ip + 1;
       (void)ipp;
       const float2 gx0 = cmulc(c, e);                                                // psi* U_x(j) psi(i+1,j)
-      const float2 gx1 = cmulc(cn, cmul(dv.Ux[jp], cne));                            // at row j+1 (its own U_x)
+      float2 gx1 = cmul(dv.Ux[jp], cne);                                             // at row j+1 (its own U_x)
+      if (yz && dv.bcx == 0 && i + 1 == nx) gx1 = cmulc(cmul(dv.Pj[jp], Pk), gx1);
+      gx1 = cmulc(cn, gx1);
       const float2 gy0 = cmulc(c, nn);                                               // psi* S+_y psi at (i,j)
       float2 ney = cne;
-      if (dv.bcy == 0 && j + 1 == ny) ney = cmulc(cmulc(Pk, dv.Pi[ip]), cne);        // jump at column i+1
+      if (yz) ney = cmul(dv.Uy[ip], cne);
+      else if (dv.bcy == 0 && j + 1 == ny) ney = cmulc(cmulc(Pk, dv.Pi[ip]), cne);   // jump at column i+1
       const float2 gy1 = cmulc(ce, ney);
       const float circ = atan2f(gx0.y, gx0.x) + atan2f(gy1.y, gy1.x) - atan2f(gx1.y, gx1.x) - atan2f(gy0.y, gy0.x);
       a3 += (double)rintf((circ + flux) / twopi);

@@ -40,7 +40,32 @@ template <int MODE> struct Cfg {
   static constexpr unsigned SMEM = HDR + NS * SB;
 };
 
-template <int MODE>
+// yz Landau gauge (Eq. 24b, 29b): U_x = exp(i h_x K) is uniform, U_y(i) and U_z(i) vary along x
+// (per-site constants uy, uz = both sites of a pair, already scaled by f c_y, f c_z)
+__device__ __forceinline__ void nsum_pair_yz(const float2 ux, const float4 &uy, const float4 &uz, const float4 &C,
+                                             const float2 &W, const float2 &E, const float4 &Nn, const float4 &Ss,
+                                             const float4 &T, const float4 &B, float2 &s0, float2 &s1) {
+  s0.x = fmaf(ux.x, C.z + W.x, s0.x);  s0.x = fmaf(-ux.y, C.w - W.y, s0.x);
+  s0.y = fmaf(ux.x, C.w + W.y, s0.y);  s0.y = fmaf(ux.y, C.z - W.x, s0.y);
+  s1.x = fmaf(ux.x, E.x + C.x, s1.x);  s1.x = fmaf(-ux.y, E.y - C.y, s1.x);
+  s1.y = fmaf(ux.x, E.y + C.y, s1.y);  s1.y = fmaf(ux.y, E.x - C.x, s1.y);
+  s0.x = fmaf(uy.x, Nn.x + Ss.x, s0.x);  s0.x = fmaf(-uy.y, Nn.y - Ss.y, s0.x);
+  s0.y = fmaf(uy.x, Nn.y + Ss.y, s0.y);  s0.y = fmaf(uy.y, Nn.x - Ss.x, s0.y);
+  s1.x = fmaf(uy.z, Nn.z + Ss.z, s1.x);  s1.x = fmaf(-uy.w, Nn.w - Ss.w, s1.x);
+  s1.y = fmaf(uy.z, Nn.w + Ss.w, s1.y);  s1.y = fmaf(uy.w, Nn.z - Ss.z, s1.y);
+  s0.x = fmaf(uz.x, T.x + B.x, s0.x);  s0.x = fmaf(-uz.y, T.y - B.y, s0.x);
+  s0.y = fmaf(uz.x, T.y + B.y, s0.y);  s0.y = fmaf(uz.y, T.x - B.x, s0.y);
+  s1.x = fmaf(uz.z, T.z + B.z, s1.x);  s1.x = fmaf(-uz.w, T.w - B.w, s1.x);
+  s1.y = fmaf(uz.z, T.w + B.w, s1.y);  s1.y = fmaf(uz.w, T.z - B.z, s1.y);
+}
+// both sites of v times the squares of their own link variables u = (u0, u1) (open faces: ghost = U^2 neighbour)
+__device__ __forceinline__ float4 sq_mul4(const float4 &u, const float4 &v, bool conj_) {
+  const float2 a = cmul(lo(u), lo(u)), b = cmul(hi(u), hi(u));
+  const float2 p = conj_ ? cmulc(a, lo(v)) : cmul(a, lo(v)), q = conj_ ? cmulc(b, hi(v)) : cmul(b, hi(v));
+  return make_float4(p.x, p.y, q.x, q.y);
+}
+
+template <int MODE, bool YZ>
 __global__ void __launch_bounds__(NTHREADS, 2) k_march_tma(const __grid_constant__ Dev dv,
                                                            const __grid_constant__ MarchMaps mm) {
   constexpr int NS = Cfg<MODE>::NS;
@@ -142,6 +167,16 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_march_tma(const __grid_constant
     L.uz = make_float2(f * dv.cz * Uz.x, f * dv.cz * Uz.y);
     L.cy = f * dv.cy;
   }
+  const int icA = min(iA, nx - 2), icB = min(iB, nx - 2);
+  float4 uyA, uyB, uzA, uzB;                                         // yz gauge: scaled U_y(i), U_z(i) of the four sites
+  if (YZ) {
+    const float sy = f * dv.cy, sz = f * dv.cz;
+    const float4 a = *reinterpret_cast<const float4 *>(dv.Uy + icA), b = *reinterpret_cast<const float4 *>(dv.Uy + icB);
+    const float4 c = *reinterpret_cast<const float4 *>(dv.Uzx + icA), d = *reinterpret_cast<const float4 *>(dv.Uzx + icB);
+    uyA = make_float4(sy * a.x, sy * a.y, sy * a.z, sy * a.w); uyB = make_float4(sy * b.x, sy * b.y, sy * b.z, sy * b.w);
+    uzA = make_float4(sz * c.x, sz * c.y, sz * c.z, sz * c.w); uzB = make_float4(sz * d.x, sz * d.y, sz * d.z, sz * d.w);
+  }
+  const bool xedge = px && (i0 == 0 || i0 + nv == nx);              // yz: the CTA touches the quasi-periodic seam in x
   unsigned nstep = 0;
   if (MODE == MODE_INIT) nstep = (unsigned)ctl->n;
   float rmax = 0.f;
@@ -221,7 +256,20 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_march_tma(const __grid_constant
     if (eB_h) EB = lds64(prv + oEB);
 
     float4 TA = TvA, TB = TvB, BA = BvA, BB = BvB;
-    if (ylo || yhi) {                                  // quasi-periodic jump in y, rows 0 and ny-1 only
+    if (YZ) {
+      if (xedge) {                                     // quasi-periodic jump in x: psi_{-1} = P_{j,k} psi_{nx-1}
+        const float2 P = cmul(dv.Pj[jc], dv.Pk[k]);
+        if (iA == 0) WA = cmul(P, WA);
+        if (iA + 1 == nx - 1) EA = cmulc(P, EA);       // psi_{nx} = P*_{j,k} psi_0
+        if (iB + 1 == nx - 1) EB = cmulc(P, EB);
+      }
+      if (!py && (j == 0 || j == ny - 1)) {            // open y faces with U_y != 1: ghost = U_y^2 neighbour
+        const float4 ua = *reinterpret_cast<const float4 *>(dv.Uy + icA), ub = *reinterpret_cast<const float4 *>(dv.Uy + icB);
+        if (j == 0) { SA = sq_mul4(ua, NA, false); SB_ = sq_mul4(ub, NB, false); }
+        else { NA = sq_mul4(ua, SA, true); NB = sq_mul4(ub, SB_, true); }
+      }
+    }
+    if (!YZ && (ylo || yhi)) {                         // quasi-periodic jump in y, rows 0 and ny-1 only
       const float2 Pk = dv.Pk[k];
       const float4 PiA = *reinterpret_cast<const float4 *>(dv.Pi + min(iA, nx - 2));
       const float4 PiB = *reinterpret_cast<const float4 *>(dv.Pi + min(iB, nx - 2));
@@ -246,16 +294,27 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_march_tma(const __grid_constant
       if (xhiB) EB = cmulc(U2, lo(CvB));
     }
     if (!pz && (k == 0 || k == nz - 1)) {              // open z faces, uniform over the CTA
-      const float2 Uz = dv.Uz[jc];
-      const float2 U2 = cmul(Uz, Uz);
-      if (k == 0) { BA = cmul4(U2, TA); BB = cmul4(U2, TB); }
-      else { TA = cmulc4(U2, BA); TB = cmulc4(U2, BB); }
+      if (YZ) {
+        const float4 ua = *reinterpret_cast<const float4 *>(dv.Uzx + icA), ub = *reinterpret_cast<const float4 *>(dv.Uzx + icB);
+        if (k == 0) { BA = sq_mul4(ua, TA, false); BB = sq_mul4(ub, TB, false); }
+        else { TA = sq_mul4(ua, BA, true); TB = sq_mul4(ub, BB, true); }
+      } else {
+        const float2 Uz = dv.Uz[jc];
+        const float2 U2 = cmul(Uz, Uz);
+        if (k == 0) { BA = cmul4(U2, TA); BB = cmul4(U2, TB); }
+        else { TA = cmulc4(U2, BA); TB = cmulc4(U2, BB); }
+      }
     }
 
     float2 sA0 = make_float2(0.f, 0.f), sA1 = sA0, sB0 = sA0, sB1 = sA0;
     if (MODE == MODE_SWEEP) { sA0 = lo(bA); sA1 = hi(bA); sB0 = lo(bB); sB1 = hi(bB); }
-    nsum_pair(L, CvA, WA, EA, NA, SA, TA, BA, sA0, sA1);
-    nsum_pair(L, CvB, WB, EB, NB, SB_, TB, BB, sB0, sB1);
+    if (YZ) {
+      nsum_pair_yz(L.ux, uyA, uzA, CvA, WA, EA, NA, SA, TA, BA, sA0, sA1);
+      nsum_pair_yz(L.ux, uyB, uzB, CvB, WB, EB, NB, SB_, TB, BB, sB0, sB1);
+    } else {
+      nsum_pair(L, CvA, WA, EA, NA, SA, TA, BA, sA0, sA1);
+      nsum_pair(L, CvB, WB, EB, NB, SB_, TB, BB, sB0, sB1);
+    }
 
     if (MODE == MODE_RHO) {
       // rho_m = sum_alpha c_alpha Im[psi*_m (S+ psi + S- psi)_m]
@@ -401,13 +460,17 @@ int march_tma_build_maps(const Dev &dv, MarchMaps *mm) {
   return rc;
 }
 
+template <int MODE, bool YZ> static cudaError_t cfg_one() {
+  return cudaFuncSetAttribute(k_march_tma<MODE, YZ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg<MODE>::SMEM);
+}
 cudaError_t march_tma_configure() {
-  cudaError_t e = cudaFuncSetAttribute(k_march_tma<MODE_SWEEP>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                       (int)Cfg<MODE_SWEEP>::SMEM);
-  if (e != cudaSuccess) return e;
-  e = cudaFuncSetAttribute(k_march_tma<MODE_INIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg<MODE_INIT>::SMEM);
-  if (e != cudaSuccess) return e;
-  return cudaFuncSetAttribute(k_march_tma<MODE_RHO>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg<MODE_RHO>::SMEM);
+  cudaError_t e;
+  if ((e = cfg_one<MODE_SWEEP, false>()) != cudaSuccess) return e;
+  if ((e = cfg_one<MODE_INIT, false>()) != cudaSuccess) return e;
+  if ((e = cfg_one<MODE_RHO, false>()) != cudaSuccess) return e;
+  if ((e = cfg_one<MODE_SWEEP, true>()) != cudaSuccess) return e;
+  if ((e = cfg_one<MODE_INIT, true>()) != cudaSuccess) return e;
+  return cfg_one<MODE_RHO, true>();
 }
 
 int march_tma_tile_w() { return TW; }
@@ -417,8 +480,12 @@ void march_tma_grid(int nx, int ny, int *gx, int *gy) {
   *gy = (ny + TH - 1) / TH;
 }
 
+template <bool YZ> static void launch_g(int mode, const Dev &dv, const MarchMaps &mm, dim3 grid, cudaStream_t st) {
+  if (mode == MODE_SWEEP) k_march_tma<MODE_SWEEP, YZ><<<grid, NTHREADS, Cfg<MODE_SWEEP>::SMEM, st>>>(dv, mm);
+  else if (mode == MODE_INIT) k_march_tma<MODE_INIT, YZ><<<grid, NTHREADS, Cfg<MODE_INIT>::SMEM, st>>>(dv, mm);
+  else k_march_tma<MODE_RHO, YZ><<<grid, NTHREADS, Cfg<MODE_RHO>::SMEM, st>>>(dv, mm);
+}
 void launch_march_tma(int mode, const Dev &dv, const MarchMaps &mm, dim3 grid, cudaStream_t st) {
-  if (mode == MODE_SWEEP) k_march_tma<MODE_SWEEP><<<grid, NTHREADS, Cfg<MODE_SWEEP>::SMEM, st>>>(dv, mm);
-  else if (mode == MODE_INIT) k_march_tma<MODE_INIT><<<grid, NTHREADS, Cfg<MODE_INIT>::SMEM, st>>>(dv, mm);
-  else k_march_tma<MODE_RHO><<<grid, NTHREADS, Cfg<MODE_RHO>::SMEM, st>>>(dv, mm);
+  if (dv.gauge_yz) launch_g<true>(mode, dv, mm, grid, st);
+  else launch_g<false>(mode, dv, mm, grid, st);
 }

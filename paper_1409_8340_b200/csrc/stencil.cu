@@ -21,7 +21,9 @@ __global__ void __launch_bounds__(256) k_jav_edges(const __grid_constant__ Dev d
     const int e = min(dv.nx, (t + 1) * tile_w) - 1;
     const int j = (int)(row % dv.ny);
     const float2 *xr = x + row * dv.nx;
-    const float2 a = xr[e], b = xr[e + 1 == dv.nx ? 0 : e + 1];
+    const float2 a = xr[e];
+    float2 b = xr[e + 1 == dv.nx ? 0 : e + 1];
+    if (dv.gauge_yz && e + 1 == dv.nx) b = cmulc(cmul(dv.Pj[j], dv.Pk[row / dv.ny]), b);   // psi_{nx} = P*_{j,k} psi_0
     const float2 ub = cmul(dv.Ux[j], b);
     acc += (double)(a.x * ub.y - a.y * ub.x);
   }
@@ -38,7 +40,7 @@ __global__ void __launch_bounds__(256) k_jav_edges(const __grid_constant__ Dev d
 
 // Per-row link variables from K (Eq. 27; gauge 24a):  U_x(j) = exp(i h_x (K + B_z ybar_j)).
 __device__ void write_Ux(const Dev &dv, double K, int tid, int nthreads) {
-  const double Bz = dv.ctl->Bz;
+  const double Bz = dv.gauge_yz ? 0.0 : dv.ctl->Bz;        // yz gauge: U_x = exp(i h_x K) on every row (Eq. 24b)
   for (int j = tid; j < dv.ny; j += nthreads) {
     const double ybar = j * dv.hy - 0.5 * dv.Ly;
     double s, c;

@@ -94,6 +94,7 @@ static bool params_ok(const tdgl_params *p) {
   if (!(p->eps_tol >= 0.f) || p->max_sweeps < 1 || p->max_sweeps > TDGL_MAX_RESID_SLOTS || p->fixed_sweeps < 0 ||
       p->fixed_sweeps > TDGL_MAX_RESID_SLOTS) return false;
   if (!(p->temperature >= 0.f)) return false;
+  if ((p->flags & TDGL_FLAG_GAUGE_YZ) && p->nz == 1) return false;          // films use the xz gauge
   return true;
 }
 
@@ -108,6 +109,9 @@ static size_t carve(const tdgl_params *p, char *base, Dev *dv) {
   q = take(p->ny * sizeof(float2)); if (dv) dv->Uz = (float2 *)q;
   q = take(p->nx * sizeof(float2)); if (dv) dv->Pi = (float2 *)q;
   q = take(p->nz * sizeof(float2)); if (dv) dv->Pk = (float2 *)q;
+  q = take(p->nx * sizeof(float2)); if (dv) dv->Uy = (float2 *)q;
+  q = take(p->nx * sizeof(float2)); if (dv) dv->Uzx = (float2 *)q;
+  q = take(p->ny * sizeof(float2)); if (dv) dv->Pj = (float2 *)q;
   const int ns[3] = {p->nx, p->ny, p->nz};
   for (int a = 0; a < 3; ++a) {
     q = take(ns[a] * sizeof(float)); if (dv) dv->lam[a] = (float *)q;
@@ -246,6 +250,7 @@ extern "C" int tdgl_create(const tdgl_params *p, tdgl_t **out) {
   dv.seed_lo = (unsigned)(p->seed & 0xffffffffull);
   dv.seed_hi = (unsigned)(p->seed >> 32);
   dv.solve_mu = (p->flags & TDGL_FLAG_SOLVE_MU) ? 1 : 0;
+  dv.gauge_yz = (p->flags & TDGL_FLAG_GAUGE_YZ) ? 1 : 0;
 
   {
     unsigned gx, gy, gz; int zc;
@@ -333,18 +338,24 @@ extern "C" int tdgl_set_pinning(tdgl_t *h, const tdgl_sphere *sph, int64_t n, fl
 
 extern "C" int tdgl_set_field_current(tdgl_t *h, float Bx, float By, float Bz, float Jx) {
   if (!h) return TDGL_EINVAL;
-  if (By != 0.f) return TDGL_EINCOMPAT;
+  const bool yz = h->dv.gauge_yz != 0;
+  if ((!yz && By != 0.f) || (yz && Bx != 0.f)) return TDGL_EINCOMPAT;   // one Landau gauge per field plane
   if (h->film && Bx != 0.f) return TDGL_EINCOMPAT;           // a film has no z links for B_x to act on
   if (Jx != 0.f && h->dv.bcx == 1) return TDGL_EINCOMPAT;
-  double bx = Bx, bz = Bz;
+  double bx = yz ? By : Bx, bz = Bz;                         // bx: the in-plane component (B_x or B_y)
   const double twopi = 2.0 * 3.14159265358979323846;
   if (h->dv.bcx == 0 && h->dv.bcy == 0) {
     const double a = h->dv.Lx * h->dv.Ly;
     const double q = std::nearbyint(bz * a / twopi);
     bz = twopi * q / a;
   }
-  if (h->dv.bcy == 0 && h->dv.bcz == 0) {
+  if (!yz && h->dv.bcy == 0 && h->dv.bcz == 0) {
     const double a = h->dv.Ly * h->dv.Lz;
+    const double q = std::nearbyint(bx * a / twopi);
+    bx = twopi * q / a;
+  }
+  if (yz && h->dv.bcx == 0 && h->dv.bcz == 0) {  // B_y = 2 pi n/(L_x L_z): continuity of P_{j,k} in z
+    const double a = h->dv.Lx * h->dv.Lz;
     const double q = std::nearbyint(bx * a / twopi);
     bx = twopi * q / a;
   }

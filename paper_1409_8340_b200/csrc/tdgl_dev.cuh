@@ -55,6 +55,10 @@ struct Dev {
   float *mu, *eps, *scratch;
   float2 *Ux, *Uz;          // per-row link variables U_x(j), U_z(j)  (Eq. 27)
   float2 *Pi, *Pk;          // quasi-periodic jump P_{i,k} = Pi[i] conj(Pk[k])
+  // yz Landau gauge (Eq. 24b, 29b): U_x = exp(i h_x K) for every row (Ux[] holds it), per-column
+  // link variables U_y(i), U_z(i), jump in x  P_{j,k} = Pj[j] Pk[k]
+  int gauge_yz;
+  float2 *Uy, *Uzx, *Pj;
   float *lam[3];            // eigenvalues of the 1-D operators per axis
   float2 *tw[3];            // FFT twiddles exp(-2 pi i m/n) per axis (power-of-two periodic axes)
   double *tab[3];           // generic transform tables: cas(2 pi m/n) or cos(pi m/(n-1))
