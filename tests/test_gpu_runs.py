@@ -132,3 +132,31 @@ def test_replicas_of_large_configs(name, shape, nsteps):
 def test_smoke_entry():
     import __graft_entry__
     __graft_entry__.smoke()
+
+
+def test_C3_current_sweep_iv_replica():
+    """C3's protocol (BASELINE.json configs[2]) on a replica: tdgl_set_field_current between legs of a current
+    sweep, E_x averaged over each leg (tdgl_obs.Ex_mean restarts at every call: the I-V curve),
+    against the oracle driven the same way; noise off for the pointwise gate."""
+    cfg = I.CONFIGS["C3"].scaled(64, 64, 32)
+    p, st, eps, (Bx, Bz), s = setup_pair(cfg, temperature=0.0)
+    bx_req, bz_req = cfg.requested_field()
+    legs, nsteps = I.C3_CURRENTS[:3], 25
+    done = 0
+    for J in legs:
+        s.set_field_current(Bx=bx_req, Bz=bz_req, Jx=J)
+        s.step(nsteps)
+        counts, _ = s.sweep_log(nsteps)
+        ex = []
+        for n in range(nsteps):
+            O.step(p, st, eps, Bx, Bz, f32(J), fixed_sweeps=int(counts[n]))
+            ex.append(st.Ex)
+        done += nsteps
+        ob = s.observables()
+        assert ob.steps == done
+        assert abs(ob.Ex_mean - float(np.mean(ex))) < 1e-7               # mean over this leg only
+        assert abs(ob.Ex - st.Ex) < 1e-7 and abs(ob.K - st.K) < 1e-6
+    psi, mu = s.get_psi_mu()
+    assert np.max(np.abs(psi.cpu().numpy() - st.psi)) <= 1e-4
+    assert rel_l2(psi.cpu().numpy(), st.psi) <= 1e-5
+    s.close()
