@@ -156,13 +156,14 @@ class Solver:
     def __init__(self, nx: int, ny: int, nz: int, bc: Sequence[int] = (0, 0, 0), h: float = 0.5, dt: float = 0.1,
                  u: float = 1.0, g: float = 1.0, eps_tol: float = 1e-6, max_sweeps: int = 100, fixed_sweeps: int = 0,
                  temperature: float = 0.0, seed: int = 0, init_amp: float = 0.01, solve_mu: bool = True,
-                 host_loop: bool = False, hxyz: Optional[Sequence[float]] = None, device: str = "cuda:0",
+                 host_loop: bool = False, hxyz: Optional[Sequence[float]] = None, device: Optional[str] = None,
                  gauge_yz: bool = False):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1409_8340_b200 needs a CUDA device (sm_100a); there is no CPU path")
         self.torch = torch
-        self.device = torch.device(device)
+        # the CURRENT device unless one is named (one process per GPU: bench.py sets it from LOCAL_RANK)
+        self.device = torch.device(device) if device is not None else torch.device("cuda", torch.cuda.current_device())
         torch.cuda.set_device(self.device)
         hx, hy, hz = (hxyz if hxyz is not None else (h, h, h))
         p = TdglParams()

@@ -57,3 +57,16 @@ def test_replica_seeds_differ_per_rank():
     import bench
     src = inspect.getsource(bench.main)
     assert "seed_offset=rank" in src
+
+
+def test_solver_binds_to_the_current_device_not_to_cuda0():
+    """One process per GPU: bench.py calls torch.cuda.set_device(LOCAL_RANK) and the Solver must allocate there."""
+    import inspect
+    from paper_1409_8340_b200.binding import Solver
+    sig = inspect.signature(Solver.__init__)
+    assert sig.parameters["device"].default is None
+    src = inspect.getsource(Solver.__init__)
+    assert "current_device()" in src
+    sys.path.insert(0, ROOT)
+    import bench
+    assert "torch.cuda.set_device(local_rank)" in inspect.getsource(bench.main)
