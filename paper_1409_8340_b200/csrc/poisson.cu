@@ -361,6 +361,9 @@ void launch_dct_s(float *data, int n, int LB, long long stride, long long ostrid
 bool dht_fast_supported(int n);
 cudaError_t dht_fast_configure(int n);
 void launch_dht_x_fast(float *data, int n, long long nrows, const float2 *tw, cudaStream_t st);
+// persistent radix-8^3 kernel for n = 512 (fft_r8.cu)
+cudaError_t dht_x_512_configure();
+void launch_dht_x_512(float *data, long long nrows, const float2 *tw, cudaStream_t st);
 void launch_dht_s_fast(float *data, int n, long long stride, long long ostride, int ncolc, int nother, const float2 *tw,
                        int divide, float scale, const float *lx, const float *ly, const float *lz, cudaStream_t st);
 
@@ -397,6 +400,7 @@ cudaError_t poisson_configure(int nx, int ny, int nz) {
     for (int kind = 0; kind < 2; ++kind) { size_t s = smem_generic(n, kind, tl_generic(n)); if (s > c) c = s; }
   }
   cudaError_t e;
+  if (nx == 512 && (e = dht_x_512_configure()) != cudaSuccess) return e;
   for (int ax = 0; ax < 3; ++ax)
     if (dht_fast_supported(ns[ax]) && (e = dht_fast_configure(ns[ax])) != cudaSuccess) return e;
   if (a && (e = cudaFuncSetAttribute(k_dht_x, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)a)) != cudaSuccess) return e;
@@ -424,7 +428,8 @@ static int transform_axis(const Dev &dv, float *data, int axis, bool divide, flo
   }
   if (!open && dht_fast_supported(n)) {
     if (axis == 0) {
-      launch_dht_x_fast(data, n, (long long)dv.ny * dv.nz, dv.tw[0], st);
+      if (n == 512) launch_dht_x_512(data, (long long)dv.ny * dv.nz, dv.tw[0], st);
+      else launch_dht_x_fast(data, n, (long long)dv.ny * dv.nz, dv.tw[0], st);
     } else {
       launch_dht_s_fast(data, n, axis == 1 ? dv.nx : plane, axis == 1 ? plane : dv.nx, dv.nx / 2,
                         axis == 1 ? dv.nz : dv.ny, dv.tw[axis], divide ? 1 : 0, scale, dv.lam[0], dv.lam[1], dv.lam[2], st);
