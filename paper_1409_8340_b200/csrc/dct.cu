@@ -58,7 +58,7 @@ __device__ __forceinline__ void bluestein_core(float2 *v, float2 *sm, const floa
 
 // x pass: contiguous rows, two rows per complex sequence
 template <int LB>
-__global__ void __launch_bounds__((LB / 8 > 256) ? LB / 8 : 256)
+__global__ void __launch_bounds__((LB / 8 > 256) ? LB / 8 : 256, (LB >= 2048) ? 2 : 1)
 k_dct_x(float *__restrict__ data, int n, long long nrows, const float2 *__restrict__ twg,
         const float2 *__restrict__ Cg, const float2 *__restrict__ Hg) {
   constexpr int TPF = LB / 8, F = (TPF >= 256) ? 1 : 256 / TPF, NT = F * TPF;
