@@ -97,6 +97,47 @@ k_dct_x(float *__restrict__ data, int n, long long nrows, const float2 *__restri
   }
 }
 
+// x pass for the long transforms (LB >= 2048): CC row pairs per CTA in the [p][f] layout of the strided pass, which
+// ncu shows free of bank conflicts, whereas the one-pair-per-CTA layout above had 34 % conflict wavefronts
+template <int LB, int CC>
+__global__ void __launch_bounds__(CC *LB / 8)
+k_dct_x2(float *__restrict__ data, int n, long long nrows, const float2 *__restrict__ twg,
+         const float2 *__restrict__ Cg, const float2 *__restrict__ Hg) {
+  constexpr int TPF = LB / 8, NT = CC * TPF;
+  extern __shared__ float4 smem4[];
+  float2 *tw = reinterpret_cast<float2 *>(smem4);
+  float2 *sm = tw + LB;
+  const int tid = threadIdx.x;
+  fill_twiddles<LB>(tw, twg, tid, NT);
+  const int f = tid % CC, j = tid / CC;
+  const int M = 2 * (n - 1);
+  const long long ra = 2 * ((long long)blockIdx.x * CC + f), rb = ra + 1;
+  const bool va = ra < nrows, vb = rb < nrows;
+  float *A = data + ra * n, *B = data + rb * n;
+  float2 v[8];
+#pragma unroll
+  for (int r = 0; r < 8; ++r) {
+    const int m = j + r * TPF;
+    float2 a = make_float2(0.f, 0.f);
+    if (m < M) {
+      const int p = (m < n) ? m : M - m;
+      a = cmulc(Cg[m], make_float2(va ? A[p] : 0.f, vb ? B[p] : 0.f));
+    }
+    v[r] = a;
+  }
+  bluestein_core<LB, false, CC>(v, sm, tw, Hg, j, f);
+  const float inv = 1.f / (float)LB;
+#pragma unroll
+  for (int r = 0; r < 8; ++r) {
+    const int q = j + r * TPF;
+    if (q < n) {
+      const float2 w = cmul(Cg[q], sm[saddr<LB, false, CC>(f, q)]);
+      if (va) A[q] = w.x * inv;
+      if (vb) B[q] = -w.y * inv;
+    }
+  }
+}
+
 // y / z pass: float2 columns (columns 2c, 2c+1 = re, im), CC columns per CTA
 template <int LB, int CC>
 __global__ void __launch_bounds__(CC *LB / 8)
@@ -157,6 +198,8 @@ template <int LB> struct DctCfg {
 template <int LB> static cudaError_t cfg_dct() {
   cudaError_t e = cudaFuncSetAttribute(k_dct_x<LB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)DctCfg<LB>::smem_x());
   if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(k_dct_x2<LB, DctCfg<LB>::CC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)DctCfg<LB>::smem_s());
+  if (e != cudaSuccess) return e;
   return cudaFuncSetAttribute(k_dct_s<LB, DctCfg<LB>::CC>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                               (int)DctCfg<LB>::smem_s());
 }
@@ -176,6 +219,11 @@ template <int LB>
 static void run_dct_x(float *data, int n, long long nrows, const float2 *T, const float2 *C, const float2 *H, cudaStream_t st) {
   constexpr int F = DctCfg<LB>::F;
   const long long npairs = (nrows + 1) / 2;
+  if (LB >= 2048) {
+    constexpr int CC = DctCfg<LB>::CC;
+    k_dct_x2<LB, CC><<<(unsigned)((npairs + CC - 1) / CC), CC * LB / 8, DctCfg<LB>::smem_s(), st>>>(data, n, nrows, T, C, H);
+    return;
+  }
   k_dct_x<LB><<<(unsigned)((npairs + F - 1) / F), F * (LB / 8), DctCfg<LB>::smem_x(), st>>>(data, n, nrows, T, C, H);
 }
 template <int LB>
