@@ -39,9 +39,15 @@ template <> __device__ __forceinline__ void dft<8>(float2 *v) {
   v[3] = cadd(e[3], o3);   v[7] = csub(e[3], o3);
 }
 
-// shared-memory address of element p of line f
-template <int N, bool XPASS, int CC> __device__ __forceinline__ int saddr(int f, int p) {
-  return XPASS ? f * (N + N / 8) + p + (p >> 3) : (CC < 8 ? (p + (p >> 3)) * CC + f : p * CC + f);
+// shared-memory address of element p of line f.  x pass (one line per 64+ consecutive threads): p + LAY (p >> 4).
+// Padding by whole groups of 16 keeps the stride-1 accesses of every stage (16 consecutive p per half-warp)
+// conflict free; the strided writes need LAY = 1 after the first stage (p = 8 jj + r) and LAY = 2 after the later
+// ones (p = 64 (jj >> 3) + (jj & 7) + 8 r), so each exchange has its own layout (every stage reads all, syncs, writes
+// all).  The result of a transform is in the LAY = 2 layout.  [ncu: the former p + (p >> 3) padding made every
+// stride-1 read of 16 lanes straddle two pad groups: 37 % of the shared wavefronts of the x pass were conflicts.]
+template <int N, bool XPASS, int CC, int LAY = 2> __device__ __forceinline__ int saddr(int f, int p) {
+  return (XPASS || CC == 1) ? f * (N + N / 8) + p + LAY * (p >> 4)      // (one column pair per CTA: same situation)
+                            : (CC < 8 ? (p + (p >> 3)) * CC + f : p * CC + f);
 }
 // elements of the shared work buffer of a y/z pass (fewer than 8 columns per CTA: rows padded 9/8 like the x pass,
 // otherwise the stride-8 accesses of the radix-8 stages fall into a few banks)
@@ -74,7 +80,7 @@ __device__ __forceinline__ void stage(float2 *v, float2 *sm, const float2 *tw, i
     for (int t = 0; t < T; ++t) {
       const int jj = j + t * (N / 8);
 #pragma unroll
-      for (int r = 0; r < R; ++r) v[t * R + r] = sm[saddr<N, XPASS, CC>(f, jj + r * NB)];
+      for (int r = 0; r < R; ++r) v[t * R + r] = sm[saddr<N, XPASS, CC, (NS == 8) ? 1 : 2>(f, jj + r * NB)];
     }
     __syncthreads();
   }
@@ -89,7 +95,7 @@ __device__ __forceinline__ void stage(float2 *v, float2 *sm, const float2 *tw, i
     dft<R>(v + t * R);
     const int base = (jj - k) * R + k;
 #pragma unroll
-    for (int r = 0; r < R; ++r) sm[saddr<N, XPASS, CC>(f, base + r * NS)] = v[t * R + r];
+    for (int r = 0; r < R; ++r) sm[saddr<N, XPASS, CC, (NS == 1) ? 1 : 2>(f, base + r * NS)] = v[t * R + r];
   }
   __syncthreads();
 }
