@@ -80,7 +80,11 @@ static void march_geometry(const tdgl_params *p, unsigned *gx, unsigned *gy, uns
   int a, b;
   march_tma_grid(p->nx, p->ny, &a, &b);
   int zc = p->nz;
-  while (zc > 8 && (long long)a * b * ((p->nz + zc - 1) / zc) < want) zc = (zc + 1) / 2;
+  // chunks of >= 32 planes while that still gives ~4 waves (each chunk re-reads two planes and pays a prologue);
+  // shorter chunks only to put at least one CTA on every SM (measured on C3: 32 planes 0.584 ms/step, 8 planes 0.616)
+  auto ctas = [&](int z) { return (long long)a * b * ((p->nz + z - 1) / z); };
+  while (zc > 32 && ctas(zc) < want) zc = (zc + 1) / 2;
+  while (zc > 8 && ctas(zc) < 148) zc = (zc + 1) / 2;
   *gx = (unsigned)a; *gy = (unsigned)b; *gz = (unsigned)((p->nz + zc - 1) / zc); *zc_out = zc;
 }
 
