@@ -180,7 +180,7 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_march_tma(const __grid_constant
   unsigned nstep = 0;
   if (MODE == MODE_INIT) nstep = (unsigned)ctl->n;
   float rmax = 0.f;
-  // J_av (Eq. 35): x links of the NEW iterate that lie inside this tile row (stencil.cu, k_jav_edges
+  // J_av (Eq. 35): x links of the NEW iterate that lie inside this tile row (step_ctl.cu, k_jav_edges
   // adds the links that cross a tile edge); only with x periodic and the mu / K part active
   const bool jact = (MODE != MODE_RHO) && dv.solve_mu && px;
   const float2 Uraw = dv.Ux[jc];
