@@ -138,56 +138,79 @@ __global__ void k_noise(const __grid_constant__ Dev dv, long long step, float2 *
 // Free energy and winding definitions: DESIGN.md "Observables" (the paper only names F_GL).
 __device__ __forceinline__ float face_w(int idx, int n, int open) { return (open && (idx == 0 || idx == n - 1)) ? 0.5f : 1.f; }
 
+// A CTA takes blocks of OBS_RB consecutive rows of one plane; a thread walks down the rows of its column, so that
+// psi(i, j+1), psi(i+1, j+1) and the x-link phase of row j+1 are carried into the next row (one row of loads and
+// one atan2 instead of two), the y-link phase of column i+1 comes from the neighbouring lane, and no per-site
+// 64-bit division is needed.  Same expressions as before: the windings are bit-identical.
+#define OBS_RB 8
 __global__ void __launch_bounds__(256) k_obs_partial(const __grid_constant__ Dev dv) {
   const float2 *__restrict__ x = dv.psi[dv.ctl->xbuf];
   const int nx = dv.nx, ny = dv.ny, nz = dv.nz;
   const float twopi = 6.283185307179586f;
   const float flux = (float)(dv.ctl->Bz * dv.hx * dv.hy);
+  const bool yz = dv.gauge_yz != 0;
+  const bool xjump = yz && dv.bcx == 0, yjump = !yz && dv.bcy == 0;
+  const int lane = threadIdx.x & 31;
+  const int nrb = (ny + OBS_RB - 1) / OBS_RB;
+  const long long nblk = (long long)nrb * nz;
+  const int nxpad = (nx + 31) & ~31;                       // whole warps iterate together (shuffles)
   double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
-  for (long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x; m < dv.N; m += (long long)gridDim.x * blockDim.x) {
-    const int i = (int)(m % nx);
-    const long long row = m / nx;
-    const int j = (int)(row % ny), k = (int)(row / ny);
-    const float2 c = x[m];
-    const float wx = face_w(i, nx, dv.bcx), wy = face_w(j, ny, dv.bcy), wz = face_w(k, nz, dv.bcz);
-    const float ab = c.x * c.x + c.y * c.y;
-    a0 += ab;
-    a1 += (double)(wx * wy * wz * (-dv.eps[m] * ab + 0.5f * ab * ab));
-    const int ip = (i + 1 == nx) ? 0 : i + 1, jp = (j + 1 == ny) ? 0 : j + 1, kp = (k + 1 == nz) ? 0 : k + 1;
-    const bool hasx = dv.bcx == 0 || i + 1 < nx, hasy = dv.bcy == 0 || j + 1 < ny, hasz = dv.bcz == 0 || k + 1 < nz;
-    const long long base = (long long)nx * ((long long)ny * k);
+  for (long long blk = blockIdx.x; blk < nblk; blk += gridDim.x) {
+    const int k = (int)(blk / nrb), jb = (int)(blk - (long long)k * nrb) * OBS_RB, je = min(ny, jb + OBS_RB);
+    const int kp = (k + 1 == nz) ? 0 : k + 1;
+    const bool hasz = dv.bcz == 0 || k + 1 < nz;
+    const float wz = face_w(k, nz, dv.bcz);
     const float2 Pk = dv.Pk[k];
-    // forward neighbours with their link variables
-    const bool yz = dv.gauge_yz != 0;
-    float2 e = cmul(dv.Ux[j], x[base + (long long)nx * j + ip]);
-    if (yz && dv.bcx == 0 && i + 1 == nx) e = cmulc(cmul(dv.Pj[j], Pk), e);       // yz: conj(P_{j,k}) psi_{0,j,k}
-    float2 nn = x[base + (long long)nx * jp + i];
-    if (yz) nn = cmul(dv.Uy[i], nn);
-    else if (dv.bcy == 0 && j + 1 == ny) nn = cmulc(cmulc(Pk, dv.Pi[i]), nn);     // xz: conj(P_{i,k}) psi_{i,0,k}
-    const float2 t = cmul(yz ? dv.Uzx[i] : dv.Uz[j], x[(long long)nx * ((long long)ny * kp + j) + i]);
-    float g = 0.f;
-    if (hasx) g += dv.cx * wy * wz * ((e.x - c.x) * (e.x - c.x) + (e.y - c.y) * (e.y - c.y));
-    if (hasy) g += dv.cy * wx * wz * ((nn.x - c.x) * (nn.x - c.x) + (nn.y - c.y) * (nn.y - c.y));
-    if (hasz) g += dv.cz * wx * wy * ((t.x - c.x) * (t.x - c.x) + (t.y - c.y) * (t.y - c.y));
-    a2 += (double)g;
-    if (hasx && hasy) {
-      // winding of the z-plaquette with corner (i, j):  g_x(i,j) + g_y(i+1,j) - g_x(i,j+1) - g_y(i,j) + B_z h_x h_y
-      const float2 ce = x[base + (long long)nx * j + ip];                            // psi(i+1, j)
-      const float2 cn = x[base + (long long)nx * jp + i];                            // psi(i, j+1)
-      float2 cne = x[base + (long long)nx * jp + ip];                                // psi(i+1, j+1)
-      const int ipp = (ip + 1 == nx) ? 0 : ip + 1;
-      (void)ipp;
-      const float2 gx0 = cmulc(c, e);                                                // psi* U_x(j) psi(i+1,j)
-      float2 gx1 = cmul(dv.Ux[jp], cne);                                             // at row j+1 (its own U_x)
-      if (yz && dv.bcx == 0 && i + 1 == nx) gx1 = cmulc(cmul(dv.Pj[jp], Pk), gx1);
-      gx1 = cmulc(cn, gx1);
-      const float2 gy0 = cmulc(c, nn);                                               // psi* S+_y psi at (i,j)
-      float2 ney = cne;
-      if (yz) ney = cmul(dv.Uy[ip], cne);
-      else if (dv.bcy == 0 && j + 1 == ny) ney = cmulc(cmulc(Pk, dv.Pi[ip]), cne);   // jump at column i+1
-      const float2 gy1 = cmulc(ce, ney);
-      const float circ = atan2f(gx0.y, gx0.x) + atan2f(gy1.y, gy1.x) - atan2f(gx1.y, gx1.x) - atan2f(gy0.y, gy0.x);
-      a3 += (double)rintf((circ + flux) / twopi);
+    const float2 *pk = x + (long long)nx * ny * k, *pkp = x + (long long)nx * ny * kp;
+    const float *ek = dv.eps + (long long)nx * ny * k;
+    for (int i0 = threadIdx.x; i0 < nxpad; i0 += 256) {
+      const bool act = i0 < nx;
+      const int i = act ? i0 : nx - 1;
+      const int ip = (i + 1 == nx) ? 0 : i + 1;
+      const bool hasx = dv.bcx == 0 || i + 1 < nx, wrapx = i + 1 == nx;
+      const float wx = face_w(i, nx, dv.bcx);
+      // x link of row j: psi*(i,j) U_x(j) psi(i+1,j) (times conj P_{j,k} on the yz-gauge seam)
+      auto xlink = [&](int j, float2 cc, float2 ee) -> float2 {
+        float2 e = cmul(dv.Ux[j], ee);
+        if (xjump && wrapx) e = cmulc(cmul(dv.Pj[j], Pk), e);
+        return e;
+      };
+      auto ylink = [&](int col, int j, float2 v) -> float2 {          // S+_y psi at column col, row j
+        if (yz) return cmul(dv.Uy[col], v);
+        if (yjump && j + 1 == ny) return cmulc(cmulc(Pk, dv.Pi[col]), v);
+        return v;
+      };
+      float2 c = pk[(long long)nx * jb + i], er = pk[(long long)nx * jb + ip];
+      float2 e = xlink(jb, c, er);
+      float gx0;
+      { const float2 g = cmulc(c, e); gx0 = atan2f(g.y, g.x); }
+      for (int j = jb; j < je; ++j) {
+        const int jp = (j + 1 == ny) ? 0 : j + 1;
+        const bool hasy = dv.bcy == 0 || j + 1 < ny;
+        const float wy = face_w(j, ny, dv.bcy);
+        const float2 nr = pk[(long long)nx * jp + i], ner = pk[(long long)nx * jp + ip];
+        const float2 t = cmul(yz ? dv.Uzx[i] : dv.Uz[j], pkp[(long long)nx * j + i]);
+        const float2 nn = ylink(i, j, nr);
+        const float ab = c.x * c.x + c.y * c.y;
+        float g = 0.f;
+        if (hasx) g += dv.cx * wy * wz * ((e.x - c.x) * (e.x - c.x) + (e.y - c.y) * (e.y - c.y));
+        if (hasy) g += dv.cy * wx * wz * ((nn.x - c.x) * (nn.x - c.x) + (nn.y - c.y) * (nn.y - c.y));
+        if (hasz) g += dv.cz * wx * wy * ((t.x - c.x) * (t.x - c.x) + (t.y - c.y) * (t.y - c.y));
+        // winding of the z-plaquette with corner (i, j):  g_x(i,j) + g_y(i+1,j) - g_x(i,j+1) - g_y(i,j) + B_z h_x h_y
+        const float2 en = xlink(jp, nr, ner);                           // row j+1
+        float gx1, gy0, gy1;
+        { const float2 q = cmulc(nr, en); gx1 = atan2f(q.y, q.x); }
+        { const float2 q = cmulc(c, nn); gy0 = atan2f(q.y, q.x); }
+        gy1 = __shfl_down_sync(0xffffffffu, gy0, 1);
+        if (lane == 31 || wrapx) { const float2 q = cmulc(er, ylink(ip, j, ner)); gy1 = atan2f(q.y, q.x); }
+        if (act) {
+          a0 += ab;
+          a1 += (double)(wx * wy * wz * (-ek[(long long)nx * j + i] * ab + 0.5f * ab * ab));
+          a2 += (double)g;
+          if (hasx && hasy) a3 += (double)rintf((gx0 + gy1 - gx1 - gy0 + flux) / twopi);
+        }
+        c = nr; er = ner; e = en; gx0 = gx1;
+      }
     }
   }
   __shared__ double sh[4][8];
@@ -244,7 +267,8 @@ void launch_spheres(const Dev &dv, const float4 *sph, long long n, float eps_in,
 }
 void launch_noise(const Dev &dv, long long step, float2 *out, cudaStream_t st) { k_noise<<<grid_for(dv.N, 256, 148 * 16), 256, 0, st>>>(dv, step, out); }
 int launch_obs(const Dev &dv, cudaStream_t st) {
-  const int nb = (int)grid_for(dv.N, 256, TDGL_NPART);
+  const long long nblk = (long long)((dv.ny + OBS_RB - 1) / OBS_RB) * dv.nz;
+  const int nb = (int)(nblk < TDGL_NPART ? nblk : TDGL_NPART);
   k_obs_partial<<<nb, 256, 0, st>>>(dv);
   k_obs_final<<<1, 256, 0, st>>>(dv, nb);
   return 2;
