@@ -215,6 +215,11 @@ static int build_graph(tdgl_t *h) {
   return TDGL_OK;
 }
 
+// inside tdgl_create a failing CUDA call releases the half-built handle (pinned flag word, events, graph objects)
+#define CKC(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { tdgl_destroy(h); return TDGL_ECUDA; } } while (0)
+#define CKCL() do { cudaError_t e_ = cudaGetLastError(); if (e_ != cudaSuccess) { tdgl_destroy(h); return TDGL_ECUDA; } } while (0)
+extern "C" int tdgl_destroy(tdgl_t *h);
+
 extern "C" int tdgl_create(const tdgl_params *p, tdgl_t **out) {
   if (!out) return TDGL_EINVAL;
   *out = nullptr;
@@ -265,16 +270,16 @@ extern "C" int tdgl_create(const tdgl_params *p, tdgl_t **out) {
   h->jav_blocks = jav_edge_blocks(dv, march_tma_tile_w());
   h->pred_sweeps = 1;
   if (film) {
-    CK(march_film_configure());
+    CKC(march_film_configure());
   } else {
-    CK(march_tma_configure());
-    if (march_tma_build_maps(dv, &h->maps) != 0) { h->last_cuda = (int)cudaErrorNotSupported; delete h; return TDGL_ECUDA; }
+    CKC(march_tma_configure());
+    if (march_tma_build_maps(dv, &h->maps) != 0) { tdgl_destroy(h); return TDGL_ECUDA; }
   }
-  if (film) CK(poisson_configure(p->nx, 1, p->ny));
-  else CK(poisson_configure(p->nx, p->ny, p->nz));
-  CK(cudaMallocHost((void **)&h->h_flag, 64));
-  CK(cudaEventCreate(&h->ev0));
-  CK(cudaEventCreate(&h->ev1));
+  if (film) CKC(poisson_configure(p->nx, 1, p->ny));
+  else CKC(poisson_configure(p->nx, p->ny, p->nz));
+  CKC(cudaMallocHost((void **)&h->h_flag, 64));
+  CKC(cudaEventCreate(&h->ev0));
+  CKC(cudaEventCreate(&h->ev1));
 
   cudaStream_t st = h->stream;
   launch_ctl_reset(dv, p->eps_tol, p->max_sweeps, p->fixed_sweeps, st);
@@ -284,7 +289,7 @@ extern "C" int tdgl_create(const tdgl_params *p, tdgl_t **out) {
   for (int a = 0; a < 3; ++a) {
     dv.bLB[a] = (bcs[a] == TDGL_BC_OPEN) ? dct_fast_lb(ns[a]) : 0;
     if (dv.bLB[a]) {
-      CK(dct_fast_configure(dv.bLB[a]));
+      CKC(dct_fast_configure(dv.bLB[a]));
       launch_build_bluestein(dv.bT[a], dv.bC[a], dv.bH[a], ns[a], dv.bLB[a], st);
       h->launches += 1;
     }
@@ -303,11 +308,11 @@ extern "C" int tdgl_create(const tdgl_params *p, tdgl_t **out) {
   launch_set_field(dv, 0.0, 0.0, 0.0, st);
   launch_step_begin(dv, st);
   h->launches += 7;
-  CKL();
+  CKCL();
   h->use_graph = !(p->flags & TDGL_FLAG_HOST_LOOP);
   if (h->use_graph) {
     int rc = build_graph(h);
-    if (rc != TDGL_OK) { int lc = h->last_cuda; tdgl_destroy(h); (void)lc; return rc; }
+    if (rc != TDGL_OK) { tdgl_destroy(h); return rc; }
   }
   *out = h;
   return TDGL_OK;
