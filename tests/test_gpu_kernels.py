@@ -311,3 +311,42 @@ def test_degenerate_sizes(shape, bc):
     assert np.max(np.abs(mu.cpu().numpy() - st.mu)) < 2e-5 * max(1.0, np.max(np.abs(st.mu)))
     assert abs(s.observables().K - st.K) < 1e-7
     s.close()
+
+
+# ---------------------------------------------------------------------------------------------------
+# parameters away from the defaults: anisotropic mesh, anisotropy g, relaxation constant u (S1)
+# ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("bc,nz", [((P_, P_, O_), 12), ((O_, P_, P_), 9), ((P_, O_, P_), 1)])
+def test_anisotropic_mesh_g_and_u(bc, nz):
+    cfg = cfg_of(40, 18, nz, bc, Bz=0.25, Bx=0.05 if nz > 1 else 0.0, Jx=0.02 if bc[0] == P_ else 0.0, temperature=1e-3,
+                 incl_fraction=0.1, incl_rmin=1.0, incl_rmax=2.0, seed=9)
+    psi0, mu0 = I.random_state(cfg, seed=4, amp=0.8)
+    kw = dict(hxyz=(0.5, 0.4, 0.6), g=1.3, u=1.7)
+    p, st, eps, (Bx, Bz), s = setup_pair(cfg, psi0=psi0, mu0=mu0, K0=0.1 if bc[0] == P_ else 0.0, fixed_sweeps=5, **kw)
+    s.step(2)
+    psi, mu = s.get_psi_mu()
+    for _ in range(2):
+        O.step(p, st, eps, Bx, Bz, f32(cfg.Jx), fixed_sweeps=5)
+    ob = s.observables()
+    assert np.max(np.abs(psi.cpu().numpy() - st.psi)) < 5e-6
+    assert np.max(np.abs(mu.cpu().numpy() - st.mu)) < 2e-5 * max(1.0, np.max(np.abs(st.mu)))
+    assert abs(ob.K - st.K) < 1e-7 and abs(ob.Ex - st.Ex) < 1e-7
+    links = O.paper_links(p, st.K, Bx, Bz)
+    F = O.free_energy(p, st.psi, eps, links)
+    assert abs(ob.free_energy - F) < 2e-6 * abs(F) + 1e-6 * p.n_sites
+    s.close()
+
+
+@pytest.mark.parametrize("nz", [8, 1])
+def test_free_energy_descends_on_the_gpu(nz):
+    """P12 on the CUDA path: without drive, noise and potential the discrete free energy never increases
+    (relaxation dynamics of Eq. 16; soft property of the CN + linearised scheme at h_t = 0.1)."""
+    cfg = cfg_of(48, 48, nz, (P_, P_, P_), nz_flux=4, incl_fraction=0.1, incl_rmin=1.5, incl_rmax=2.5, seed=12)
+    p, st, eps, B, s = setup_pair(cfg, solve_mu=False)
+    last = s.observables().free_energy
+    for _ in range(30):
+        s.step(2)
+        F = s.observables().free_energy
+        assert F <= last + 1e-6 * abs(last)
+        last = F
+    s.close()
