@@ -226,6 +226,8 @@ def _S(f, th, axis, bc):
     Periodic: indices wrap.  Open: the ghost value follows from n.(grad - iA~)psi = 0, i.e.
     U* f_{-1} = U f_{1} and U f_{N} = U* f_{N-2}: at the first site S- := S+, at the last S+ := S-."""
     e = np.exp(1j * th)
+    if f.dtype == np.complex64:          # single-precision replay (reading R3): fp64 phases, fp32 link variables
+        e = e.astype(np.complex64)
     sp = e * np.roll(f, -1, axis)
     sm = np.roll(np.conj(e) * f, 1, axis)
     if bc == OPEN:
@@ -302,12 +304,18 @@ def langevin_noise_at(p: Params, step: int, m):
     return zeta_max(p) * (philox.uniform_pm1(x0) + 1j * philox.uniform_pm1(x1))
 
 
+def box_muller(x0, x1):
+    """Two independent N(0,1) deviates per pair of Philox words (S13): u1, u2 uniform in (0, 1) from x0, x1,
+    g1 + i g2 = sqrt(-2 ln u1) exp(2 pi i u2)  (Box and Muller, 1958)."""
+    u1, u2 = philox.uniform_01(x0), philox.uniform_01(x1)
+    rad = np.sqrt(-2.0 * np.log(u1))
+    return rad * np.cos(2.0 * math.pi * u2) + 1j * rad * np.sin(2.0 * math.pi * u2)
+
+
 def initial_state(p: Params, init_amp: float) -> State:
     """psi0 = 1 + init_amp (N(0,1) + i N(0,1)), Box-Muller on Philox stream 1; mu = 0, K = 0 (S13)."""
     x0, x1 = philox.site_words(p.n_sites, 0, 1, p.seed)
-    u1, u2 = philox.uniform_01(x0), philox.uniform_01(x1)
-    rad = np.sqrt(-2.0 * np.log(u1))
-    psi = 1.0 + init_amp * (rad * np.cos(2.0 * math.pi * u2) + 1j * rad * np.sin(2.0 * math.pi * u2))
+    psi = 1.0 + init_amp * box_muller(x0, x1)
     return State(psi=psi.reshape(p.shape), mu=np.zeros(p.shape))
 
 
@@ -505,6 +513,8 @@ def step(p: Params, st: State, eps, Bx: float, Bz: float, Jext: float,
     if p.solve_mu:                                                            # step 6 (S4: updated K)
         links = links_fn(K)
         mu = solve_poisson(p, supercurrent_divergence(p, psi, links))
+        if psi.dtype == np.complex64:    # single-precision replay (R3): mu is stored in fp32 like psi
+            mu = mu.astype(np.float32)
     st.psi, st.mu, st.K, st.n = psi, mu, K, st.n + 1
     st.Ex, st.Jav = Ex, Jav
     st.sweeps_last, st.max_resid2 = sweeps, r2
