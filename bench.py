@@ -128,10 +128,25 @@ def throughput(n_sites, sweeps_all, steps_per_rank, world, ms):
     return n_sites * sweeps_all / (ms * 1e-3), world * steps_per_rank / (ms * 1e-3)
 
 
+def replica_seed(cfg: I.Config, rank: int) -> int:
+    """Replicas are independent problems: rank r draws its initial state and noise from Philox key seed + r."""
+    return cfg.seed + rank
+
+
+def config_dict(cfg: I.Config, world: int = 1):
+    """The `config` object of the JSON line; the same keys for our arm and for `--impl reference`."""
+    N = cfg.n_sites
+    return {"workload": cfg.name, "grid": [cfg.nx, cfg.ny, cfg.nz], "bc": list(cfg.bc), "h": cfg.h, "dt": cfg.dt,
+            "Bz": cfg.Bz, "Bx": cfg.Bx, "Jx": cfg.Jx, "T": cfg.temperature, "inclusion_fraction": cfg.incl_fraction,
+            "eps_tol": 1e-6, "parallelism": "replicas only" if world > 1 else "1 GPU",
+            "l2": "working set %.2f GB >> 126 MB L2, no flush needed" % (44.0 * N / 1e9),
+            "loop": "CUDA graph per step, WHILE node around the sweep, no host sync"}
+
+
 def make_solver(cfg: I.Config, host_loop=False, seed_offset=0):
     from paper_1409_8340_b200 import Solver
     s = Solver(cfg.nx, cfg.ny, cfg.nz, bc=cfg.bc, h=cfg.h, dt=cfg.dt, eps_tol=1e-6, max_sweeps=100,
-               temperature=cfg.temperature, seed=cfg.seed + seed_offset, init_amp=cfg.init_amp, solve_mu=True,
+               temperature=cfg.temperature, seed=replica_seed(cfg, seed_offset), init_amp=cfg.init_amp, solve_mu=True,
                host_loop=host_loop)
     s.set_pinning(I.sphere_list(cfg), cfg.eps_in, cfg.eps_out)
     bx, bz = cfg.requested_field()
@@ -139,13 +154,23 @@ def make_solver(cfg: I.Config, host_loop=False, seed_offset=0):
     return s
 
 
-def oracle_sample(cfg: I.Config, budget_s: float = 20.0):
-    """The fp64 oracle as it stands on a bounded sample of the workload: the same physics on a z-slab of
-    the grid (full x, y extent, 16 planes), as many steps as fit the budget (>= 2)."""
+def _slab(cfg: I.Config):
+    """The bounded sample: the same physics (boundary types, field, inclusions, current, noise) on a z-slab of
+    the grid with the full x, y extent and 16 planes."""
+    nz = min(cfg.nz, 16)
+    return cfg.scaled(cfg.nx, cfg.ny, nz, f"{cfg.name} slab {cfg.nx}x{cfg.ny}x{nz}")
+
+
+def _oracle_worker(args):
+    """One host core: the fp64 oracle as it stands (numpy, one thread) stepping its own replica of the slab
+    (Philox key and initial state offset by the worker index) until the time budget is spent."""
+    name, widx, budget_s = args
+    for v in ("OMP_NUM_THREADS", "OPENBLAS_NUM_THREADS", "MKL_NUM_THREADS"):
+        os.environ[v] = "1"
+    from dataclasses import replace
     from oracle import tdgl_oracle as O
     from gpu_common import f32, oracle_params
-    nz = min(cfg.nz, 16)
-    sub = cfg.scaled(cfg.nx, cfg.ny, nz, f"{cfg.name} slab {cfg.nx}x{cfg.ny}x{nz}")
+    sub = replace(_slab(I.CONFIGS[name]), seed=I.CONFIGS[name].seed + widx)
     p = oracle_params(sub)
     eps = O.epsilon_from_spheres(p, I.sphere_list(sub), sub.eps_in, sub.eps_out)
     bx, bz = sub.requested_field()
@@ -158,33 +183,62 @@ def oracle_sample(cfg: I.Config, budget_s: float = 20.0):
     while steps < 2 or (time.perf_counter() - t0 < budget_s and steps < 1000):
         O.step(p, st, eps, Bx, Bz, f32(sub.Jx))
         steps += 1
-    dt = time.perf_counter() - t0
-    sweeps = st.sweeps_total - sw0
-    return {"value": p.n_sites * sweeps / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
-            "sample": f"{sub.name}, {steps} steps, {sweeps} sweeps, {dt:.1f} s (numpy fp64, single thread)",
-            "steps_per_s_on_sample": steps / dt, "ms_per_step_sample": 1e3 * dt / steps,
-            "host_cores_available": os.cpu_count()}
+    return p.n_sites, steps, st.sweeps_total - sw0, time.perf_counter() - t0
+
+
+def host_cores() -> int:
+    try:
+        return len(os.sched_getaffinity(0))
+    except AttributeError:
+        return os.cpu_count() or 1
+
+
+def oracle_sample(cfg: I.Config, budget_s: float = 20.0, cores: int = 0):
+    """The fp64 oracle timed on ALL host cores of this box: one process per core (the oracle is single-threaded
+    numpy), each stepping an independent replica of the slab sample for `budget_s` seconds.
+    value = site-iterations of all workers / the slowest worker's time."""
+    import multiprocessing as mp
+    cores = cores or host_cores()
+    sub = _slab(cfg)
+    slab_gb = 16.0 * sub.n_sites * 40 / 1e9                    # ~40 fp64-complex temporaries per oracle step
+    try:
+        avail = os.sysconf("SC_AVPHYS_PAGES") * os.sysconf("SC_PAGE_SIZE") / 1e9
+        cores = max(1, min(cores, int(0.6 * avail / slab_gb)))
+    except (ValueError, OSError):
+        pass
+    t0 = time.perf_counter()
+    if cores == 1:
+        res = [_oracle_worker((cfg.name, 0, budget_s))]
+    else:
+        with mp.get_context("spawn").Pool(cores) as pool:
+            res = pool.map(_oracle_worker, [(cfg.name, w, budget_s) for w in range(cores)])
+    wall = time.perf_counter() - t0
+    n_sites = res[0][0]
+    steps = sum(r[1] for r in res)
+    sweeps = sum(r[2] for r in res)
+    dt = max(r[3] for r in res)
+    return {"value": n_sites * sweeps / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"{sub.name} (C-order numpy fp64 oracle as it stands), {cores} independent replicas on {cores} "
+                      f"host cores, {steps} steps and {sweeps} sweeps in {dt:.1f} s",
+            "steps_per_s_on_sample": steps / dt, "ms_per_step_sample": 1e3 * dt * cores / steps,
+            "host_cores_available": host_cores(), "wall_s": wall}
 
 
 def run_reference(args, cfg):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    budget = 8.0
-    vals, t_all = [], time.perf_counter()
-    for _ in range(max(1, args.warmup if args.warmup < 2 else 1)):
-        oracle_sample(cfg, 2.0)
-    res = None
-    per = []
-    for _ in range(max(1, min(args.steps, 8))):
-        res = oracle_sample(cfg, budget)
-        per.append(res["value"])
-    v = float(np.mean(per))
+    # one pool of workers for the whole run: an untimed first step per worker (warm-up: page-in, FFT plans), then
+    # oracle steps until the budget is spent (>= 2 per worker); sized so that the run ends within a few minutes
+    t_all = time.perf_counter()
+    res = oracle_sample(cfg, budget_s=min(60.0, max(10.0, 2.0 * args.steps)))
+    v = res["value"]
     out = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
            "warmup": args.warmup, "ms_per_step": res["ms_per_step_sample"], "higher_is_better": True,
            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-           "config": {"workload": cfg.name, "grid": [cfg.nx, cfg.ny, cfg.nz], "note": "each bench step = one bounded oracle sample"},
-           "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": res["sample"]},
+           "config": dict(config_dict(cfg), parallelism="%d host cores" % res["cores"], l2="n/a (host)",
+                          loop="oracle.step on a bounded slab sample per bench step; " + res["sample"]),
+           "cpu_baseline": {"value": v, "unit": UNIT, "cores": res["cores"], "kind": "oracle", "sample": res["sample"]},
            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
            "gpu_launches": 0, "wall_s": time.perf_counter() - t_all}
     print(json.dumps(out), flush=True)
@@ -273,7 +327,11 @@ def main():
                     "peak": peak, "unit": "GB/s", "frac": ach / peak, "peak_source": how,
                     "avg_launch_ms": avg_ms, "launches_timed": int(n_l),
                     "algorithmic_bytes_per_launch": SWEEP_BYTES_PER_SITE * N,
-                    "traffic": (tr or {}).get("dram_bytes_per_launch") if (tr or {}).get("sites") == N else None}
+                    "timed_in": "host-loop mode (TDGL_FLAG_HOST_LOOP): CUDA events around each single sweep launch after a "
+                                "stream sync; `value` is timed in graph mode, where launches overlap their predecessors' tails",
+                    "traffic": (tr or {}).get("dram_bytes_per_launch") if (tr or {}).get("sites") == N else None,
+                    "traffic_source": "profiles/sweep_traffic.txt (dram__bytes_read.sum + dram__bytes_write.sum of one committed "
+                                      "ncu --set full capture of this kernel on this grid; not measured in this run)"}
         sh.close()
         del sh
 
@@ -321,11 +379,7 @@ def main():
         "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
         "data": "synthetic", "steps_per_s": steps_per_s, "sweeps_per_step": sweeps_all / (K * world),
-        "config": {"workload": cfg.name, "grid": [cfg.nx, cfg.ny, cfg.nz], "bc": list(cfg.bc), "h": cfg.h, "dt": cfg.dt,
-                   "Bz": cfg.Bz, "Bx": cfg.Bx, "Jx": cfg.Jx, "T": cfg.temperature, "inclusion_fraction": cfg.incl_fraction,
-                   "eps_tol": 1e-6, "parallelism": "replicas only" if world > 1 else "1 GPU",
-                   "l2": "working set %.2f GB >> 126 MB L2, no flush needed" % (44.0 * N / 1e9),
-                   "loop": "CUDA graph per step, WHILE node around the sweep, no host sync"},
+        "config": config_dict(cfg, world),
         "clocks": clocks, "e2e": e2e, "gpu_launches": launches_all, "roofline": roof, "cpu_baseline": cpu,
         "state": {"mean_abs2": ob1.mean_abs2, "Ex": ob1.Ex, "K": ob1.K, "vortices_per_slice": ob1.vortices_per_slice,
                   "status": ob1.status},

@@ -13,7 +13,7 @@
  *
  * Data layout.  Site (i, j, k) of an nx x ny x nz mesh has the multi-index m = i + nx*(j + ny*k)
  * (x fastest).  psi is an array of N = nx*ny*nz interleaved (re, im) fp32 pairs, mu and eps
- * are fp32 arrays of N values.  nx must be even (rows are moved as 16-byte vectors).
+ * are fp32 arrays of N values.  nx must be even (rows are moved as 16-byte vectors); for a 3D mesh ny, nz <= 65535.
  *
  * Errors.  Every call returns an int: 0 = TDGL_OK, negative = error (nothing was done), positive =
  * warning (the call completed).  No exceptions, no aborts, nothing is printed.
@@ -30,7 +30,8 @@ extern "C" {
 #define TDGL_OK            0
 #define TDGL_EINVAL      (-1)   /* bad size / mesh / bc / pointer / struct_size                         */
 #define TDGL_ENOMEM      (-2)   /* workspace too small or not 256-byte aligned                          */
-#define TDGL_EINCOMPAT   (-3)   /* open x with Jx != 0, or By != 0 (yz gauge not built)         */
+#define TDGL_EINCOMPAT   (-3)   /* open x with Jx != 0; a field component the Landau gauge chosen  */
+                                /* at create cannot carry (By in the xz gauge, Bx in the yz gauge or film) */
 #define TDGL_ECUDA       (-4)   /* a CUDA runtime call failed; tdgl_last_cuda_error() has the code      */
 #define TDGL_WMAXSWEEPS    1    /* some step hit max_sweeps before max|r|^2 < eps_tol (S10)             */
 
@@ -105,10 +106,13 @@ int tdgl_destroy(tdgl_t *h);
  * The workspace scratch array holds the device copy, so n <= N/4. */
 int tdgl_set_pinning(tdgl_t *h, const tdgl_sphere *spheres_host, int64_t n, float eps_in, float eps_out);
 
-/* Applied field (xz Landau gauge, Eq. 24a) and transport current J_ext along x (Eq. 21).
- * B_z is snapped to 2 pi n_z/(Lx Ly) iff x and y are periodic, B_x to 2 pi n_x/(Ly Lz) iff y and z are
- * (P:467, S16); the effective values are reported by tdgl_observables.  Resets Ex_mean.
- * Errors: TDGL_EINCOMPAT if By != 0, or Jx != 0 with open x. */
+/* Applied field and transport current J_ext along x (Eq. 21).  The Landau gauge is fixed at create (S23):
+ * xz gauge (default; Eq. 24a): B = (Bx, 0, Bz); yz gauge (TDGL_FLAG_GAUGE_YZ; Eq. 24b): B = (0, By, Bz).
+ * B_z is snapped to 2 pi n_z/(Lx Ly) iff x and y are periodic; B_x to 2 pi n_x/(Ly Lz) iff y and z are; B_y to
+ * 2 pi n_y/(Lx Lz) iff x and z are; the effective values are reported by tdgl_observables.
+ * Resets Ex_mean.
+ * Errors: TDGL_EINCOMPAT if By != 0 in the xz gauge, Bx != 0 in the yz gauge or for a film, or Jx != 0 with
+ * open x. */
 int tdgl_set_field_current(tdgl_t *h, float Bx, float By, float Bz, float Jx);
 
 /* nsteps time steps in the paper's order "psi, then E, then mu": the implicit
@@ -117,7 +121,8 @@ int tdgl_set_field_current(tdgl_t *h, float Bx, float By, float Bz, float Jx);
 int tdgl_step(tdgl_t *h, int32_t nsteps);
 
 /* Device-to-device copy of the current state into caller buffers (either may be NULL):
- * psi_dev: N (re, im) fp32 pairs; mu_dev: N fp32.  Asynchronous on `stream`. */
+ * psi_dev: N (re, im) fp32 pairs, 16-byte aligned; mu_dev: N fp32.  Asynchronous on `stream` (which of the two psi buffers
+ * is current is device state; a copy kernel reads it on the device, the host never waits). */
 int tdgl_get_psi_mu(tdgl_t *h, void *psi_dev, void *mu_dev);
 
 /* Runs the reductions (a8) and fills *out_host.  Synchronises the stream. */

@@ -88,9 +88,6 @@ def lib() -> C.CDLL:
     L.tdgl_launch_count.restype = i64
     L.tdgl_launch_count.argtypes = [vp]
     L.tdgl_sweep_timing.argtypes = [vp, i32, C.POINTER(f64), C.POINTER(i64)]
-    for name in EXPORTS:
-        if getattr(L, name).restype is C.c_int and name not in ("tdgl_strerror",):
-            pass
     _lib = L
     return L
 

@@ -76,6 +76,15 @@ __global__ void k_set_field(const __grid_constant__ Dev dv, double Bx, double Bz
   }
 }
 
+// tdgl_get_psi_mu: copy the CURRENT psi buffer (ctl->xbuf, device state) to the caller's array, 16 bytes per access
+__global__ void __launch_bounds__(256) k_copy_psi(const __grid_constant__ Dev dv, float2 *__restrict__ out) {
+  const float4 *__restrict__ src = reinterpret_cast<const float4 *>(dv.psi[dv.ctl->xbuf & 1]);
+  float4 *dst = reinterpret_cast<float4 *>(out);
+  const long long n2 = dv.N / 2;                      // nx is even
+  for (long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x; m < n2; m += (long long)gridDim.x * blockDim.x)
+    dst[m] = __ldcs(src + m);
+}
+
 __global__ void k_fill_f32(float *p, long long n, float v) {
   for (long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x; m < n; m += (long long)gridDim.x * blockDim.x) p[m] = v;
 }
@@ -265,6 +274,7 @@ void launch_spheres(const Dev &dv, const float4 *sph, long long n, float eps_in,
     k_spheres<<<g, 128, 0, st>>>(dv, sph + off, eps_in);
   }
 }
+void launch_copy_psi(const Dev &dv, float2 *out, cudaStream_t st) { k_copy_psi<<<grid_for(dv.N / 2, 256, 148 * 16), 256, 0, st>>>(dv, out); }
 void launch_noise(const Dev &dv, long long step, float2 *out, cudaStream_t st) { k_noise<<<grid_for(dv.N, 256, 148 * 16), 256, 0, st>>>(dv, step, out); }
 int launch_obs(const Dev &dv, cudaStream_t st) {
   const long long nblk = (long long)((dv.ny + OBS_RB - 1) / OBS_RB) * dv.nz;

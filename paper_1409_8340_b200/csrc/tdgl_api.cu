@@ -30,6 +30,7 @@ void launch_fill(float *p, long long n, float v, cudaStream_t st);
 void launch_spheres(const Dev &dv, const float4 *sph, long long n, float eps_in, cudaStream_t st);
 void launch_noise(const Dev &dv, long long step, float2 *out, cudaStream_t st);
 int launch_obs(const Dev &dv, cudaStream_t st);
+void launch_copy_psi(const Dev &dv, float2 *out, cudaStream_t st);
 
 #define MODE_SWEEP 0
 #define MODE_INIT 1
@@ -66,10 +67,22 @@ struct tdgl {
 
 static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
+// SMs of the current device (B200: 148), queried once; the launch geometry is sized in multiples of it
+static int sm_count() {
+  static int n = 0;
+  if (n <= 0) {
+    int dev = 0, v = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0) n = v;
+    else { cudaGetLastError(); return 148; }
+  }
+  return n;
+}
+
 // launch geometry of the marching kernels (march_tma.cu): 128 x 8 tiles, one warp per row; z chunks chosen
 // so that there are enough CTAs for ~4 waves of 2 CTAs/SM, chunks of at least 8 planes
 static void march_geometry(const tdgl_params *p, unsigned *gx, unsigned *gy, unsigned *gz, int *zc_out) {
-  const long long want = 148ll * 2 * 4;
+  const long long nsm = sm_count();
+  const long long want = nsm * 2 * 4;
   if (p->nz == 1) {            // film (march_film.cu): strips of 1024 sites in x, chunks of rows in y
     const int a = march_film_strips(p->nx);
     int yc = p->ny;
@@ -84,7 +97,7 @@ static void march_geometry(const tdgl_params *p, unsigned *gx, unsigned *gy, uns
   // shorter chunks only to put at least one CTA on every SM (measured on C3: 32 planes 0.584 ms/step, 8 planes 0.616)
   auto ctas = [&](int z) { return (long long)a * b * ((p->nz + z - 1) / z); };
   while (zc > 32 && ctas(zc) < want) zc = (zc + 1) / 2;
-  while (zc > 8 && ctas(zc) < 148) zc = (zc + 1) / 2;
+  while (zc > 8 && ctas(zc) < nsm) zc = (zc + 1) / 2;
   *gx = (unsigned)a; *gy = (unsigned)b; *gz = (unsigned)((p->nz + zc - 1) / zc); *zc_out = zc;
 }
 
@@ -92,6 +105,8 @@ static bool params_ok(const tdgl_params *p) {
   if (!p || p->struct_size != sizeof(tdgl_params)) return false;
   if (p->nx < 2 || p->ny < 2 || p->nz < 1 || (p->nx & 1)) return false;      // nz = 1: film (2D mode, S22)
   if ((long long)p->nx * p->ny * p->nz > (1ll << 40)) return false;
+  // the strided transform passes put the "other" extent into grid.y (<= 65535): ny, nz for a 3D mesh, none for a film
+  if (p->nz > 1 && (p->ny > 65535 || p->nz > 65535)) return false;
   if (!(p->hx > 0.f) || !(p->hy > 0.f) || !(p->hz > 0.f) || !(p->dt > 0.f) || !(p->u > 0.f) || !(p->g > 0.f)) return false;
   for (int a = 0; a < 3; ++a)
     if (p->bc[a] != TDGL_BC_PERIODIC && p->bc[a] != TDGL_BC_OPEN) return false;
@@ -176,6 +191,12 @@ static int enqueue_after_solve(tdgl_t *h, cudaStream_t st) {
   return n;
 }
 
+// inside a capture segment: a failing call (or a failed captured launch) ends the capture and discards what it built,
+// so that tdgl_destroy never sees a stream that is still capturing
+#define CKCAP(call) do { cudaError_t e_ = (call); if (e_ == cudaSuccess) e_ = cudaGetLastError(); \
+    if (e_ != cudaSuccess) { cudaGraph_t junk_ = nullptr; cudaStreamEndCapture(cs, &junk_); cudaGetLastError(); \
+      return cuda_fail(h, e_); } } while (0)
+
 static int build_graph(tdgl_t *h) {
   CK(cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking));
   CK(cudaGraphCreate(&h->graph, 0));
@@ -188,10 +209,11 @@ static int build_graph(tdgl_t *h) {
   CK(cudaStreamBeginCaptureToGraph(cs, h->graph, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal));
   launch_step_begin(h->dv, cs);
   march(h, MODE_INIT, h->dv, cs);
+  CKCAP(cudaSuccess);
   cudaStreamCaptureStatus status;
   const cudaGraphNode_t *deps = nullptr;
   size_t ndeps = 0;
-  CK(cudaStreamGetCaptureInfo(cs, &status, nullptr, nullptr, &deps, &ndeps));
+  CKCAP(cudaStreamGetCaptureInfo(cs, &status, nullptr, nullptr, &deps, &ndeps));
   std::vector<cudaGraphNode_t> tail(deps, deps + ndeps);
   cudaGraph_t g2;
   CK(cudaStreamEndCapture(cs, &g2));
@@ -206,10 +228,12 @@ static int build_graph(tdgl_t *h) {
   cudaGraph_t body = np.conditional.phGraph_out[0];
   CK(cudaStreamBeginCaptureToGraph(cs, body, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal));
   march(h, MODE_SWEEP, h->dv, cs);
+  CKCAP(cudaSuccess);
   CK(cudaStreamEndCapture(cs, &g2));
   // segment B: everything after the psi solve
   CK(cudaStreamBeginCaptureToGraph(cs, h->graph, &cond, nullptr, 1, cudaStreamCaptureModeThreadLocal));
   h->fixed_per_step = 2 + enqueue_after_solve(h, cs);
+  CKCAP(cudaSuccess);
   CK(cudaStreamEndCapture(cs, &g2));
   CK(cudaGraphInstantiate(&h->exec, h->graph, 0));
   return TDGL_OK;
@@ -428,12 +452,12 @@ extern "C" int tdgl_step(tdgl_t *h, int32_t nsteps) {
 }
 
 extern "C" int tdgl_get_psi_mu(tdgl_t *h, void *psi_dev, void *mu_dev) {
-  if (!h) return TDGL_EINVAL;
+  if (!h || ((uintptr_t)psi_dev & 15)) return TDGL_EINVAL;
   if (psi_dev) {
-    // which buffer holds psi is device state: read it (4 bytes) before the copy
-    CK(cudaMemcpyAsync(h->h_flag + 4, &h->dv.ctl->xbuf, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
-    CK(cudaStreamSynchronize(h->stream));
-    CK(cudaMemcpyAsync(psi_dev, h->dv.psi[h->h_flag[4] & 1], (size_t)h->dv.N * sizeof(float2), cudaMemcpyDeviceToDevice, h->stream));
+    // which buffer holds psi is device state (ctl->xbuf): the copy kernel reads it on the device
+    launch_copy_psi(h->dv, (float2 *)psi_dev, h->stream);
+    h->launches += 1;
+    CKL();
   }
   if (mu_dev) CK(cudaMemcpyAsync(mu_dev, h->dv.mu, (size_t)h->dv.N * sizeof(float), cudaMemcpyDeviceToDevice, h->stream));
   return TDGL_OK;
@@ -465,7 +489,7 @@ extern "C" const char *tdgl_strerror(int code) {
     case TDGL_OK: return "ok";
     case TDGL_EINVAL: return "invalid argument (size, mesh, boundary type, pointer or struct_size)";
     case TDGL_ENOMEM: return "workspace too small or misaligned";
-    case TDGL_EINCOMPAT: return "incompatible request (open x with a current, or By != 0)";
+    case TDGL_EINCOMPAT: return "incompatible request (open x with a current, or a field component the chosen Landau gauge cannot carry)";
     case TDGL_ECUDA: return "CUDA runtime error";
     case TDGL_WMAXSWEEPS: return "warning: Jacobi iteration hit max_sweeps";
     default: return "unknown code";
@@ -565,9 +589,10 @@ extern "C" int64_t tdgl_launch_count(const tdgl_t *h) {
   int64_t n = h->launches;
   if (h->use_graph && h->graph_steps > 0) {
     long long tot = 0, steps = 0;
-    cudaStreamSynchronize(h->stream);
-    cudaMemcpy(&tot, &h->dv.ctl->sweeps_total, sizeof(long long), cudaMemcpyDeviceToHost);
-    cudaMemcpy(&steps, &h->dv.ctl->n, sizeof(long long), cudaMemcpyDeviceToHost);
+    if (cudaMemcpyAsync(&tot, &h->dv.ctl->sweeps_total, sizeof(long long), cudaMemcpyDeviceToHost, h->stream) != cudaSuccess ||
+        cudaMemcpyAsync(&steps, &h->dv.ctl->n, sizeof(long long), cudaMemcpyDeviceToHost, h->stream) != cudaSuccess ||
+        cudaStreamSynchronize(h->stream) != cudaSuccess)
+      return -1;
     // per graph step: fixed_per_step kernels (begin, init+sweep 1, ...) + the further sweeps
     n += h->graph_steps * (int64_t)h->fixed_per_step + (tot - steps);
   }

@@ -50,23 +50,50 @@ def test_single_rank_needs_no_process_group():
     assert v == pytest.approx(10 * 5 / 1e-3) and s == pytest.approx(2 / 1e-3)
 
 
-def test_replica_seeds_differ_per_rank():
-    """Replicas are independent problems: bench.make_solver offsets the Philox seed by the rank."""
-    import inspect
+def _seed_worker(rank, world, port, out):
     sys.path.insert(0, ROOT)
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
     import bench
-    src = inspect.getsource(bench.main)
-    assert "seed_offset=rank" in src
+    import tdgl_inputs as I
+    from oracle import tdgl_oracle as O
+    cfg = I.CONFIGS["C2"].scaled(8, 8, 4)
+    seed = bench.replica_seed(cfg, rank)
+    # what the replica's seed feeds: the Philox key of its initial state and Langevin stream
+    psi0 = O.initial_state(O.Params(8, 8, 4, seed=seed), cfg.init_amp).psi
+    t = torch.zeros(world, 1 + psi0.size, dtype=torch.float64)
+    t[rank, 0] = seed
+    t[rank, 1:] = torch.from_numpy(psi0.real.ravel().copy())
+    dist.all_reduce(t)
+    if rank == 0:
+        torch.save(t, out)
+    dist.barrier()
+    dist.destroy_process_group()
 
 
+def test_replicas_draw_from_different_philox_keys(tmp_path):
+    """Replicas are independent problems: each rank's seed is distinct and gives a different initial field."""
+    world, out = 2, str(tmp_path / "s.pt")
+    mp.spawn(_seed_worker, args=(world, _free_port(), out), nprocs=world, join=True)
+    t = torch.load(out)
+    assert t[0, 0] != t[1, 0]
+    assert float((t[0, 1:] - t[1, 1:]).abs().max()) > 1e-3
+
+
+@pytest.mark.gpu
 def test_solver_binds_to_the_current_device_not_to_cuda0():
-    """One process per GPU: bench.py calls torch.cuda.set_device(LOCAL_RANK) and the Solver must allocate there."""
-    import inspect
-    from paper_1409_8340_b200.binding import Solver
-    sig = inspect.signature(Solver.__init__)
-    assert sig.parameters["device"].default is None
-    src = inspect.getsource(Solver.__init__)
-    assert "current_device()" in src
-    sys.path.insert(0, ROOT)
-    import bench
-    assert "torch.cuda.set_device(local_rank)" in inspect.getsource(bench.main)
+    """One process per GPU: bench.py calls torch.cuda.set_device(LOCAL_RANK); the Solver allocates its workspace on
+    the CURRENT device and enqueues on that device's current stream."""
+    from paper_1409_8340_b200 import Solver
+    cur = torch.cuda.current_device()
+    s = Solver(16, 8, 4)
+    assert s.device.index == cur and s.workspace.device.index == cur
+    assert s.stream.cuda_stream == torch.cuda.current_stream(s.device).cuda_stream
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        s2 = Solver(16, 8, 4)
+        assert s2.stream.cuda_stream == side.cuda_stream
+        s2.step(2)
+        assert s2.observables().steps == 2
+        s2.close()
+    s.close()
