@@ -42,6 +42,9 @@ extern "C" {
 #define TDGL_FLAG_GAUGE_YZ 4u   /* field in the yz plane: Landau gauge A = xbar [0, Bz, -By] (Eq. 24b),
                                    quasi-periodic jump in x.  set_field_current then takes By (Bx
                                    must be 0) and tdgl_obs.Bx_eff reports the effective B_y.  Not for films. */
+#define TDGL_FLAG_MU_REFINE   8u /* always run one step of iterative refinement after the mu solve (below)       */
+#define TDGL_FLAG_MU_NOREFINE 16u /* never run it.  Neither flag: automatic, iff tdgl_mu_gain() > TDGL_MU_REFINE_GAIN */
+#define TDGL_MU_REFINE_GAIN 200.0
 #define TDGL_FLAG_HOST_LOOP 2u  /* test/diagnostic: host-driven sweep loop instead of the CUDA-graph
                                    WHILE node (identical arithmetic)                                     */
 
@@ -130,6 +133,16 @@ int tdgl_observables(tdgl_t *h, tdgl_obs *out_host);
 
 const char *tdgl_strerror(int code);
 int tdgl_last_cuda_error(const tdgl_t *h);
+
+/* Accuracy of the fp32 mu solve (Eq. 18).  The solver's own roundings and those of rho = div j_s are
+ * white, and Delta_h^{-1} amplifies white noise by G = ((1/N) sum_{q != 0} 1/lambda_q^2)^{1/2} (lambda_q: eigenvalues
+ * of the 7-point operator for this mesh and boundary types): |delta mu| ~ 2e-7 G rms(rho), measured.  G < 2 on the
+ * 3D BASELINE grids, but it grows like L^{3/2} on quasi-one-dimensional meshes (500 on a 1026 x 3 film with open x).
+ * With refinement on, every mu solve is followed by mu += Delta_h^{-1}(rho_64 - Delta_h mu), the residual being
+ * evaluated in fp64 from psi (fp64 link variables): one more stencil pass and one more solve per step, 4 more
+ * bytes of workspace per site.  tdgl_mu_gain returns G for these params (host arithmetic only; -1 if invalid). */
+double tdgl_mu_gain(const tdgl_params *p_host);
+int tdgl_mu_refine_enabled(const tdgl_t *h);      /* 1 / 0 */
 
 /* ---- extensions used by the tests and the bench (not part of the paper's problem statement) ---- */
 

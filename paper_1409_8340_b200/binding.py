@@ -12,13 +12,13 @@ _LIB_PATH = os.environ.get("TDGL_LIB") or os.path.join(_HERE, "libtdgl.so")     
 
 TDGL_OK, TDGL_EINVAL, TDGL_ENOMEM, TDGL_EINCOMPAT, TDGL_ECUDA, TDGL_WMAXSWEEPS = 0, -1, -2, -3, -4, 1
 TDGL_BC_PERIODIC, TDGL_BC_OPEN = 0, 1
-TDGL_FLAG_SOLVE_MU, TDGL_FLAG_HOST_LOOP, TDGL_FLAG_GAUGE_YZ = 1, 2, 4
+TDGL_FLAG_SOLVE_MU, TDGL_FLAG_HOST_LOOP, TDGL_FLAG_GAUGE_YZ, TDGL_FLAG_MU_REFINE, TDGL_FLAG_MU_NOREFINE = 1, 2, 4, 8, 16
 
 EXPORTS = (
     "tdgl_workspace_bytes", "tdgl_create", "tdgl_destroy", "tdgl_set_pinning", "tdgl_set_field_current", "tdgl_step",
     "tdgl_get_psi_mu", "tdgl_observables", "tdgl_strerror", "tdgl_last_cuda_error", "tdgl_set_state", "tdgl_set_solver",
     "tdgl_set_sweep_schedule", "tdgl_get_sweep_log", "tdgl_get_eps", "tdgl_debug_noise", "tdgl_debug_poisson",
-    "tdgl_debug_rho", "tdgl_launch_count", "tdgl_sweep_timing",
+    "tdgl_debug_rho", "tdgl_launch_count", "tdgl_sweep_timing", "tdgl_mu_gain", "tdgl_mu_refine_enabled",
 )
 
 
@@ -88,6 +88,9 @@ def lib() -> C.CDLL:
     L.tdgl_launch_count.restype = i64
     L.tdgl_launch_count.argtypes = [vp]
     L.tdgl_sweep_timing.argtypes = [vp, i32, C.POINTER(f64), C.POINTER(i64)]
+    L.tdgl_mu_gain.restype = f64
+    L.tdgl_mu_gain.argtypes = [C.POINTER(TdglParams)]
+    L.tdgl_mu_refine_enabled.argtypes = [vp]
     _lib = L
     return L
 
@@ -154,7 +157,7 @@ class Solver:
                  u: float = 1.0, g: float = 1.0, eps_tol: float = 1e-6, max_sweeps: int = 100, fixed_sweeps: int = 0,
                  temperature: float = 0.0, seed: int = 0, init_amp: float = 0.01, solve_mu: bool = True,
                  host_loop: bool = False, hxyz: Optional[Sequence[float]] = None, device: Optional[str] = None,
-                 gauge_yz: bool = False):
+                 gauge_yz: bool = False, mu_refine: Optional[bool] = None):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1409_8340_b200 needs a CUDA device (sm_100a); there is no CPU path")
@@ -170,7 +173,8 @@ class Solver:
         p.eps_tol, p.max_sweeps, p.fixed_sweeps = eps_tol, max_sweeps, fixed_sweeps
         p.temperature, p.seed, p.init_amp = temperature, seed, init_amp
         p.flags = ((TDGL_FLAG_SOLVE_MU if solve_mu else 0) | (TDGL_FLAG_HOST_LOOP if host_loop else 0)
-                   | (TDGL_FLAG_GAUGE_YZ if gauge_yz else 0))
+                   | (TDGL_FLAG_GAUGE_YZ if gauge_yz else 0)
+                   | (0 if mu_refine is None else (TDGL_FLAG_MU_REFINE if mu_refine else TDGL_FLAG_MU_NOREFINE)))
         nbytes = tdgl_workspace_bytes(p)
         if nbytes == 0:
             raise TdglError(TDGL_EINVAL, "tdgl_workspace_bytes")
@@ -265,6 +269,12 @@ class Solver:
         rho = t.empty(self.shape, dtype=t.float32, device=self.device)
         _check(lib().tdgl_debug_rho(self.h, rho.data_ptr()), "tdgl_debug_rho", self.h)
         return rho
+
+    def mu_gain(self) -> float:
+        return float(lib().tdgl_mu_gain(C.byref(self.params)))
+
+    def mu_refine_enabled(self) -> bool:
+        return bool(lib().tdgl_mu_refine_enabled(self.h))
 
     def launch_count(self) -> int:
         return int(lib().tdgl_launch_count(self.h))

@@ -48,16 +48,20 @@ __global__ void k_set_field(const __grid_constant__ Dev dv, double Bx, double Bz
       const double xbar = i * dv.hx - 0.5 * dv.Lx;
       sincos(-dv.hy * Bz * xbar, &s, &c);
       dv.Uy[i] = make_float2((float)c, (float)s);
+      dv.Uy64[i] = make_double2(c, s);
       sincos(dv.hz * By * xbar, &s, &c);
       dv.Uzx[i] = make_float2((float)c, (float)s);
+      dv.Uzx64[i] = make_double2(c, s);
     }
     for (int j = tid; j < dv.ny; j += nth) {
       sincos(-(double)j * dv.hy * dv.Lx * Bz, &s, &c);
       dv.Pj[j] = make_float2((float)c, (float)s);
+      dv.Pj64[j] = make_double2(c, s);
     }
     for (int k = tid; k < dv.nz; k += nth) {
       sincos((double)k * dv.hz * dv.Lx * By, &s, &c);
       dv.Pk[k] = make_float2((float)c, (float)s);
+      dv.Pk64[k] = make_double2(c, s);
     }
     return;
   }
@@ -65,14 +69,17 @@ __global__ void k_set_field(const __grid_constant__ Dev dv, double Bx, double Bz
     const double ybar = j * dv.hy - 0.5 * dv.Ly;
     sincos(-dv.hz * Bx * ybar, &s, &c);
     dv.Uz[j] = make_float2((float)c, (float)s);
+    dv.Uz64[j] = make_double2(c, s);
   }
   for (int i = tid; i < dv.nx; i += nth) {
     sincos((double)i * dv.hx * dv.Ly * Bz, &s, &c);
     dv.Pi[i] = make_float2((float)c, (float)s);
+    dv.Pi64[i] = make_double2(c, s);
   }
   for (int k = tid; k < dv.nz; k += nth) {
     sincos((double)k * dv.hz * dv.Ly * Bx, &s, &c);
     dv.Pk[k] = make_float2((float)c, (float)s);
+    dv.Pk64[k] = make_double2(c, s);
   }
 }
 

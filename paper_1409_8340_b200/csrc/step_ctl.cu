@@ -46,6 +46,7 @@ __device__ void write_Ux(const Dev &dv, double K, int tid, int nthreads) {
     double s, c;
     sincos(dv.hx * (K + Bz * ybar), &s, &c);
     dv.Ux[j] = make_float2((float)c, (float)s);
+    dv.Ux64[j] = make_double2(c, s);
   }
 }
 

@@ -31,6 +31,8 @@ void launch_spheres(const Dev &dv, const float4 *sph, long long n, float eps_in,
 void launch_noise(const Dev &dv, long long step, float2 *out, cudaStream_t st);
 int launch_obs(const Dev &dv, cudaStream_t st);
 void launch_copy_psi(const Dev &dv, float2 *out, cudaStream_t st);
+void launch_mu_residual(const Dev &dv, const float *rho, const float *mu, float *out, cudaStream_t st);
+void launch_mu_add(const Dev &dv, float *mu, const float *delta, cudaStream_t st);
 
 #define MODE_SWEEP 0
 #define MODE_INIT 1
@@ -117,6 +119,43 @@ static bool params_ok(const tdgl_params *p) {
   return true;
 }
 
+// White-noise gain of the discrete inverse Laplacian, G = ((1/N) sum_{q != 0} 1/lambda_q^2)^{1/2} (refine.cu): the factor
+// by which the solve amplifies the (white) fp32 roundings of rho and of the transform passes.  1/lambda^2 falls like
+// |q|^-4, so the 48 smallest eigenvalues per axis carry the sum.  Host, fp64, from the params alone.
+static double mu_gain(const tdgl_params *p) {
+  const bool film = p->nz == 1;
+  const int ns[3] = {p->nx, p->ny, p->nz};
+  const int bcs[3] = {p->bc[0], p->bc[1], film ? TDGL_BC_PERIODIC : p->bc[2]};
+  const double cs[3] = {1.0 / ((double)p->hx * p->hx), 1.0 / ((double)p->hy * p->hy),
+                        film ? 0.0 : 1.0 / ((double)p->g * p->g * (double)p->hz * p->hz)};
+  const double pi = 3.14159265358979323846;
+  std::vector<double> lam[3];
+  for (int a = 0; a < 3; ++a) {
+    const int n = ns[a], keep = n < 48 ? n : 48;
+    // eigenvalues in ascending |lambda|: open q = 0, 1, 2, ...; periodic 0, then the pairs (q, n - q)
+    for (int t = 0; t < keep; ++t) {
+      double ang;
+      if (n == 1) ang = 0.0;
+      else if (bcs[a] == TDGL_BC_OPEN) ang = pi * t / (n - 1);
+      else ang = 2.0 * pi * ((t + 1) / 2) / n;
+      lam[a].push_back(cs[a] * (2.0 - 2.0 * std::cos(ang)));
+    }
+  }
+  double sum = 0.0;
+  for (double lx : lam[0]) for (double ly : lam[1]) for (double lz : lam[2]) {
+    const double l = lx + ly + lz;
+    if (l > 1e-14) sum += 1.0 / (l * l);
+  }
+  return std::sqrt(sum / ((double)p->nx * p->ny * p->nz));
+}
+// Refinement of the mu solve: forced by TDGL_FLAG_MU_REFINE, suppressed by TDGL_FLAG_MU_NOREFINE, otherwise
+// automatic for meshes whose gain exceeds TDGL_MU_REFINE_GAIN (quasi-1D / thin long films; never the 3D BASELINE grids)
+static bool want_refine(const tdgl_params *p) {
+  if (!(p->flags & TDGL_FLAG_SOLVE_MU) || (p->flags & TDGL_FLAG_MU_NOREFINE)) return false;
+  if (p->flags & TDGL_FLAG_MU_REFINE) return true;
+  return mu_gain(p) > TDGL_MU_REFINE_GAIN;
+}
+
 // workspace carving; with base == nullptr only the size is computed
 static size_t carve(const tdgl_params *p, char *base, Dev *dv) {
   const size_t N = (size_t)p->nx * p->ny * p->nz;
@@ -131,6 +170,13 @@ static size_t carve(const tdgl_params *p, char *base, Dev *dv) {
   q = take(p->nx * sizeof(float2)); if (dv) dv->Uy = (float2 *)q;
   q = take(p->nx * sizeof(float2)); if (dv) dv->Uzx = (float2 *)q;
   q = take(p->ny * sizeof(float2)); if (dv) dv->Pj = (float2 *)q;
+  q = take(p->ny * sizeof(double2)); if (dv) dv->Ux64 = (double2 *)q;
+  q = take(p->ny * sizeof(double2)); if (dv) dv->Uz64 = (double2 *)q;
+  q = take(p->nx * sizeof(double2)); if (dv) dv->Pi64 = (double2 *)q;
+  q = take(p->nz * sizeof(double2)); if (dv) dv->Pk64 = (double2 *)q;
+  q = take(p->nx * sizeof(double2)); if (dv) dv->Uy64 = (double2 *)q;
+  q = take(p->nx * sizeof(double2)); if (dv) dv->Uzx64 = (double2 *)q;
+  q = take(p->ny * sizeof(double2)); if (dv) dv->Pj64 = (double2 *)q;
   const int ns[3] = {p->nx, p->ny, p->nz};
   for (int a = 0; a < 3; ++a) {
     q = take(ns[a] * sizeof(float)); if (dv) dv->lam[a] = (float *)q;
@@ -156,6 +202,7 @@ static size_t carve(const tdgl_params *p, char *base, Dev *dv) {
   q = take(N * sizeof(float)); if (dv) dv->mu = (float *)q;
   q = take(N * sizeof(float)); if (dv) dv->eps = (float *)q;
   q = take(N * sizeof(float)); if (dv) dv->scratch = (float *)q;
+  if (want_refine(p)) { q = take(N * sizeof(float)); if (dv) { dv->resid = (float *)q; dv->mu_refine = 1; } }
   return off;
 }
 
@@ -187,6 +234,11 @@ static int enqueue_after_solve(tdgl_t *h, cudaStream_t st) {
   if (h->dv.solve_mu) {
     march(h, MODE_RHO, h->dv, st); ++n;
     n += poisson_solve(h->dvp, h->dv.mu, true, st);
+    if (h->dv.mu_refine) {                       // mu += S(rho_64 - Delta_h mu)  (refine.cu)
+      launch_mu_residual(h->dv, nullptr, h->dv.mu, h->dv.resid, st); ++n;
+      n += poisson_solve(h->dvp, h->dv.resid, true, st);
+      launch_mu_add(h->dv, h->dv.mu, h->dv.resid, st); ++n;
+    }
   }
   return n;
 }
@@ -496,6 +548,8 @@ extern "C" const char *tdgl_strerror(int code) {
   }
 }
 extern "C" int tdgl_last_cuda_error(const tdgl_t *h) { return h ? h->last_cuda : 0; }
+extern "C" double tdgl_mu_gain(const tdgl_params *p) { return params_ok(p) ? mu_gain(p) : -1.0; }
+extern "C" int tdgl_mu_refine_enabled(const tdgl_t *h) { return h ? h->dv.mu_refine : TDGL_EINVAL; }
 
 extern "C" int tdgl_set_state(tdgl_t *h, const void *psi_dev, const void *mu_dev, double K) {
   if (!h || !psi_dev) return TDGL_EINVAL;
@@ -567,9 +621,16 @@ extern "C" int tdgl_debug_noise(tdgl_t *h, int64_t step, void *zeta_dev) {
 
 extern "C" int tdgl_debug_poisson(tdgl_t *h, const void *rho_dev, void *mu_dev) {
   if (!h || !rho_dev || !mu_dev) return TDGL_EINVAL;
+  if (h->dv.mu_refine)                            // keep rho: the residual needs it after the in-place solve
+    CK(cudaMemcpyAsync(h->dv.resid, rho_dev, (size_t)h->dv.N * sizeof(float), cudaMemcpyDeviceToDevice, h->stream));
   if (rho_dev != mu_dev)
     CK(cudaMemcpyAsync(mu_dev, rho_dev, (size_t)h->dv.N * sizeof(float), cudaMemcpyDeviceToDevice, h->stream));
   h->launches += poisson_solve(h->dvp, (float *)mu_dev, true, h->stream);
+  if (h->dv.mu_refine) {
+    launch_mu_residual(h->dv, h->dv.resid, (const float *)mu_dev, h->dv.resid, h->stream);
+    h->launches += 2 + poisson_solve(h->dvp, h->dv.resid, true, h->stream);
+    launch_mu_add(h->dv, (float *)mu_dev, h->dv.resid, h->stream);
+  }
   CKL();
   return TDGL_OK;
 }

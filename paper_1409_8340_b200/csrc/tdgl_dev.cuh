@@ -59,6 +59,10 @@ struct Dev {
   // link variables U_y(i), U_z(i), jump in x  P_{j,k} = Pj[j] Pk[k]
   int gauge_yz;
   float2 *Uy, *Uzx, *Pj;
+  // fp64 copies of all link / jump tables and the residual array of the mu refinement step (refine.cu)
+  double2 *Ux64, *Uz64, *Pi64, *Pk64, *Uy64, *Uzx64, *Pj64;
+  float *resid;             // N floats, only when mu_refine
+  int mu_refine;            // one step of iterative refinement after every mu solve
   float *lam[3];            // eigenvalues of the 1-D operators per axis
   float2 *tw[3];            // FFT twiddles exp(-2 pi i m/n) per axis (power-of-two periodic axes)
   double *tab[3];           // generic transform tables: cas(2 pi m/n) or cos(pi m/(n-1))

@@ -22,17 +22,17 @@ def oracle_params(cfg: I.Config, eps_tol=1e-6, max_sweeps=100, solve_mu=True, te
 
 
 def make_solver(cfg: I.Config, eps_tol=1e-6, max_sweeps=100, solve_mu=True, temperature=None, host_loop=False,
-                fixed_sweeps=0, hxyz=None, g=1.0, u=1.0):
+                fixed_sweeps=0, hxyz=None, g=1.0, u=1.0, mu_refine=None):
     from paper_1409_8340_b200 import Solver
     return Solver(cfg.nx, cfg.ny, cfg.nz, bc=cfg.bc, h=cfg.h, dt=cfg.dt, g=g, u=u, eps_tol=eps_tol, max_sweeps=max_sweeps,
                   fixed_sweeps=fixed_sweeps, temperature=cfg.temperature if temperature is None else temperature,
-                  seed=cfg.seed, init_amp=cfg.init_amp, solve_mu=solve_mu, host_loop=host_loop, hxyz=hxyz)
+                  seed=cfg.seed, init_amp=cfg.init_amp, solve_mu=solve_mu, host_loop=host_loop, hxyz=hxyz, mu_refine=mu_refine)
 
 
 def setup_pair(cfg: I.Config, psi0=None, mu0=None, K0=0.0, with_pinning=True, **kw):
     """Returns (oracle params, oracle state, eps, (Bx, Bz) effective, solver) with identical inputs."""
     import torch
-    p = oracle_params(cfg, **{k: v for k, v in kw.items() if k not in ("host_loop", "fixed_sweeps")})
+    p = oracle_params(cfg, **{k: v for k, v in kw.items() if k not in ("host_loop", "fixed_sweeps", "mu_refine")})
     s = make_solver(cfg, **kw)
     spheres = I.sphere_list(cfg) if with_pinning else np.zeros((0, 4), np.float32)
     eps = O.epsilon_from_spheres(p, spheres, cfg.eps_in, cfg.eps_out)

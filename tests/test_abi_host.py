@@ -180,3 +180,31 @@ def test_input_recipes_match_the_baseline_configs():
     V = (c.nx * c.h) * (c.ny * c.h) * (c.nz * c.h)
     assert len(a) == round(-np.log(1 - 0.10) * V / (4 / 3 * np.pi * 2.0 ** 3))
     assert len(I.sphere_list(I.CONFIGS["C1"])) == 0
+
+
+def test_mu_gain_is_the_white_noise_gain_of_the_inverse_laplacian(L):
+    """tdgl_mu_gain (host arithmetic only): G = ((1/N) sum_{q != 0} 1/lambda_q^2)^{1/2} against the exact sum over the
+    oracle's eigenvalue table on small meshes; the automatic refinement rule G > TDGL_MU_REFINE_GAIN = 200 leaves the
+    3D BASELINE grids alone and catches long thin meshes."""
+    import math
+    from oracle import tdgl_oracle as O
+    L.tdgl_mu_gain.restype = C.c_double
+
+    def gain_c(nx, ny, nz, bc, h=(0.5, 0.5, 0.5), g=1.0):
+        p = _params(nx=nx, ny=ny, nz=nz, hx=h[0], hy=h[1], hz=h[2], g=g)
+        p.bc[0], p.bc[1], p.bc[2] = bc
+        return L.tdgl_mu_gain(C.byref(p))
+
+    for (nx, ny, nz), bc, h, g in [((34, 13, 11), (0, 1, 1), (0.5, 0.4, 0.7), 1.3), ((200, 6, 1), (1, 0, 0), (0.5, 0.5, 0.5), 1.0),
+                                   ((64, 64, 32), (0, 0, 1), (0.5, 0.5, 0.5), 1.0), ((30, 30, 30), (1, 1, 1), (0.5, 0.5, 0.5), 1.0)]:
+        f32 = lambda v: float(np.float32(v))
+        p = O.Params(nx, ny, nz, hx=f32(h[0]), hy=f32(h[1]), hz=f32(h[2]), g=f32(g), bc=(bc[0], bc[1], 0 if nz == 1 else bc[2]))
+        lam = O.laplacian_eigenvalues(p).ravel()
+        lam = lam[np.abs(lam) > 1e-12]
+        exact = math.sqrt(np.sum(1.0 / lam ** 2) / p.n_sites)
+        assert abs(gain_c(nx, ny, nz, bc, h, g) - exact) < 1e-2 * exact, (nx, ny, nz, bc)   # 48 lowest modes per axis carry the sum
+    assert gain_c(512, 512, 256, (0, 0, 1)) < 1.0 and gain_c(1024, 1024, 512, (1, 1, 1)) < 3.0
+    assert gain_c(256, 256, 128, (0, 0, 1)) < 1.0 and gain_c(64, 64, 64, (0, 0, 0)) < 1.0
+    assert gain_c(1026, 4, 1, (1, 1, 0)) > 400.0 and gain_c(2050, 10, 1, (1, 0, 0)) > 700.0
+    bad = _params(nx=31)
+    assert L.tdgl_mu_gain(C.byref(bad)) == -1.0

@@ -27,8 +27,6 @@ def test_film_one_step_fixed_sweeps(bc, shape, host_loop):
     """Two steps of five sweeps: ragged strips (1100 = 1024 + 76, 2050 = 2 x 1024 + 2), short chunks, every
     boundary combination, noise, inclusions, current."""
     nx, ny = shape
-    if nx > 2000 and bc[0] == O_:
-        nx = 1300            # a 1025-xi0 long open axis puts fp32 low modes of mu beyond the 2e-5 gate (DESIGN.md H4)
     cfg = film(nx, ny, bc, Bz=0.3, Jx=0.02 if bc[0] == P_ else 0.0, temperature=1e-3, incl_fraction=0.15,
                incl_rmin=1.0, incl_rmax=2.0, seed=2)
     psi0, mu0 = I.random_state(cfg, seed=21, amp=0.8)
@@ -52,8 +50,6 @@ def test_film_one_step_fixed_sweeps(bc, shape, host_loop):
 @pytest.mark.parametrize("shape", [(64, 64), (128, 40), (34, 22), (512, 256), (2048, 24), (24, 2048), (4096, 12),
                                    (16, 4096), (8192, 8), (8, 8192)])
 def test_film_poisson(bc, shape):
-    if max(shape) > 1366 and O_ in (bc[0] if shape[0] > 1366 else P_, bc[1] if shape[1] > 1366 else P_):
-        pytest.skip("open axes longer than 1366 points take the O(n^2) transform: too slow for a test, H4 accuracy")
     nx, ny = shape
     cfg = film(nx, ny, bc)
     p, st, eps, B, s = setup_pair(cfg, with_pinning=False)

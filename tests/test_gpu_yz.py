@@ -61,6 +61,28 @@ def test_yz_one_step_fixed_sweeps(bc, host_loop):
     s.close()
 
 
+@pytest.mark.parametrize("bc", [(P_, P_, P_), (O_, O_, O_), (P_, O_, P_)])
+def test_yz_mu_refinement(bc):
+    """The fp64 residual of the mu refinement step (refine.cu) in the yz gauge: per-column U_y(i), U_z(i), jump in x.
+    A long thin mesh and a rough state, refinement forced on: mu meets the 2e-5 gate after one step."""
+    from paper_1409_8340_b200 import Solver
+    cfg = I.Config("yzr", 900, 6, 5, tuple(bc), Jx=0.02 if bc[0] == P_ else 0.0, seed=4)
+    psi0, mu0 = I.random_state(cfg, seed=6, amp=0.8)
+    K0 = 0.2 if bc[0] == P_ else 0.0
+    p = oracle_params(cfg)
+    By, Bz, _, _ = O.snap_field_yz(p, f32(0.05), f32(0.3))
+    st = O.State(psi=psi0.astype(np.complex128), mu=mu0.astype(np.float64), K=K0)
+    s = Solver(cfg.nx, cfg.ny, cfg.nz, bc=cfg.bc, h=cfg.h, dt=cfg.dt, fixed_sweeps=1, gauge_yz=True, mu_refine=True)
+    s.set_field_current(By=0.05, Bz=0.3, Jx=cfg.Jx)
+    s.set_state(torch.from_numpy(psi0), torch.from_numpy(mu0), K0)
+    s.step(1)
+    O.step(p, st, np.ones(p.shape), 0.0, Bz, f32(cfg.Jx), fixed_sweeps=1, links_fn=lambda K: O.paper_links_yz(p, K, By, Bz))
+    psi, mu = s.get_psi_mu()
+    assert np.max(np.abs(psi.cpu().numpy() - st.psi)) < 5e-6
+    assert np.max(np.abs(mu.cpu().numpy() - st.mu)) < 2e-5 * max(1.0, np.max(np.abs(st.mu)))
+    s.close()
+
+
 @pytest.mark.parametrize("shape", [(132, 37, 9), (260, 20, 12)])
 def test_yz_ragged_tiles_and_seams(shape):
     """Several tiles in x (the jump acts on the first and the last one only), ragged tiles in x and y."""
