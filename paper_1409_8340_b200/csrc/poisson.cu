@@ -357,6 +357,10 @@ void launch_dct_x(float *data, int n, int LB, long long nrows, const float2 *T, 
                   cudaStream_t st);
 void launch_dct_s(float *data, int n, int LB, long long stride, long long ostride, int ncolc, int nother,
                   const float2 *T, const float2 *C, const float2 *H, cudaStream_t st);
+// prime-factor DCT-I for the lengths that have a plan (dct_pfa.cu)
+void launch_dct_pfa_x(int kind, float *data, long long nrows, const unsigned short *tab, cudaStream_t st);
+void launch_dct_pfa_s(int kind, float *data, long long stride, long long ostride, int ncolc, int nother, const unsigned short *tab,
+                      cudaStream_t st);
 // register-blocked fast path (fft.cu)
 bool dht_fast_supported(int n);
 cudaError_t dht_fast_configure(int n);
@@ -420,6 +424,12 @@ static int transform_axis(const Dev &dv, float *data, int axis, bool divide, flo
   if (n == 1) return 0;                                   // a periodic axis of one point: the transform is the identity
   const bool open = bcs[axis] == 1;
   const long long plane = (long long)dv.nx * dv.ny;
+  if (open && dv.pfaK[axis] >= 0 && !divide) {
+    if (axis == 0) launch_dct_pfa_x(dv.pfaK[0], data, (long long)dv.ny * dv.nz, dv.pfaT[0], st);
+    else launch_dct_pfa_s(dv.pfaK[axis], data, axis == 1 ? dv.nx : plane, axis == 1 ? plane : dv.nx, dv.nx / 2,
+                          axis == 1 ? dv.nz : dv.ny, dv.pfaT[axis], st);
+    return 1;
+  }
   if (open && dv.bLB[axis] && !divide) {
     if (axis == 0) launch_dct_x(data, n, dv.bLB[0], (long long)dv.ny * dv.nz, dv.bT[0], dv.bC[0], dv.bH[0], st);
     else launch_dct_s(data, n, dv.bLB[axis], axis == 1 ? dv.nx : plane, axis == 1 ? plane : dv.nx, dv.nx / 2,

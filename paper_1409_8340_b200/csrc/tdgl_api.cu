@@ -20,6 +20,10 @@ int poisson_solve(const Dev &dv, float *data, bool thomas_open_z, cudaStream_t s
 int dct_fast_lb(int n);
 cudaError_t dct_fast_configure(int LB);
 void launch_build_bluestein(float2 *T, float2 *C, float2 *H, int n, int LB, cudaStream_t st);
+int dct_pfa_kind(int n);
+size_t dct_pfa_table_entries(int kind);
+void dct_pfa_build_table(int kind, bool xpass, unsigned short *host_out);
+cudaError_t dct_pfa_configure(int kind);
 void launch_init_state(const Dev &dv, float amp, cudaStream_t st);
 void launch_ctl_reset(const Dev &dv, float tol, int maxs, int fixed, cudaStream_t st);
 void launch_ctl_solver(const Dev &dv, float tol, int maxs, int fixed, cudaStream_t st);
@@ -185,6 +189,11 @@ static size_t carve(const tdgl_params *p, char *base, Dev *dv) {
     q = take(4096 * sizeof(float2)); if (dv) dv->bT[a] = (float2 *)q;
     q = take(4096 * sizeof(float2)); if (dv) dv->bC[a] = (float2 *)q;
     q = take(4096 * sizeof(float2)); if (dv) dv->bH[a] = (float2 *)q;
+    // open x / y axis whose length has a prime-factor DCT-I plan (open z is solved by the Thomas algorithm)
+    const bool open_xy = a < 2 && p->bc[a] == TDGL_BC_OPEN;
+    const int kind = open_xy ? dct_pfa_kind(ns[a]) : -1;
+    q = take(dct_pfa_table_entries(kind) * sizeof(unsigned short));
+    if (dv) { dv->pfaK[a] = kind; dv->pfaT[a] = kind >= 0 ? (const unsigned short *)q : nullptr; }
   }
   q = take((size_t)TDGL_NPART * 4 * sizeof(double)); if (dv) dv->part = (double *)q;
   {
@@ -363,6 +372,14 @@ extern "C" int tdgl_create(const tdgl_params *p, tdgl_t **out) {
   const double cs[3] = {cx, cy, cz};
   for (int a = 0; a < 3; ++a) launch_build_tables(dv.lam[a], dv.tw[a], dv.tab[a], ns[a], bcs[a], cs[a], st);
   for (int a = 0; a < 3; ++a) {
+    if (dv.pfaK[a] >= 0) {                          // prime-factor DCT-I: index tables built on the host
+      CKC(dct_pfa_configure(dv.pfaK[a]));
+      std::vector<unsigned short> tab(dct_pfa_table_entries(dv.pfaK[a]));
+      dct_pfa_build_table(dv.pfaK[a], a == 0, tab.data());
+      CKC(cudaMemcpyAsync((void *)dv.pfaT[a], tab.data(), tab.size() * sizeof(unsigned short), cudaMemcpyHostToDevice, st));
+      CKC(cudaStreamSynchronize(st));               // the host table dies at the end of this block
+      continue;
+    }
     dv.bLB[a] = (bcs[a] == TDGL_BC_OPEN) ? dct_fast_lb(ns[a]) : 0;
     if (dv.bLB[a]) {
       CKC(dct_fast_configure(dv.bLB[a]));
@@ -379,6 +396,7 @@ extern "C" int tdgl_create(const tdgl_params *p, tdgl_t **out) {
     q.lam[1] = dv.lam[2]; q.lam[2] = dv.lam[1];        // lam of the length-1 periodic axis is {0}
     q.tw[2] = dv.tw[1]; q.tab[2] = dv.tab[1];
     q.bT[2] = dv.bT[1]; q.bC[2] = dv.bC[1]; q.bH[2] = dv.bH[1]; q.bLB[2] = dv.bLB[1]; q.bLB[1] = 0;
+    q.pfaK[2] = dv.pfaK[1]; q.pfaT[2] = dv.pfaT[1]; q.pfaK[1] = -1; q.pfaT[1] = nullptr;
   }
   launch_init_state(dv, p->init_amp, st);
   launch_set_field(dv, 0.0, 0.0, 0.0, st);

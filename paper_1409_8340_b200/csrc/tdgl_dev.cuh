@@ -68,6 +68,8 @@ struct Dev {
   double *tab[3];           // generic transform tables: cas(2 pi m/n) or cos(pi m/(n-1))
   float2 *bT[3], *bC[3], *bH[3];   // Bluestein tables of the fast DCT-I per open axis (dct.cu)
   int bLB[3];               // its FFT length, 0 = axis not open / not supported
+  const unsigned short *pfaT[3];   // index tables of the prime-factor DCT-I per open axis (dct_pfa.cu)
+  int pfaK[3];              // its plan, -1 = none (the axis is periodic or its length has no plan)
   double *part;             // TDGL_NPART*4 partial sums
   double *jpart;            // one J_av partial sum per CTA of the marching kernels (in-tile x links of the new iterate)
   int *sweep_log; float *resid_log; int *sched;

@@ -133,10 +133,15 @@ def test_poisson_solve(bc, shape):
                                       ((P_, P_, O_), (128, 1024, 3)), ((P_, P_, P_), (1024, 64, 128)),
                                       ((P_, O_, P_), (64, 20, 256)), ((O_, P_, P_), (30, 512, 64)),
                                       ((O_, O_, O_), (1024, 40, 6)), ((P_, O_, O_), (64, 1000, 5)),
-                                      ((O_, O_, P_), (514, 300, 8)), ((O_, P_, O_), (1366, 64, 3))])
+                                      ((O_, O_, P_), (514, 300, 8)), ((O_, P_, O_), (1366, 64, 3)),
+                                      # prime-factor DCT-I (dct_pfa.cu): n = 1024, 256, 64 along x (rows) and y (columns),
+                                      # odd row counts, ragged column groups, film
+                                      ((O_, O_, P_), (64, 1024, 4)), ((O_, O_, O_), (256, 256, 8)), ((O_, P_, P_), (1024, 5, 3)),
+                                      ((P_, O_, O_), (36, 1024, 3)), ((O_, O_, P_), (1024, 64, 1)), ((P_, O_, P_), (70, 256, 5)),
+                                      ((O_, O_, O_), (1024, 1024, 4))])
 def test_poisson_solve_fast_transform_sizes(bc, shape):
     """The register-blocked Hartley kernels (n = 64..1024), x pass, strided pass and the fused
-    transform-divide-transform of a periodic z axis."""
+    transform-divide-transform of a periodic z axis; Bluestein and prime-factor DCT-I on open axes."""
     nx, ny, nz = shape
     cfg = cfg_of(nx, ny, nz, bc)
     p = oracle_params(cfg)
