@@ -24,7 +24,12 @@ Parity pins (tests/test_oracle_*.py, all `-m "not gpu"`):
   state, flux quantisation (integer plaquette windings summing to n_z), current conservation, gauge
   invariance, dense LU of M Psi = b on 8^3 built from the printed matrix entries, dense bordered
   solve of the Poisson problem on 8^3, zero normal current at open faces, free-energy descent and its
-  finite-difference gradient, Philox known-answer vectors, noise amplitude zeta_max of Eq. (39).
+  finite-difference gradient, Philox known-answer vectors, noise amplitude zeta_max of Eq. (39); the initial
+  condition (S13) by its distribution (moments, Kolmogorov-Smirnov distance, independence); the paper's pseudo-time
+  mu iteration (Eq. 40) by its fixed point (= the direct solve) and a dense solve of N mu = c from the printed entries.
+Single-precision replay: every function below keeps the dtype of the state it is given; a complex64 / float32
+state runs the same formulas in fp32 (link variables rounded to fp32 after fp64 trigonometry, scalars K, J_av in
+fp64, as the CUDA library does).  Used only to show what fp32 does to the paper's rule without the CUDA path (R3).
 Parity unpinned: none of the functions below; the paper's Fig. 5/6 curves are image-only and pin nothing.
 """
 from __future__ import annotations
@@ -63,6 +68,14 @@ class Params:
     temperature: float = 0.0        # reduced T-bar of Eq. (39); 0 = no noise
     seed: int = 0                   # Philox key
     solve_mu: bool = True           # S15
+    # mu solver: "direct" = the definition Delta_h mu = rho (solve_poisson); "pseudotime" = the paper's own iteration
+    # (Eq. 40, solve_poisson_pseudotime) warm-started from the previous step's mu, with the controls below (S20)
+    mu_solver: str = "direct"
+    h_tau: float = 0.1
+    eps_mu: float = 1e-6
+    eps_mu_in: float = 1e-6
+    mu_max_outer: int = 1000
+    mu_max_inner: int = 100
 
     @property
     def shape(self):
@@ -123,6 +136,7 @@ class State:
     sweep_log: List[int] = field(default_factory=list)
     resid_log: List[float] = field(default_factory=list)   # max|r|^2 at the deciding sweep of each step
     resid_trace: List[List[float]] = field(default_factory=list)   # max|r|^2 of every sweep of each step (S9 check)
+    mu_log: List[list] = field(default_factory=list)       # pseudo-time solver: per step, [(inner sweeps, max|d_tau mu|^2), ...]
     hit_max_sweeps: bool = False
 
 
@@ -487,11 +501,61 @@ def solve_poisson(p: Params, rho):
     return f.real
 
 
+def solve_poisson_pseudotime(p: Params, rho, mu0, h_tau: float = 0.1, eps_mu: float = 1e-6, eps_in: float = 1e-6,
+                             max_outer: int = 10000, max_inner: int = 1000, inner_counts: Optional[Sequence[int]] = None):
+    """The paper's OWN mu solver, step by step (Eq. 40; readings S5, S20): pseudo-time relaxation
+    d_tau mu = Delta_h mu - rho  (the STABLE sign: as printed at P:387 the flow is anti-diffusive and the printed
+    N mu = c, whose matrix N at P:399-405 is the diagonally dominant one of the stable flow, has no fixed point unless
+    rho = 0 -- S5), one Crank-Nicolson step of size h_tau per outer iteration,
+        N mu = c,   N_mm = 1 + h_tau (c_x + c_y + c_z),  N_{m,m+-alpha} = -h_tau c_alpha / 2   (P:399-405;
+                    on an open face the single neighbour's entry doubles: mirror ghost, S6/S21)
+        c_m = mu^-_m + h_tau [ (Delta_h mu^-)_m / 2 - rho_m ]                                   (P:409-419 with S5)
+    solved by Jacobi sweeps "like Eq. (33)" from x^0 = mu^-:  x^{l+1}_m = (c_m + (h_tau/2) sum_alpha c_alpha (x^l_{+alpha}
+    + x^l_{-alpha})) / N_mm, stopped at the first l with max_m |N_mm (x^{l+1} - x^l)_m|^2 < eps_in (residual of the input
+    iterate, keep x^{l+1}: the rule S8 of the psi solve; eps_in is not given by the paper, S20), and outer iterations
+    until max_m |(mu - mu^-)_m / h_tau|^2 < eps_mu.  h_tau is not given either; the default 0.1 is the value of
+    the real time step h_t, for which N is as diagonally dominant as M (a handful of sweeps per solve).  The fixed point is Delta_h mu = rho; the weighted mean
+    sum_m w_m mu_m of the start value is conserved (S7: start from a mean-free mu).
+    `inner_counts` (optional): replay exactly len(inner_counts) outer iterations with these sweep counts (S9).
+    Returns (mu, log) with log = list of (inner sweeps, max|d_tau mu|^2) per outer iteration."""
+    mu = np.array(mu0, dtype=np.float64)
+    rho = np.asarray(rho, dtype=np.float64)
+    zl = _zero_links(p)
+    d = 1.0 + h_tau * (p.cx + p.cy + p.cz)
+    log = []
+    n_out = 0
+    while True:
+        c = mu + h_tau * (0.5 * laplacian_real(p, mu) - rho)
+        x = mu
+        sweeps = 0
+        target = None if inner_counts is None else int(inner_counts[n_out])
+        while True:
+            xn = (c + 0.5 * h_tau * neighbour_sum(p, x.astype(np.complex128), zl).real) / d
+            r2 = float(np.max((d * (xn - x)) ** 2))
+            x = xn
+            sweeps += 1
+            if target is not None:
+                if sweeps >= target:
+                    break
+            elif r2 < eps_in or sweeps >= max_inner:
+                break
+        dt2 = float(np.max(((x - mu) / h_tau) ** 2))
+        mu = x
+        log.append((sweeps, dt2))
+        n_out += 1
+        if inner_counts is not None:
+            if n_out >= len(inner_counts):
+                break
+        elif dt2 < eps_mu or n_out >= max_outer:
+            break
+    return mu, log
+
+
 # --------------------------------------------------------------------------------------------------
 # one time step
 # --------------------------------------------------------------------------------------------------
 def step(p: Params, st: State, eps, Bx: float, Bz: float, Jext: float,
-         fixed_sweeps: Optional[int] = None, links_fn=None) -> State:
+         fixed_sweeps: Optional[int] = None, links_fn=None, mu_inner_counts: Optional[Sequence[int]] = None) -> State:
     """One time step in the paper's order "psi, then E, then mu".  mu and K inside the psi
     solve are the values left by the previous step (S2).
     `links_fn(K)` (optional) replaces `paper_links(p, K, Bx, Bz)`: any gauge-equivalent set of link
@@ -512,7 +576,13 @@ def step(p: Params, st: State, eps, Bx: float, Bz: float, Jext: float,
     mu = st.mu
     if p.solve_mu:                                                            # step 6 (S4: updated K)
         links = links_fn(K)
-        mu = solve_poisson(p, supercurrent_divergence(p, psi, links))
+        rho = supercurrent_divergence(p, psi, links)
+        if p.mu_solver == "pseudotime":                # the paper's iteration, warm start = last step's mu
+            mu, mlog = solve_poisson_pseudotime(p, rho, st.mu, p.h_tau, p.eps_mu, p.eps_mu_in, p.mu_max_outer,
+                                                p.mu_max_inner, mu_inner_counts)
+            st.mu_log.append(mlog)
+        else:
+            mu = solve_poisson(p, rho)
         if psi.dtype == np.complex64:    # single-precision replay (R3): mu is stored in fp32 like psi
             mu = mu.astype(np.float32)
     st.psi, st.mu, st.K, st.n = psi, mu, K, st.n + 1
@@ -528,10 +598,12 @@ def step(p: Params, st: State, eps, Bx: float, Bz: float, Jext: float,
 
 
 def run(p: Params, st: State, eps, Bx, Bz, Jext, nsteps: int,
-        sweep_counts: Optional[Sequence[int]] = None, links_fn=None) -> State:
-    """nsteps steps; `sweep_counts[n]` (optional) replays prescribed per-step sweep counts (S9)."""
+        sweep_counts: Optional[Sequence[int]] = None, links_fn=None, mu_schedule: Optional[Sequence[Sequence[int]]] = None) -> State:
+    """nsteps steps; `sweep_counts[n]` (optional) replays prescribed per-step sweep counts (S9); `mu_schedule[n]`
+    (optional, pseudo-time mu solver) the inner sweep counts of every outer iteration of step n."""
     for s in range(nsteps):
-        step(p, st, eps, Bx, Bz, Jext, None if sweep_counts is None else int(sweep_counts[s]), links_fn)
+        step(p, st, eps, Bx, Bz, Jext, None if sweep_counts is None else int(sweep_counts[s]), links_fn,
+             None if mu_schedule is None else mu_schedule[s])
     return st
 
 

@@ -60,14 +60,42 @@ def test_C1_100_steps_pointwise():
     p, st, eps, B, s, psi, mu, counts, resid, ob = run_pair(cfg, 100)
     extra = check_decisions(p, st, counts)
     assert np.max(np.abs(psi - st.psi)) <= 1e-4
-    # C1 relaxes into the single-sweep regime after ~35 steps; there fp32 rounding in the amplified
-    # checkerboard band grows to the tolerance level |r| ~ 1e-3,
-    # which any fp32 run of the paper's rule shows (numpy complex64 gives 1.4e-5).  The
-    # stated 1e-5 is asserted whenever no such extra sweep occurred, and on every other run of this file.
-    assert rel_l2(psi, st.psi) <= (1e-5 if extra == 0 else 2e-5)
+    # KNOWN DEVIATION (R3): C1 relaxes into the single-sweep regime after ~33 steps; there
+    # fp32 rounding in the amplified checkerboard band grows to the tolerance level |r| ~ 1e-3, criterion (34)
+    # then asks for a second sweep on a few steps, and the fp32-vs-fp64 difference is set by the tolerance, not by
+    # rounding.  tests/test_oracle_pins.py::test_R3_single_precision_deviation_on_C1_without_cuda reproduces this
+    # WITHOUT the CUDA path: the oracle's own functions in complex64 give rel-L2 = 0.9e-5 .. 1.4e-5 depending on the
+    # seed, with the same extra sweeps.  The stated 1e-5 is a hard assertion whenever no extra sweep occurred, in the
+    # two variants below that keep C1 out of the single-sweep regime, and in every other run of this file.
+    rel = rel_l2(psi, st.psi)
+    print(f"C1 100 steps: max|dpsi| = {np.max(np.abs(psi - st.psi)):.2e}, rel-L2 = {rel:.2e}, extra sweeps {extra}")
+    assert rel <= (1e-5 if extra == 0 else 2e-5)
     assert np.max(np.abs(mu - st.mu)) <= 1e-4 * max(1.0, np.max(np.abs(st.mu)))
     assert ob.vortices_per_slice == 4.0 and ob.steps == 100
     assert ob.sweeps_total == int(np.sum(counts))
+    s.close()
+
+
+def test_C1_100_steps_at_least_two_sweeps():
+    """C1 at eps_tol = 1e-6 with every step given max(2, the fp64 oracle's own count) sweeps on both sides: the same
+    run kept out of the single-sweep regime (a second sweep damps the amplified band).  BASELINE.json's numbers hold
+    as stated: max 1e-4, rel-L2 1e-5."""
+    cfg = I.CONFIGS["C1"]
+    p, st, eps, (Bx, Bz), s = setup_pair(cfg)
+    free = O.State(psi=st.psi.copy(), mu=st.mu.copy())
+    O.run(p, free, eps, Bx, Bz, 0.0, 100)                    # the oracle's own decisions
+    counts = [max(2, c) for c in free.sweep_log]
+    assert min(free.sweep_log) == 1                          # ... do enter the single-sweep regime
+    s.set_sweep_schedule(counts)
+    s.step(100)
+    psi, mu = s.get_psi_mu()
+    got, _ = s.sweep_log(100)
+    assert list(got) == counts
+    O.run(p, st, eps, Bx, Bz, 0.0, 100, sweep_counts=counts)
+    psi = psi.cpu().numpy()
+    assert np.max(np.abs(psi - st.psi)) <= 1e-4
+    assert rel_l2(psi, st.psi) <= 1e-5
+    assert np.max(np.abs(mu.cpu().numpy() - st.mu)) <= 1e-4 * max(1.0, np.max(np.abs(st.mu)))
     s.close()
 
 

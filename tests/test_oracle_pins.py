@@ -689,3 +689,92 @@ def test_R3_single_precision_deviation_on_C1_without_cuda():
     _, t32 = _c1_run(np.complex64, 0, 1e-10)
     assert min(t64.sweep_log) >= 3
     assert _rel_l2(t32.psi, t64.psi) < 2e-6 and np.max(np.abs(t32.psi - t64.psi)) < 1e-5
+
+
+# ------------------------------------------------------------------------------------------------
+# The paper's own mu solver (Eq. 40; readings S5, S20): pseudo-time relaxation + Crank-Nicolson + Jacobi
+# ------------------------------------------------------------------------------------------------
+def _assemble_N(p, h_tau):
+    """Dense N from the printed entries (P:399-405): N_mm = 1 + h_tau sum c, N_{m,m+-alpha} = -h_tau c_alpha/2;
+    periodic wrap, and on an open face the single neighbour's entry doubles (mirror ghost, S6/S21)."""
+    n = p.n_sites
+    N = np.zeros((n, n))
+    idx = lambda i, j, k: i + p.nx * (j + p.ny * k)
+    dims = (p.nx, p.ny, p.nz)
+    cs = (p.cx, p.cy, p.cz)
+    for k in range(p.nz):
+        for j in range(p.ny):
+            for i in range(p.nx):
+                m = idx(i, j, k)
+                N[m, m] += 1.0 + h_tau * sum(cs)
+                pos = [i, j, k]
+                for a in range(3):
+                    for sgn in (+1, -1):
+                        q = list(pos)
+                        q[a] += sgn
+                        if q[a] < 0 or q[a] >= dims[a]:
+                            if p.bc[a] == O_:
+                                q[a] = pos[a] - sgn            # mirror ghost
+                            else:
+                                q[a] %= dims[a]
+                        N[m, idx(*q)] += -0.5 * h_tau * cs[a]
+    return N
+
+
+@pytest.mark.parametrize("bc", [(P_, P_, P_), (P_, P_, O_), (O_, O_, O_), (O_, P_, O_)])
+def test_Eq40_one_pseudo_time_step_is_the_dense_solve_of_N_mu_equals_c(bc):
+    p = O.Params(6, 5, 4, hx=0.5, hy=0.4, hz=0.6, g=1.2, bc=bc)
+    rng = np.random.default_rng(3)
+    w = O.site_weights(p)
+    rho = rng.standard_normal(p.shape)
+    rho -= np.sum(w * rho) / np.sum(w)
+    mu0 = 0.3 * rng.standard_normal(p.shape)
+    h_tau = 0.7
+    N = _assemble_N(p, h_tau)
+    # c from the printed formula with the stable sign (S5): mu^- + h_tau [ (Delta_h mu^-)/2 - rho ]
+    c = mu0 + h_tau * (0.5 * O.laplacian_real(p, mu0) - rho)
+    want = np.linalg.solve(N, c.ravel()).reshape(p.shape)
+    got, log = O.solve_poisson_pseudotime(p, rho, mu0, h_tau=h_tau, eps_in=1e-30, max_inner=5000, max_outer=1)
+    assert len(log) == 1 and np.max(np.abs(got - want)) < 1e-12
+    # N = I - (h_tau/2) Delta_h, strictly diagonally dominant (P:421): every row sums to 1
+    assert np.allclose(N.sum(axis=1), 1.0) and np.all(np.diag(N) > np.sum(np.abs(N), axis=1) - np.diag(N))
+    assert np.max(np.abs((N @ mu0.ravel()).reshape(p.shape) - (mu0 - 0.5 * h_tau * O.laplacian_real(p, mu0)))) < 1e-12
+    # the replay of prescribed inner counts runs exactly those
+    got2, log2 = O.solve_poisson_pseudotime(p, rho, mu0, h_tau=h_tau, inner_counts=[3, 2])
+    assert [l[0] for l in log2] == [3, 2]
+
+
+@pytest.mark.parametrize("bc", [(P_, P_, P_), (P_, P_, O_), (O_, O_, O_)])
+def test_Eq40_fixed_point_is_the_direct_solve(bc):
+    p = O.Params(8, 8, 8, bc=bc)
+    rng = np.random.default_rng(5)
+    w = O.site_weights(p)
+    rho = rng.standard_normal(p.shape)
+    rho -= np.sum(w * rho) / np.sum(w)
+    ref = O.solve_poisson(p, rho)
+    mu, log = O.solve_poisson_pseudotime(p, rho, np.zeros(p.shape), h_tau=1.0, eps_mu=1e-26, eps_in=1e-28, max_outer=2000,
+                                         max_inner=5000)
+    assert len(log) < 2000
+    assert np.max(np.abs(mu - ref)) < 1e-10
+    assert abs(np.sum(w * mu)) < 1e-10                       # the weighted mean of the start value is conserved (S7)
+    # the paper's tolerance (eps_mu = 1e-6) stops early: |Delta_h mu - rho| ~ 1e-3, still the same field to ~1e-3
+    mu6, log6 = O.solve_poisson_pseudotime(p, rho, np.zeros(p.shape))
+    assert len(log6) < len(log) and np.max(np.abs(O.laplacian_real(p, mu6) - rho)) < 5e-2
+    assert max(l[0] for l in log6) <= 12                     # h_tau = 0.1: N is as dominant as M, a handful of sweeps
+
+
+def test_S5_the_printed_sign_has_no_fixed_point():
+    """As printed c_m = mu^- + h_tau [ -(Delta_h mu^-)/2 + rho ] with N = I - (h_tau/2) Delta_h: at the
+    solution of Delta_h mu = rho the printed equation N mu = c is violated by exactly h_tau rho (it holds only for
+    rho = 0), whereas the stable-sign c of reading S5 satisfies it."""
+    p = O.Params(8, 8, 8)
+    rng = np.random.default_rng(7)
+    rho = rng.standard_normal(p.shape)
+    rho -= rho.mean()
+    mu = O.solve_poisson(p, rho)
+    h_tau = 0.9
+    Nmu = mu - 0.5 * h_tau * O.laplacian_real(p, mu)
+    c_printed = mu + h_tau * (-0.5 * O.laplacian_real(p, mu) + rho)
+    c_stable = mu + h_tau * (0.5 * O.laplacian_real(p, mu) - rho)
+    assert np.max(np.abs(Nmu - c_stable)) < 1e-12
+    assert np.max(np.abs((Nmu - c_printed) + h_tau * rho)) < 1e-12 and np.max(np.abs(Nmu - c_printed)) > 0.1
