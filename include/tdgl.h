@@ -45,6 +45,13 @@ extern "C" {
 #define TDGL_FLAG_MU_REFINE   8u /* always run one step of iterative refinement after the mu solve (below)       */
 #define TDGL_FLAG_MU_NOREFINE 16u /* never run it.  Neither flag: automatic, iff tdgl_mu_gain() > TDGL_MU_REFINE_GAIN */
 #define TDGL_MU_REFINE_GAIN 200.0
+#define TDGL_FLAG_MU_ITERATIVE 32u /* solve mu by the paper's own iteration (Eq. 40: pseudo-time relaxation,
+                                   Crank-Nicolson, Jacobi; readings S5, S20) instead of the direct transform solver.
+                                   Host-driven loop.  Controls: tdgl_set_mu_solver.  Not with TDGL_FLAG_MU_REFINE. */
+#define TDGL_FLAG_FP64 64u      /* the DOUBLE-PRECISION build (the paper ships and times SP and DP):
+                                   psi, b, d, mu in double (104 B/site of workspace), every kernel of the step in fp64;
+                                   mu is solved by the pseudo-time iteration (the direct solver is fp32 only).  psi / mu
+                                   buffers of tdgl_get_psi_mu, tdgl_set_state, tdgl_debug_* are then double (pairs). */
 #define TDGL_FLAG_HOST_LOOP 2u  /* test/diagnostic: host-driven sweep loop instead of the CUDA-graph
                                    WHILE node (identical arithmetic)                                     */
 
@@ -142,6 +149,17 @@ int tdgl_last_cuda_error(const tdgl_t *h);
  * evaluated in fp64 from psi (fp64 link variables): one more stencil pass and one more solve per step, 4 more
  * bytes of workspace per site.  tdgl_mu_gain returns G for these params (host arithmetic only; -1 if invalid). */
 double tdgl_mu_gain(const tdgl_params *p_host);
+
+/* The pseudo-time mu iteration (TDGL_FLAG_MU_ITERATIVE / TDGL_FLAG_FP64 only; else TDGL_EINVAL).  Per time step, warm-started
+ * from the previous step's mu: outer iterations mu^- -> mu of one Crank-Nicolson step of d_tau mu = Delta_h mu - rho with
+ * virtual step h_tau, N mu = c (Eq. 40) by Jacobi sweeps until max|N_mm (x^{l+1} - x^l)|^2 < eps_in, until
+ * max|(mu - mu^-)/h_tau|^2 < eps_mu.  Defaults (S20): h_tau = 0.1, eps_mu = eps_in = 1e-6, max_outer = 1000,
+ * max_inner = 100. */
+int tdgl_set_mu_solver(tdgl_t *h, float h_tau, float eps_mu, float eps_in, int32_t max_outer, int32_t max_inner);
+/* Log of the last `nsolves` mu solves (one per time step): outer_host[s] = outer iterations of solve s (oldest first);
+ * inner_host = the Jacobi sweep counts of all those outer iterations in order (sum(outer_host) entries, at most
+ * inner_cap, else TDGL_ENOMEM); *n_inner_host = that number.  Host arrays, any may be NULL.  Synchronises the stream. */
+int tdgl_get_mu_log(tdgl_t *h, int32_t nsolves, int32_t *outer_host, int32_t *inner_host, int32_t inner_cap, int32_t *n_inner_host);
 int tdgl_mu_refine_enabled(const tdgl_t *h);      /* 1 / 0 */
 
 /* ---- extensions used by the tests and the bench (not part of the paper's problem statement) ---- */

@@ -13,12 +13,14 @@ _LIB_PATH = os.environ.get("TDGL_LIB") or os.path.join(_HERE, "libtdgl.so")     
 TDGL_OK, TDGL_EINVAL, TDGL_ENOMEM, TDGL_EINCOMPAT, TDGL_ECUDA, TDGL_WMAXSWEEPS = 0, -1, -2, -3, -4, 1
 TDGL_BC_PERIODIC, TDGL_BC_OPEN = 0, 1
 TDGL_FLAG_SOLVE_MU, TDGL_FLAG_HOST_LOOP, TDGL_FLAG_GAUGE_YZ, TDGL_FLAG_MU_REFINE, TDGL_FLAG_MU_NOREFINE = 1, 2, 4, 8, 16
+TDGL_FLAG_MU_ITERATIVE, TDGL_FLAG_FP64 = 32, 64
 
 EXPORTS = (
     "tdgl_workspace_bytes", "tdgl_create", "tdgl_destroy", "tdgl_set_pinning", "tdgl_set_field_current", "tdgl_step",
     "tdgl_get_psi_mu", "tdgl_observables", "tdgl_strerror", "tdgl_last_cuda_error", "tdgl_set_state", "tdgl_set_solver",
     "tdgl_set_sweep_schedule", "tdgl_get_sweep_log", "tdgl_get_eps", "tdgl_debug_noise", "tdgl_debug_poisson",
     "tdgl_debug_rho", "tdgl_launch_count", "tdgl_sweep_timing", "tdgl_mu_gain", "tdgl_mu_refine_enabled",
+    "tdgl_set_mu_solver", "tdgl_get_mu_log",
 )
 
 
@@ -91,6 +93,8 @@ def lib() -> C.CDLL:
     L.tdgl_mu_gain.restype = f64
     L.tdgl_mu_gain.argtypes = [C.POINTER(TdglParams)]
     L.tdgl_mu_refine_enabled.argtypes = [vp]
+    L.tdgl_set_mu_solver.argtypes = [vp, f32, f32, f32, i32, i32]
+    L.tdgl_get_mu_log.argtypes = [vp, i32, C.POINTER(i32), C.POINTER(i32), i32, C.POINTER(i32)]
     _lib = L
     return L
 
@@ -157,7 +161,7 @@ class Solver:
                  u: float = 1.0, g: float = 1.0, eps_tol: float = 1e-6, max_sweeps: int = 100, fixed_sweeps: int = 0,
                  temperature: float = 0.0, seed: int = 0, init_amp: float = 0.01, solve_mu: bool = True,
                  host_loop: bool = False, hxyz: Optional[Sequence[float]] = None, device: Optional[str] = None,
-                 gauge_yz: bool = False, mu_refine: Optional[bool] = None):
+                 gauge_yz: bool = False, mu_refine: Optional[bool] = None, mu_iterative: bool = False, fp64: bool = False):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1409_8340_b200 needs a CUDA device (sm_100a); there is no CPU path")
@@ -174,7 +178,9 @@ class Solver:
         p.temperature, p.seed, p.init_amp = temperature, seed, init_amp
         p.flags = ((TDGL_FLAG_SOLVE_MU if solve_mu else 0) | (TDGL_FLAG_HOST_LOOP if host_loop else 0)
                    | (TDGL_FLAG_GAUGE_YZ if gauge_yz else 0)
-                   | (0 if mu_refine is None else (TDGL_FLAG_MU_REFINE if mu_refine else TDGL_FLAG_MU_NOREFINE)))
+                   | (0 if mu_refine is None else (TDGL_FLAG_MU_REFINE if mu_refine else TDGL_FLAG_MU_NOREFINE))
+                   | (TDGL_FLAG_MU_ITERATIVE if mu_iterative else 0) | (TDGL_FLAG_FP64 if fp64 else 0))
+        self.fp64 = bool(fp64)
         nbytes = tdgl_workspace_bytes(p)
         if nbytes == 0:
             raise TdglError(TDGL_EINVAL, "tdgl_workspace_bytes")
@@ -208,10 +214,15 @@ class Solver:
     def step(self, n=1):
         tdgl_step(self.h, n)
 
+    @property
+    def real_dtype(self):
+        """torch dtype of the state the library holds: float32, or float64 with TDGL_FLAG_FP64."""
+        return self.torch.float64 if self.fp64 else self.torch.float32
+
     def get_psi_mu(self):
         t = self.torch
-        psi = t.empty(self.shape + (2,), dtype=t.float32, device=self.device)
-        mu = t.empty(self.shape, dtype=t.float32, device=self.device)
+        psi = t.empty(self.shape + (2,), dtype=self.real_dtype, device=self.device)
+        mu = t.empty(self.shape, dtype=self.real_dtype, device=self.device)
         tdgl_get_psi_mu(self.h, psi.data_ptr(), mu.data_ptr())
         return t.view_as_complex(psi), mu
 
@@ -221,11 +232,11 @@ class Solver:
     # extensions
     def set_state(self, psi, mu=None, K: float = 0.0):
         t = self.torch
-        psi = t.view_as_real(psi.to(self.device, t.complex64).contiguous())
+        psi = t.view_as_real(psi.to(self.device, t.complex128 if self.fp64 else t.complex64).contiguous())
         assert psi.numel() == 2 * self.n_sites
         mu_ptr = None
         if mu is not None:
-            mu = mu.to(self.device, t.float32).contiguous()
+            mu = mu.to(self.device, self.real_dtype).contiguous()
             assert mu.numel() == self.n_sites
             mu_ptr = mu.data_ptr()
         _check(lib().tdgl_set_state(self.h, psi.data_ptr(), mu_ptr, float(K)), "tdgl_set_state", self.h)
@@ -254,21 +265,41 @@ class Solver:
 
     def debug_noise(self, step: int):
         t = self.torch
-        z = t.empty(self.shape + (2,), dtype=t.float32, device=self.device)
+        z = t.empty(self.shape + (2,), dtype=self.real_dtype, device=self.device)
         _check(lib().tdgl_debug_noise(self.h, step, z.data_ptr()), "tdgl_debug_noise", self.h)
         return t.view_as_complex(z)
 
     def debug_poisson(self, rho):
         t = self.torch
-        mu = rho.to(self.device, t.float32).contiguous().clone()
+        mu = rho.to(self.device, self.real_dtype).contiguous().clone()
         _check(lib().tdgl_debug_poisson(self.h, mu.data_ptr(), mu.data_ptr()), "tdgl_debug_poisson", self.h)
         return mu
 
     def debug_rho(self):
         t = self.torch
-        rho = t.empty(self.shape, dtype=t.float32, device=self.device)
+        rho = t.empty(self.shape, dtype=self.real_dtype, device=self.device)
         _check(lib().tdgl_debug_rho(self.h, rho.data_ptr()), "tdgl_debug_rho", self.h)
         return rho
+
+    def set_mu_solver(self, h_tau: float = 0.1, eps_mu: float = 1e-6, eps_in: float = 1e-6, max_outer: int = 1000,
+                      max_inner: int = 100):
+        _check(lib().tdgl_set_mu_solver(self.h, h_tau, eps_mu, eps_in, max_outer, max_inner), "tdgl_set_mu_solver", self.h)
+
+    def mu_log(self, nsolves: int):
+        """(outer iterations per solve, list of per-solve lists of inner sweep counts) of the last nsolves mu solves."""
+        outer = np.zeros(nsolves, dtype=np.int32)
+        n_in = C.c_int32()
+        _check(lib().tdgl_get_mu_log(self.h, nsolves, outer.ctypes.data_as(C.POINTER(C.c_int32)), None, 0, C.byref(n_in)),
+               "tdgl_get_mu_log", self.h)
+        inner = np.zeros(max(1, n_in.value), dtype=np.int32)
+        _check(lib().tdgl_get_mu_log(self.h, nsolves, outer.ctypes.data_as(C.POINTER(C.c_int32)),
+                                     inner.ctypes.data_as(C.POINTER(C.c_int32)), len(inner), C.byref(n_in)),
+               "tdgl_get_mu_log", self.h)
+        out, pos = [], 0
+        for o in outer:
+            out.append([int(v) for v in inner[pos:pos + o]])
+            pos += o
+        return outer, out
 
     def mu_gain(self) -> float:
         return float(lib().tdgl_mu_gain(C.byref(self.params)))

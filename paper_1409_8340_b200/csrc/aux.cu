@@ -24,6 +24,10 @@ __global__ void k_ctl_reset(const __grid_constant__ Dev dv, float eps_tol, int m
   c->ticket = 0u; c->ticket2 = 0u;
   c->eps_tol = eps_tol; c->max_sweeps = max_sweeps; c->fixed_sweeps = fixed_sweeps;
   c->sched_n = 0; c->sched_pos = 0; c->Jext = 0.0; c->Bx = 0.0; c->Bz = 0.0;
+  c->h_tau = 0.1f; c->eps_mu = 1e-6f; c->eps_mu_in = 1e-6f; c->mu_max_outer = 1000; c->mu_max_inner = 100;   // S20
+  c->mu_inner = 0; c->mu_inner_done = 0; c->mu_outer = 0; c->mu_done = 0; c->mu_sched_n = 0; c->mu_sched_pos = 0;
+  c->mu_ticket = 0u; c->mu_r2bits = 0ull; c->mu_log_pos = 0; c->mu_solves = 0; c->mu_outer_total = 0; c->mu_inner_total = 0;
+  c->mu_dt2_last = 0.0;
 }
 __global__ void k_ctl_solver(const __grid_constant__ Dev dv, float eps_tol, int max_sweeps, int fixed_sweeps) {
   dv.ctl->eps_tol = eps_tol; dv.ctl->max_sweeps = max_sweeps; dv.ctl->fixed_sweeps = fixed_sweeps;
@@ -283,6 +287,7 @@ void launch_spheres(const Dev &dv, const float4 *sph, long long n, float eps_in,
 }
 void launch_copy_psi(const Dev &dv, float2 *out, cudaStream_t st) { k_copy_psi<<<grid_for(dv.N / 2, 256, 148 * 16), 256, 0, st>>>(dv, out); }
 void launch_noise(const Dev &dv, long long step, float2 *out, cudaStream_t st) { k_noise<<<grid_for(dv.N, 256, 148 * 16), 256, 0, st>>>(dv, step, out); }
+void launch_obs_final(const Dev &dv, int npart, cudaStream_t st) { k_obs_final<<<1, 256, 0, st>>>(dv, npart); }
 int launch_obs(const Dev &dv, cudaStream_t st) {
   const long long nblk = (long long)((dv.ny + OBS_RB - 1) / OBS_RB) * dv.nz;
   const int nb = (int)(nblk < TDGL_NPART ? nblk : TDGL_NPART);

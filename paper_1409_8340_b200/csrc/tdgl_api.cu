@@ -36,6 +36,22 @@ void launch_noise(const Dev &dv, long long step, float2 *out, cudaStream_t st);
 int launch_obs(const Dev &dv, cudaStream_t st);
 void launch_copy_psi(const Dev &dv, float2 *out, cudaStream_t st);
 void launch_mu_residual(const Dev &dv, const float *rho, const float *mu, float *out, cudaStream_t st);
+void launch_obs_final(const Dev &dv, int npart, cudaStream_t st);
+// plain.cu: double-precision build and the pseudo-time mu iteration
+void launch_march64(int mode, const Dev &dv, cudaStream_t st);
+int launch_jav64(const Dev &dv, cudaStream_t st);
+void launch_init_state64(const Dev &dv, double amp, cudaStream_t st);
+void launch_noise64(const Dev &dv, long long step, double2 *out, cudaStream_t st);
+void launch_copy_psi64(const Dev &dv, double2 *out, cudaStream_t st);
+int launch_obs64(const Dev &dv, cudaStream_t st);
+void launch_fill64(double *p, long long n, double v, cudaStream_t st);
+void launch_mu_begin(const Dev &dv, cudaStream_t st);
+void launch_mu_end(const Dev &dv, cudaStream_t st);
+void launch_mu_rhs(const Dev &dv, void *mu, cudaStream_t st);
+void launch_mu_sweep(const Dev &dv, void *mu, cudaStream_t st);
+void launch_mu_finish(const Dev &dv, void *mu, cudaStream_t st);
+void launch_mu_controls(const Dev &dv, float h_tau, float eps_mu, float eps_in, int max_outer, int max_inner, cudaStream_t st);
+void launch_mu_sched(const Dev &dv, int n, cudaStream_t st);
 void launch_mu_add(const Dev &dv, float *mu, const float *delta, cudaStream_t st);
 
 #define MODE_SWEEP 0
@@ -64,6 +80,7 @@ struct tdgl {
   // host loop
   int *h_flag;                 // pinned: [0] done, [1] sweeps
   int pred_sweeps;
+  int pred_mu_inner;           // pseudo-time mu iteration: predicted Jacobi sweeps per outer iteration
   // sweep timing
   bool timing;
   double t_ms;
@@ -120,6 +137,7 @@ static bool params_ok(const tdgl_params *p) {
       p->fixed_sweeps > TDGL_MAX_RESID_SLOTS) return false;
   if (!(p->temperature >= 0.f)) return false;
   if ((p->flags & TDGL_FLAG_GAUGE_YZ) && p->nz == 1) return false;          // films use the xz gauge
+  if ((p->flags & TDGL_FLAG_MU_REFINE) && (p->flags & (TDGL_FLAG_MU_ITERATIVE | TDGL_FLAG_FP64))) return false;
   return true;
 }
 
@@ -154,8 +172,13 @@ static double mu_gain(const tdgl_params *p) {
 }
 // Refinement of the mu solve: forced by TDGL_FLAG_MU_REFINE, suppressed by TDGL_FLAG_MU_NOREFINE, otherwise
 // automatic for meshes whose gain exceeds TDGL_MU_REFINE_GAIN (quasi-1D / thin long films; never the 3D BASELINE grids)
+static bool is_fp64(const tdgl_params *p) { return (p->flags & TDGL_FLAG_FP64) != 0; }
+// the pseudo-time iteration is the mu solver of the double-precision build (the direct solver is fp32 only)
+static bool is_mu_iterative(const tdgl_params *p) {
+  return (p->flags & TDGL_FLAG_SOLVE_MU) && (p->flags & (TDGL_FLAG_MU_ITERATIVE | TDGL_FLAG_FP64));
+}
 static bool want_refine(const tdgl_params *p) {
-  if (!(p->flags & TDGL_FLAG_SOLVE_MU) || (p->flags & TDGL_FLAG_MU_NOREFINE)) return false;
+  if (!(p->flags & TDGL_FLAG_SOLVE_MU) || (p->flags & TDGL_FLAG_MU_NOREFINE) || is_mu_iterative(p)) return false;
   if (p->flags & TDGL_FLAG_MU_REFINE) return true;
   return mu_gain(p) > TDGL_MU_REFINE_GAIN;
 }
@@ -204,14 +227,37 @@ static size_t carve(const tdgl_params *p, char *base, Dev *dv) {
   q = take(TDGL_LOGCAP * sizeof(int)); if (dv) dv->sweep_log = (int *)q;
   q = take(TDGL_LOGCAP * sizeof(float)); if (dv) dv->resid_log = (float *)q;
   q = take(TDGL_LOGCAP * sizeof(int)); if (dv) dv->sched = (int *)q;
-  q = take(N * sizeof(float2)); if (dv) dv->psi[0] = (float2 *)q;
-  q = take(N * sizeof(float2)); if (dv) dv->psi[1] = (float2 *)q;
-  q = take(N * sizeof(float2)); if (dv) dv->b = (float2 *)q;
-  q = take(N * sizeof(float2)); if (dv) dv->d = (float2 *)q;
-  q = take(N * sizeof(float)); if (dv) dv->mu = (float *)q;
-  q = take(N * sizeof(float)); if (dv) dv->eps = (float *)q;
-  q = take(N * sizeof(float)); if (dv) dv->scratch = (float *)q;
-  if (want_refine(p)) { q = take(N * sizeof(float)); if (dv) { dv->resid = (float *)q; dv->mu_refine = 1; } }
+  q = take(TDGL_MULOGCAP * sizeof(int)); if (dv) dv->mu_log = (int *)q;
+  q = take(TDGL_LOGCAP * sizeof(int)); if (dv) dv->mu_outer_log = (int *)q;
+  q = take(TDGL_LOGCAP * sizeof(int)); if (dv) dv->mu_sched = (int *)q;
+  const bool f64 = is_fp64(p), iter = is_mu_iterative(p);
+  if (f64) {                                   // double-precision state: 72 B/site + the iteration's 32 B/site
+    q = take(N * sizeof(double2)); if (dv) dv->psi64[0] = (double2 *)q;
+    q = take(N * sizeof(double2)); if (dv) dv->psi64[1] = (double2 *)q;
+    q = take(N * sizeof(double2)); if (dv) dv->b64 = (double2 *)q;
+    q = take(N * sizeof(double2)); if (dv) dv->d64 = (double2 *)q;
+    q = take(N * sizeof(double)); if (dv) dv->mu64 = (double *)q;
+    q = take(N * sizeof(float)); if (dv) dv->eps = (float *)q;
+    q = take(N * sizeof(float)); if (dv) dv->scratch = (float *)q;          // sphere list of tdgl_set_pinning
+  } else {
+    q = take(N * sizeof(float2)); if (dv) dv->psi[0] = (float2 *)q;
+    q = take(N * sizeof(float2)); if (dv) dv->psi[1] = (float2 *)q;
+    q = take(N * sizeof(float2)); if (dv) dv->b = (float2 *)q;
+    q = take(N * sizeof(float2)); if (dv) dv->d = (float2 *)q;
+    q = take(N * sizeof(float)); if (dv) dv->mu = (float *)q;
+    q = take(N * sizeof(float)); if (dv) dv->eps = (float *)q;
+    q = take(N * sizeof(float)); if (dv) dv->scratch = (float *)q;
+    if (want_refine(p)) { q = take(N * sizeof(float)); if (dv) { dv->resid = (float *)q; dv->mu_refine = 1; } }
+  }
+  if (iter) {                                  // rho, c and the two Jacobi iterates of Eq. (40)
+    const size_t es = f64 ? sizeof(double) : sizeof(float);
+    q = take(N * es); if (dv) dv->mu_rho = q;
+    q = take(N * es); if (dv) dv->mu_c = q;
+    q = take(N * es); if (dv) dv->mu_xa = q;
+    q = take(N * es); if (dv) dv->mu_xb = q;
+    if (dv) dv->mu_iterative = 1;
+  }
+  if (dv) dv->fp64 = f64 ? 1 : 0;
   return off;
 }
 
@@ -228,19 +274,64 @@ extern "C" uint64_t tdgl_workspace_bytes(const tdgl_params *p) {
 }
 
 static void march(tdgl_t *h, int mode, const Dev &dv, cudaStream_t st) {
-  if (h->film) launch_march_film(mode, dv, h->mgrid, st);
+  if (dv.fp64) launch_march64(mode, dv, st);
+  else if (h->film) launch_march_film(mode, dv, h->mgrid, st);
   else launch_march_tma(mode, dv, h->maps, h->mgrid, st);
+}
+
+// One solve of the paper's pseudo-time mu iteration (Eq. 40; plain.cu), host-driven: per outer iteration the right side c,
+// Jacobi sweeps until the device-side inner test passes (speculative launches return at once when it has), the outer
+// update and test.  `mu` holds mu^- (warm start) and receives mu; rho is in dv.mu_rho.  Two 8-byte flag reads per outer
+// iteration.  Returns the launches made, or -1 on a CUDA error.
+static int mu_iterative_solve(tdgl_t *h, void *mu) {
+  cudaStream_t st = h->stream;
+  const Dev &dv = h->dv;
+  int n = 0;
+  launch_mu_begin(dv, st); ++n;
+  for (;;) {
+    launch_mu_rhs(dv, mu, st); ++n;
+    int launched = 0;
+    for (;;) {
+      int burst = h->pred_mu_inner - launched;
+      if (burst < 1) burst = 1;
+      for (int s = 0; s < burst; ++s) { launch_mu_sweep(dv, mu, st); ++launched; ++n; }
+      if (cudaMemcpyAsync(h->h_flag + 8, &dv.ctl->mu_inner, 2 * sizeof(int), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+          cudaStreamSynchronize(st) != cudaSuccess) return -1;
+      if (h->h_flag[9]) break;
+    }
+    h->pred_mu_inner = h->h_flag[8] < 1 ? 1 : h->h_flag[8];
+    launch_mu_finish(dv, mu, st); ++n;
+    if (cudaMemcpyAsync(h->h_flag + 10, &dv.ctl->mu_done, sizeof(int), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+        cudaStreamSynchronize(st) != cudaSuccess) return -1;
+    if (h->h_flag[10]) break;
+  }
+  launch_mu_end(dv, st); ++n;
+  return n;
 }
 
 // the kernels of one step after the psi solve: J_av + K (a5), rho (a6), mu (a7)
 static int enqueue_after_solve(tdgl_t *h, cudaStream_t st) {
   int n = 0;
   const bool kact = h->dv.solve_mu && h->dv.bcx == 0;
-  // J_av: the in-tile x links were summed by the last sweep (one partial per CTA); the links that cross a
-  // tile edge are summed here
-  if (kact) { launch_jav_edges(h->dv, march_tma_tile_w(), h->jav_blocks, st); ++n; }
-  launch_step_finish(h->dv, (int)(h->mgrid.x * h->mgrid.y * h->mgrid.z), h->jav_blocks, st); ++n;
-  if (h->dv.solve_mu) {
+  if (h->dv.fp64) {
+    // double-precision build: J_av by its own pass over all x links (fp64 partials in dv.part)
+    int np = 0;
+    if (kact) { np = launch_jav64(h->dv, st); ++n; }
+    launch_step_finish(h->dv, 0, np, st); ++n;
+  } else {
+    // J_av: the in-tile x links were summed by the last sweep (one partial per CTA); the links that cross a
+    // tile edge are summed here
+    if (kact) { launch_jav_edges(h->dv, march_tma_tile_w(), h->jav_blocks, st); ++n; }
+    launch_step_finish(h->dv, (int)(h->mgrid.x * h->mgrid.y * h->mgrid.z), h->jav_blocks, st); ++n;
+  }
+  if (h->dv.solve_mu && h->dv.mu_iterative) {
+    Dev d2 = h->dv;                               // the rho kernel writes where "mu" points: into the iteration's rho array
+    d2.mu = (float *)h->dv.mu_rho; d2.mu64 = (double *)h->dv.mu_rho;
+    march(h, MODE_RHO, d2, st); ++n;
+    const int m = mu_iterative_solve(h, h->dv.fp64 ? (void *)h->dv.mu64 : (void *)h->dv.mu);
+    if (m < 0) return -1;
+    n += m;
+  } else if (h->dv.solve_mu) {
     march(h, MODE_RHO, h->dv, st); ++n;
     n += poisson_solve(h->dvp, h->dv.mu, true, st);
     if (h->dv.mu_refine) {                       // mu += S(rho_64 - Delta_h mu)  (refine.cu)
@@ -345,6 +436,13 @@ extern "C" int tdgl_create(const tdgl_params *p, tdgl_t **out) {
   dv.seed_hi = (unsigned)(p->seed >> 32);
   dv.solve_mu = (p->flags & TDGL_FLAG_SOLVE_MU) ? 1 : 0;
   dv.gauge_yz = (p->flags & TDGL_FLAG_GAUGE_YZ) ? 1 : 0;
+  // the same constants in double, from the fp32 values that crossed the ABI widened (R2): what the fp64 oracle uses
+  dv.cx64 = cx; dv.cy64 = cy; dv.cz64 = cz;
+  dv.csum2_64 = 2.0 * (cx + cy + cz);
+  dv.ht2_64 = 0.5 * ((double)p->dt / (double)p->u);
+  dv.u64 = (double)p->u;
+  dv.zeta_max64 = p->temperature > 0.f ? std::sqrt(3.0 * (double)p->temperature * (double)p->u /
+                                                   (2.0 * dv.dt * dv.hx * dv.hy * (film ? 1.0 : dv.hz))) : 0.0;
 
   {
     unsigned gx, gy, gz; int zc;
@@ -354,7 +452,10 @@ extern "C" int tdgl_create(const tdgl_params *p, tdgl_t **out) {
   }
   h->jav_blocks = jav_edge_blocks(dv, march_tma_tile_w());
   h->pred_sweeps = 1;
-  if (film) {
+  h->pred_mu_inner = 1;
+  if (dv.fp64) {
+    // plain kernels: nothing to configure
+  } else if (film) {
     CKC(march_film_configure());
   } else {
     CKC(march_tma_configure());
@@ -398,12 +499,14 @@ extern "C" int tdgl_create(const tdgl_params *p, tdgl_t **out) {
     q.bT[2] = dv.bT[1]; q.bC[2] = dv.bC[1]; q.bH[2] = dv.bH[1]; q.bLB[2] = dv.bLB[1]; q.bLB[1] = 0;
     q.pfaK[2] = dv.pfaK[1]; q.pfaT[2] = dv.pfaT[1]; q.pfaK[1] = -1; q.pfaT[1] = nullptr;
   }
-  launch_init_state(dv, p->init_amp, st);
+  if (dv.fp64) launch_init_state64(dv, (double)p->init_amp, st);
+  else launch_init_state(dv, p->init_amp, st);
   launch_set_field(dv, 0.0, 0.0, 0.0, st);
   launch_step_begin(dv, st);
   h->launches += 7;
   CKCL();
-  h->use_graph = !(p->flags & TDGL_FLAG_HOST_LOOP);
+  // the pseudo-time mu iteration has two nested data-dependent loops: it is driven from the host
+  h->use_graph = !(p->flags & TDGL_FLAG_HOST_LOOP) && !dv.mu_iterative && !dv.fp64;
   if (h->use_graph) {
     int rc = build_graph(h);
     if (rc != TDGL_OK) { tdgl_destroy(h); return rc; }
@@ -502,7 +605,11 @@ static int step_host_loop(tdgl_t *h) {
     }
   }
   h->pred_sweeps = h->h_flag[0] < 1 ? 1 : h->h_flag[0];
-  h->launches += enqueue_after_solve(h, st);
+  {
+    const int m = enqueue_after_solve(h, st);
+    if (m < 0) return cuda_fail(h, cudaGetLastError());
+    h->launches += m;
+  }
   CKL();
   return TDGL_OK;
 }
@@ -523,6 +630,11 @@ extern "C" int tdgl_step(tdgl_t *h, int32_t nsteps) {
 
 extern "C" int tdgl_get_psi_mu(tdgl_t *h, void *psi_dev, void *mu_dev) {
   if (!h || ((uintptr_t)psi_dev & 15)) return TDGL_EINVAL;
+  if (h->dv.fp64) {                                 // double-precision build: N double pairs / N doubles
+    if (psi_dev) { launch_copy_psi64(h->dv, (double2 *)psi_dev, h->stream); h->launches += 1; CKL(); }
+    if (mu_dev) CK(cudaMemcpyAsync(mu_dev, h->dv.mu64, (size_t)h->dv.N * sizeof(double), cudaMemcpyDeviceToDevice, h->stream));
+    return TDGL_OK;
+  }
   if (psi_dev) {
     // which buffer holds psi is device state (ctl->xbuf): the copy kernel reads it on the device
     launch_copy_psi(h->dv, (float2 *)psi_dev, h->stream);
@@ -535,7 +647,8 @@ extern "C" int tdgl_get_psi_mu(tdgl_t *h, void *psi_dev, void *mu_dev) {
 
 extern "C" int tdgl_observables(tdgl_t *h, tdgl_obs *out) {
   if (!h || !out) return TDGL_EINVAL;
-  h->launches += launch_obs(h->dv, h->stream);
+  if (h->dv.fp64) { launch_obs_final(h->dv, launch_obs64(h->dv, h->stream), h->stream); h->launches += 2; }
+  else h->launches += launch_obs(h->dv, h->stream);
   CKL();
   Ctl c;
   CK(cudaMemcpyAsync(&c, h->dv.ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, h->stream));
@@ -566,13 +679,54 @@ extern "C" const char *tdgl_strerror(int code) {
   }
 }
 extern "C" int tdgl_last_cuda_error(const tdgl_t *h) { return h ? h->last_cuda : 0; }
+extern "C" int tdgl_set_mu_solver(tdgl_t *h, float h_tau, float eps_mu, float eps_in, int32_t max_outer, int32_t max_inner) {
+  if (!h || !h->dv.mu_iterative || !(h_tau > 0.f) || !(eps_mu >= 0.f) || !(eps_in >= 0.f) || max_outer < 1 || max_inner < 1) return TDGL_EINVAL;
+  launch_mu_controls(h->dv, h_tau, eps_mu, eps_in, max_outer, max_inner, h->stream);
+  h->launches += 1;
+  CKL();
+  return TDGL_OK;
+}
+
+extern "C" int tdgl_get_mu_log(tdgl_t *h, int32_t nsolves, int32_t *outer_host, int32_t *inner_host, int32_t inner_cap,
+                               int32_t *n_inner_host) {
+  if (!h || !h->dv.mu_iterative || nsolves < 0 || nsolves > TDGL_LOGCAP || inner_cap < 0) return TDGL_EINVAL;
+  Ctl c;
+  CK(cudaMemcpyAsync(&c, h->dv.ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, h->stream));
+  CK(cudaStreamSynchronize(h->stream));
+  if (nsolves > c.mu_solves) return TDGL_EINVAL;
+  std::vector<int> lo(TDGL_LOGCAP);
+  CK(cudaMemcpyAsync(lo.data(), h->dv.mu_outer_log, TDGL_LOGCAP * sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+  CK(cudaStreamSynchronize(h->stream));
+  long long total = 0;
+  for (int s = 0; s < nsolves; ++s) {
+    const int o = lo[(c.mu_solves - nsolves + s) % TDGL_LOGCAP];
+    if (outer_host) outer_host[s] = o;
+    total += o;
+  }
+  if (n_inner_host) *n_inner_host = (int32_t)total;
+  if (total > TDGL_MULOGCAP) return TDGL_EINVAL;
+  if (inner_host) {
+    if (total > inner_cap) return TDGL_ENOMEM;
+    std::vector<int> li(TDGL_MULOGCAP);
+    CK(cudaMemcpyAsync(li.data(), h->dv.mu_log, (size_t)TDGL_MULOGCAP * sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
+    for (long long q = 0; q < total; ++q) inner_host[q] = li[(c.mu_log_pos - total + q) % TDGL_MULOGCAP];
+  }
+  return TDGL_OK;
+}
+
 extern "C" double tdgl_mu_gain(const tdgl_params *p) { return params_ok(p) ? mu_gain(p) : -1.0; }
 extern "C" int tdgl_mu_refine_enabled(const tdgl_t *h) { return h ? h->dv.mu_refine : TDGL_EINVAL; }
 
 extern "C" int tdgl_set_state(tdgl_t *h, const void *psi_dev, const void *mu_dev, double K) {
   if (!h || !psi_dev) return TDGL_EINVAL;
-  CK(cudaMemcpyAsync(h->dv.psi[0], psi_dev, (size_t)h->dv.N * sizeof(float2), cudaMemcpyDeviceToDevice, h->stream));
-  if (mu_dev) CK(cudaMemcpyAsync(h->dv.mu, mu_dev, (size_t)h->dv.N * sizeof(float), cudaMemcpyDeviceToDevice, h->stream));
+  if (h->dv.fp64) {
+    CK(cudaMemcpyAsync(h->dv.psi64[0], psi_dev, (size_t)h->dv.N * sizeof(double2), cudaMemcpyDeviceToDevice, h->stream));
+    if (mu_dev) CK(cudaMemcpyAsync(h->dv.mu64, mu_dev, (size_t)h->dv.N * sizeof(double), cudaMemcpyDeviceToDevice, h->stream));
+  } else {
+    CK(cudaMemcpyAsync(h->dv.psi[0], psi_dev, (size_t)h->dv.N * sizeof(float2), cudaMemcpyDeviceToDevice, h->stream));
+    if (mu_dev) CK(cudaMemcpyAsync(h->dv.mu, mu_dev, (size_t)h->dv.N * sizeof(float), cudaMemcpyDeviceToDevice, h->stream));
+  }
   launch_ctl_state(h->dv, K, h->stream);
   launch_step_begin(h->dv, h->stream);
   h->launches += 2;
@@ -631,7 +785,8 @@ extern "C" int tdgl_get_eps(tdgl_t *h, void *eps_dev) {
 
 extern "C" int tdgl_debug_noise(tdgl_t *h, int64_t step, void *zeta_dev) {
   if (!h || !zeta_dev) return TDGL_EINVAL;
-  launch_noise(h->dv, step, (float2 *)zeta_dev, h->stream);
+  if (h->dv.fp64) launch_noise64(h->dv, step, (double2 *)zeta_dev, h->stream);
+  else launch_noise(h->dv, step, (float2 *)zeta_dev, h->stream);
   h->launches += 1;
   CKL();
   return TDGL_OK;
@@ -639,6 +794,16 @@ extern "C" int tdgl_debug_noise(tdgl_t *h, int64_t step, void *zeta_dev) {
 
 extern "C" int tdgl_debug_poisson(tdgl_t *h, const void *rho_dev, void *mu_dev) {
   if (!h || !rho_dev || !mu_dev) return TDGL_EINVAL;
+  if (h->dv.mu_iterative) {                       // the pseudo-time iteration from mu = 0 on the given rho
+    const size_t es = h->dv.fp64 ? sizeof(double) : sizeof(float);
+    CK(cudaMemcpyAsync(h->dv.mu_rho, rho_dev, (size_t)h->dv.N * es, cudaMemcpyDeviceToDevice, h->stream));
+    CK(cudaMemsetAsync(mu_dev, 0, (size_t)h->dv.N * es, h->stream));
+    const int m = mu_iterative_solve(h, mu_dev);
+    if (m < 0) return cuda_fail(h, cudaGetLastError());
+    h->launches += m;
+    CKL();
+    return TDGL_OK;
+  }
   if (h->dv.mu_refine)                            // keep rho: the residual needs it after the in-place solve
     CK(cudaMemcpyAsync(h->dv.resid, rho_dev, (size_t)h->dv.N * sizeof(float), cudaMemcpyDeviceToDevice, h->stream));
   if (rho_dev != mu_dev)
@@ -657,6 +822,7 @@ extern "C" int tdgl_debug_rho(tdgl_t *h, void *rho_dev) {
   if (!h || !rho_dev) return TDGL_EINVAL;
   Dev d2 = h->dv;
   d2.mu = (float *)rho_dev;                       // the rho kernel writes where mu lives
+  d2.mu64 = (double *)rho_dev;
   march(h, MODE_RHO, d2, h->stream);
   h->launches += 1;
   CKL();

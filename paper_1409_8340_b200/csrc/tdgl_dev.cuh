@@ -7,6 +7,7 @@
 #define TDGL_LOGCAP 65536            // ring of per-step sweep counts / residuals
 #define TDGL_MAX_RESID_SLOTS 1024    // >= max_sweeps
 #define TDGL_NPART 2048              // partial sums of the two-stage fp64 reductions
+#define TDGL_MULOGCAP (1 << 18)      // ring of inner sweep counts of the pseudo-time mu iteration (one entry per outer iteration)
 
 // Control block, resident in the workspace; written by kernels only (the host reads it back).
 struct Ctl {
@@ -33,6 +34,15 @@ struct Ctl {
   double Bx, Bz;            // effective field
   unsigned int resid_bits[TDGL_MAX_RESID_SLOTS];   // max |r|^2 of sweep l as uint bits (>= 0 floats order like uints)
   double obs[8];            // observables scratch
+  // the paper's pseudo-time mu iteration (plain.cu; Eq. 40): controls, loop state, statistics
+  float h_tau, eps_mu, eps_mu_in;
+  int mu_max_outer, mu_max_inner;
+  int mu_inner, mu_inner_done, mu_outer, mu_done;
+  int mu_sched_n, mu_sched_pos;
+  unsigned int mu_ticket;
+  unsigned long long mu_r2bits;
+  long long mu_log_pos, mu_solves, mu_outer_total, mu_inner_total;
+  double mu_dt2_last;
 };
 
 struct Dev {
@@ -73,6 +83,15 @@ struct Dev {
   double *part;             // TDGL_NPART*4 partial sums
   double *jpart;            // one J_av partial sum per CTA of the marching kernels (in-tile x links of the new iterate)
   int *sweep_log; float *resid_log; int *sched;
+  // double-precision build (TDGL_FLAG_FP64, plain.cu): the state in double, constants in double
+  int fp64;
+  double2 *psi64[2], *b64, *d64;
+  double *mu64;
+  double cx64, cy64, cz64, csum2_64, ht2_64, u64, zeta_max64;
+  // pseudo-time mu iteration (TDGL_FLAG_MU_ITERATIVE): rho, c, two Jacobi iterates (float or double), logs
+  int mu_iterative;
+  void *mu_rho, *mu_c, *mu_xa, *mu_xb;
+  int *mu_log, *mu_outer_log, *mu_sched;
   unsigned long long cond_handle;   // cudaGraphConditionalHandle of the WHILE node (graph mode)
   int use_cond;
 };
