@@ -143,11 +143,11 @@ def config_dict(cfg: I.Config, world: int = 1):
             "loop": "CUDA graph per step, WHILE node around the sweep, no host sync"}
 
 
-def make_solver(cfg: I.Config, host_loop=False, seed_offset=0):
+def make_solver(cfg: I.Config, host_loop=False, seed_offset=0, fp64=False, mu_iterative=False):
     from paper_1409_8340_b200 import Solver
     s = Solver(cfg.nx, cfg.ny, cfg.nz, bc=cfg.bc, h=cfg.h, dt=cfg.dt, eps_tol=1e-6, max_sweeps=100,
                temperature=cfg.temperature, seed=replica_seed(cfg, seed_offset), init_amp=cfg.init_amp, solve_mu=True,
-               host_loop=host_loop)
+               host_loop=host_loop, fp64=fp64, mu_iterative=mu_iterative)
     s.set_pinning(I.sphere_list(cfg), cfg.eps_in, cfg.eps_out)
     bx, bz = cfg.requested_field()
     s.set_field_current(Bx=bx, Bz=bz, Jx=cfg.Jx)
@@ -253,6 +253,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--fp64", action="store_true", help="the double-precision build (TDGL_FLAG_FP64; the paper's DP mode)")
+    ap.add_argument("--mu-iterative", action="store_true", help="the paper's own pseudo-time mu solver (TDGL_FLAG_MU_ITERATIVE)")
+    ap.add_argument("--h-tau", type=float, default=0.1, help="virtual time step of the pseudo-time mu solver (S20)")
     args = ap.parse_args()
     cfg = I.CONFIGS[args.config]
     if args.impl == "reference":
@@ -282,7 +285,11 @@ def main():
             torch.cuda.synchronize()
 
     # ---- resident run (graph mode) --------------------------------------------------------------
-    s = make_solver(cfg, seed_offset=rank)
+    mode = dict(fp64=args.fp64, mu_iterative=args.mu_iterative)
+    bytes_per_site = SWEEP_BYTES_PER_SITE * (2.0 if args.fp64 else 1.0)
+    s = make_solver(cfg, seed_offset=rank, **mode)
+    if args.fp64 or args.mu_iterative:
+        s.set_mu_solver(h_tau=args.h_tau)
     s.step(W)
     barrier()
     ob0 = s.observables()
@@ -298,6 +305,10 @@ def main():
     ms = e0.elapsed_time(e1)
     clocks = sampler.stop()
     ob1 = s.observables()
+    mu_stats = None
+    if args.fp64 or args.mu_iterative:
+        outer, inner = s.mu_log(min(K, 1000))
+        mu_stats = {"outer_per_step": float(np.mean(outer)), "inner_per_outer": float(np.mean([np.mean(i) for i in inner if i]))}
     launches = s.launch_count() - l0 - 2           # minus the two observables kernels
     sweeps = ob1.sweeps_total - ob0.sweeps_total
     ms, sweeps_all, launches_all = reduce_over_ranks([ms, sweeps, launches], dist if world > 1 else None, dev)
@@ -311,7 +322,9 @@ def main():
     if rank == 0 or world > 1:
         psi, mu = s.get_psi_mu()
         K0 = s.observables().K
-        sh = make_solver(cfg, host_loop=True, seed_offset=rank)
+        sh = make_solver(cfg, host_loop=True, seed_offset=rank, **mode)
+        if args.fp64 or args.mu_iterative:
+            sh.set_mu_solver(h_tau=args.h_tau)
         sh.set_state(psi, mu, K0)
         sh.step(3)
         sh.sweep_timing(True)
@@ -320,16 +333,16 @@ def main():
         peak, how = measured_peak()
         if n_l > 0:
             avg_ms = t_ms / n_l
-            ach = SWEEP_BYTES_PER_SITE * N / (avg_ms * 1e-3) / 1e9
+            ach = bytes_per_site * N / (avg_ms * 1e-3) / 1e9
             tr = ncu_traffic()
-            kname = "k_march_film<SWEEP>" if cfg.nz == 1 else "k_march_tma<SWEEP>"
+            kname = "k_march64<SWEEP>" if args.fp64 else ("k_march_film<SWEEP>" if cfg.nz == 1 else "k_march_tma<SWEEP>")
             roof = {"bound": "hbm", "kernel": kname + " (Jacobi sweep + max-residual)", "achieved": ach,
                     "peak": peak, "unit": "GB/s", "frac": ach / peak, "peak_source": how,
                     "avg_launch_ms": avg_ms, "launches_timed": int(n_l),
-                    "algorithmic_bytes_per_launch": SWEEP_BYTES_PER_SITE * N,
+                    "algorithmic_bytes_per_launch": bytes_per_site * N,
                     "timed_in": "host-loop mode (TDGL_FLAG_HOST_LOOP): CUDA events around each single sweep launch after a "
                                 "stream sync; `value` is timed in graph mode, where launches overlap their predecessors' tails",
-                    "traffic": (tr or {}).get("dram_bytes_per_launch") if (tr or {}).get("sites") == N else None,
+                    "traffic": (tr or {}).get("dram_bytes_per_launch") if ((tr or {}).get("sites") == N and not args.fp64) else None,
                     "traffic_source": "profiles/sweep_traffic.txt (dram__bytes_read.sum + dram__bytes_write.sum of one committed "
                                       "ncu --set full capture of this kernel on this grid; not measured in this run)"}
         sh.close()
@@ -342,7 +355,7 @@ def main():
             hm = mu.cpu().pin_memory()
             dp = torch.empty_like(torch.view_as_real(psi))
             dm = torch.empty_like(mu)
-            h2d = hp.numel() * 4 + hm.numel() * 4
+            h2d = hp.numel() * hp.element_size() + hm.numel() * hm.element_size()
             d2h = h2d + 136
             obx = s.observables()
             for it in range(2 + Ke):
@@ -377,9 +390,10 @@ def main():
     out = {
         "metric": METRIC if args.config == "C4" else METRIC.replace("512x512x256", "%dx%dx%d" % (cfg.nx, cfg.ny, cfg.nz)),
         "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
-        "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64" if args.fp64 else "f32",
         "data": "synthetic", "steps_per_s": steps_per_s, "sweeps_per_step": sweeps_all / (K * world),
-        "config": config_dict(cfg, world),
+        "config": dict(config_dict(cfg, world), **({"mu_solver": "pseudo-time iteration (Eq. 40), host-driven loop"} if (args.fp64 or args.mu_iterative) else {})),
+        "mu_iteration": mu_stats,
         "clocks": clocks, "e2e": e2e, "gpu_launches": launches_all, "roofline": roof, "cpu_baseline": cpu,
         "state": {"mean_abs2": ob1.mean_abs2, "Ex": ob1.Ex, "K": ob1.K, "vortices_per_slice": ob1.vortices_per_slice,
                   "status": ob1.status},

@@ -84,6 +84,19 @@ __device__ __forceinline__ cd neighbour_sum(const Dev &dv, const double2 *__rest
   return acc;
 }
 
+// Launch geometry of the one-thread-per-site kernels: 128 threads along x; a CTA walks a chunk of PLAIN_CH sites along
+// the slowest axis that has an extent (z; y for a film), so that a 67 M-site grid launches 32 k CTAs, not 524 k: every
+// CTA ends with two atomics on the same two words (max residual, ticket), which serialise in L2.
+#define PLAIN_CH 16
+struct Chunk { int i, j0, j1, k0, k1; };
+__device__ __forceinline__ Chunk chunk_of(const Dev &dv) {
+  Chunk c;
+  c.i = blockIdx.x * 128 + threadIdx.x;
+  if (dv.nz > 1) { c.j0 = blockIdx.y; c.j1 = c.j0 + 1; c.k0 = blockIdx.z * PLAIN_CH; c.k1 = min(dv.nz, c.k0 + PLAIN_CH); }
+  else { c.j0 = blockIdx.y * PLAIN_CH; c.j1 = min(dv.ny, c.j0 + PLAIN_CH); c.k0 = 0; c.k1 = 1; }
+  return c;
+}
+
 // CTA-wide max of a non-negative double -> thread 0 (blockDim.x <= 1024)
 __device__ __forceinline__ double block_max(double v, double *sh) {
   for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_down_sync(0xffffffffu, v, o));
@@ -110,10 +123,13 @@ __global__ void __launch_bounds__(128) k_march64(const __grid_constant__ Dev dv)
   const int xb = ctl->xbuf;
   const double2 *__restrict__ xin = dv.psi64[xb];
   double2 *__restrict__ xout = dv.psi64[xb ^ 1];
-  const int i = blockIdx.x * 128 + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
+  const Chunk ch = chunk_of(dv);
+  const int i = ch.i;
   const bool act = i < dv.nx;
   double r2 = 0.0;
-  if (act) {
+  if (act)
+  for (int k = ch.k0; k < ch.k1; ++k)
+  for (int j = ch.j0; j < ch.j1; ++j) {
     const Site s = site_of(dv, i, j, k);
     const long long m = (long long)i + (long long)dv.nx * (j + (long long)dv.ny * k);
     const cd c = ldc(xin + m);
@@ -149,7 +165,7 @@ __global__ void __launch_bounds__(128) k_march64(const __grid_constant__ Dev dv)
       const cd out = mk(y.x / m2, y.y / m2);
       xout[m] = make_double2(out.x, out.y);
       const double ex = out.x - c.x, ey = out.y - c.y;
-      r2 = (ex * ex + ey * ey) * m2;
+      r2 = fmax(r2, (ex * ex + ey * ey) * m2);
     }
   }
   if (MODE != MODE_RHO) {
@@ -306,8 +322,11 @@ template <class T>
 __global__ void __launch_bounds__(128) k_mu_rhs(const __grid_constant__ Dev dv, MuArrays<T> A) {
   Ctl *ctl = dv.ctl;
   if (ctl->mu_done) return;
-  const int i = blockIdx.x * 128 + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
-  if (i < dv.nx) {
+  const Chunk ch = chunk_of(dv);
+  const int i = ch.i;
+  if (i < dv.nx)
+  for (int k = ch.k0; k < ch.k1; ++k)
+  for (int j = ch.j0; j < ch.j1; ++j) {
     const Site s = site_of(dv, i, j, k);
     const long long m = (long long)i + (long long)dv.nx * (j + (long long)dv.ny * k);
     double ctr;
@@ -328,9 +347,12 @@ __global__ void __launch_bounds__(128) k_mu_sweep(const __grid_constant__ Dev dv
   const int l = ctl->mu_inner;
   const T *__restrict__ xin = (l == 0) ? A.mu : ((l & 1) ? A.xa : A.xb);
   T *__restrict__ xout = (l & 1) ? A.xb : A.xa;
-  const int i = blockIdx.x * 128 + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
+  const Chunk ch = chunk_of(dv);
+  const int i = ch.i;
   double r2 = 0.0;
-  if (i < dv.nx) {
+  if (i < dv.nx)
+  for (int k = ch.k0; k < ch.k1; ++k)
+  for (int j = ch.j0; j < ch.j1; ++j) {
     const Site s = site_of(dv, i, j, k);
     const long long m = (long long)i + (long long)dv.nx * (j + (long long)dv.ny * k);
     double ctr;
@@ -339,7 +361,7 @@ __global__ void __launch_bounds__(128) k_mu_sweep(const __grid_constant__ Dev dv
     const T xn = (T)(((double)A.c[m] + 0.5 * ht * ns) / d);
     xout[m] = xn;
     const double r = d * ((double)xn - ctr);
-    r2 = r * r;
+    r2 = fmax(r2, r * r);
   }
   __shared__ double sh[4];
   const double bm = block_max(r2, sh);
@@ -368,14 +390,17 @@ __global__ void __launch_bounds__(128) k_mu_finish(const __grid_constant__ Dev d
   if (ctl->mu_done) return;
   const int l = ctl->mu_inner;                                    // >= 1 sweeps were done: the last wrote xa (l odd) / xb (l even)
   const T *__restrict__ x = (l & 1) ? A.xa : A.xb;
-  const int i = blockIdx.x * 128 + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
+  const Chunk ch = chunk_of(dv);
+  const int i = ch.i;
   double d2 = 0.0;
-  if (i < dv.nx) {
+  if (i < dv.nx)
+  for (int k = ch.k0; k < ch.k1; ++k)
+  for (int j = ch.j0; j < ch.j1; ++j) {
     const long long m = (long long)i + (long long)dv.nx * (j + (long long)dv.ny * k);
     const T xn = x[m];
     const double dt = ((double)xn - (double)A.mu[m]) / (double)ctl->h_tau;
     A.mu[m] = xn;
-    d2 = dt * dt;
+    d2 = fmax(d2, dt * dt);
   }
   __shared__ double sh[4];
   const double bm = block_max(d2, sh);
@@ -426,7 +451,10 @@ unsigned grid1(long long n, int block, int cap) {
   long long g = (n + block - 1) / block;
   return (unsigned)(g < 1 ? 1 : (g > cap ? cap : g));
 }
-dim3 grid3(const Dev &dv) { return dim3((dv.nx + 127) / 128, dv.ny, dv.nz); }
+dim3 grid3(const Dev &dv) {
+  if (dv.nz > 1) return dim3((dv.nx + 127) / 128, dv.ny, (dv.nz + PLAIN_CH - 1) / PLAIN_CH);
+  return dim3((dv.nx + 127) / 128, (dv.ny + PLAIN_CH - 1) / PLAIN_CH, 1);
+}
 
 template <class T> MuArrays<T> mu_arrays(const Dev &dv, void *mu) {
   MuArrays<T> A;
