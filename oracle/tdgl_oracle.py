@@ -76,6 +76,11 @@ class Params:
     eps_mu_in: float = 1e-6
     mu_max_outer: int = 1000
     mu_max_inner: int = 100
+    # S25: insulating inclusions (P:511 (ii): "no-current (open) boundary conditions across internal grid edges").
+    # Boolean array of the grid shape, True = superconductor, False = a site inside an insulating inclusion (removed:
+    # psi = 0, mu = 0).  Every link ("grid edge") between a superconducting and a removed site is CUT: it carries no
+    # current and drops out of the covariant Laplacian, of rho = div j_s and of Delta_h mu.  None = no such inclusions.
+    sc_mask: Optional[np.ndarray] = None
 
     @property
     def shape(self):
@@ -255,19 +260,52 @@ def _S(f, th, axis, bc):
     return sp, sm
 
 
+def _link_exists(p: Params, axis, bc):
+    """S25: (e+, e-), 1 where the forward / backward link of site m along `axis` exists: both ends are superconducting
+    sites.  On an EXTERNAL open face the paper's rule stands (S- := S+ at the first site, S+ := S- at the last,
+    P:471): the mirrored term exists iff the link it mirrors does."""
+    m = p.sc_mask
+    fw = np.roll(m, -1, axis)
+    bw = np.roll(m, 1, axis)
+    if bc == OPEN:
+        first = [slice(None)] * 3
+        last = [slice(None)] * 3
+        first[axis] = 0
+        last[axis] = -1
+        first, last = tuple(first), tuple(last)
+        bw = bw.copy()
+        fw = fw.copy()
+        bw[first] = np.roll(m, -1, axis)[first]
+        fw[last] = np.roll(m, 1, axis)[last]
+    return (m & fw).astype(np.float64), (m & bw).astype(np.float64)
+
+
 def neighbour_sum(p: Params, f, links):
-    """sum_alpha c_alpha (S+_alpha f + S-_alpha f)_m, c_x = 1/h_x^2, c_y = 1/h_y^2, c_z = 1/(g h_z)^2."""
+    """sum_alpha c_alpha (S+_alpha f + S-_alpha f)_m, c_x = 1/h_x^2, c_y = 1/h_y^2, c_z = 1/(g h_z)^2; with insulating
+    inclusions (S25) only over the links that exist."""
     thx, thy, thz = links
     xp, xm = _S(f, thx, 2, p.bc[0])
     yp, ym = _S(f, thy, 1, p.bc[1])
     zp, zm = _S(f, thz, 0, p.bc[2])
-    return p.cx * (xp + xm) + p.cy * (yp + ym) + p.cz * (zp + zm)
+    if p.sc_mask is None:
+        return p.cx * (xp + xm) + p.cy * (yp + ym) + p.cz * (zp + zm)
+    ex, ey, ez = (_link_exists(p, 2, p.bc[0]), _link_exists(p, 1, p.bc[1]), _link_exists(p, 0, p.bc[2]))
+    return (p.cx * (ex[0] * xp + ex[1] * xm) + p.cy * (ey[0] * yp + ey[1] * ym) + p.cz * (ez[0] * zp + ez[1] * zm))
+
+
+def link_diagonal(p: Params):
+    """sum over the links of site m of c_alpha: 2 (c_x + c_y + c_z) (the "2 sum c" of M_mm), or, with insulating
+    inclusions (S25), the sum over the links that exist (an array)."""
+    if p.sc_mask is None:
+        return 2.0 * (p.cx + p.cy + p.cz)
+    ex, ey, ez = (_link_exists(p, 2, p.bc[0]), _link_exists(p, 1, p.bc[1]), _link_exists(p, 0, p.bc[2]))
+    return p.cx * (ex[0] + ex[1]) + p.cy * (ey[0] + ey[1]) + p.cz * (ez[0] + ez[1])
 
 
 def covariant_laplacian(p: Params, f, links):
     """Eq. (29a): (L f)_m = sum_alpha c_alpha (S+ f + S- f - 2 f)_m.  On open faces this is
-    the printed 2 (U f_1 - f_0)/h^2 form."""
-    return neighbour_sum(p, f, links) - 2.0 * (p.cx + p.cy + p.cz) * f
+    the printed 2 (U f_1 - f_0)/h^2 form; a cut link (S25) contributes nothing."""
+    return neighbour_sum(p, f, links) - link_diagonal(p) * f
 
 
 def _zero_links(p: Params):
@@ -291,6 +329,8 @@ def site_weights(p: Params):
             w[tuple(sl)] *= 0.5
             sl[axis] = -1
             w[tuple(sl)] *= 0.5
+    if p.sc_mask is not None:                       # removed sites carry no weight (S25)
+        w = w * p.sc_mask
     return w
 
 
@@ -405,8 +445,10 @@ def build_system(p: Params, psi, mu, eps, links, zeta=None):
     c = np.abs(psi) ** 2
     if zeta is None:
         zeta = 0.0
+    elif p.sc_mask is not None:
+        zeta = zeta * p.sc_mask                     # no order parameter, hence no Langevin term, on a removed site (S25)
     b = psi + ht2 * ((eps - 1j * p.u * mu) * psi - c * psi + covariant_laplacian(p, psi, links) + 2.0 * zeta)
-    d = 1.0 + ht2 * (c + 2.0 * (p.cx + p.cy + p.cz) - eps + 1j * p.u * mu)
+    d = 1.0 + ht2 * (c + link_diagonal(p) - eps + 1j * p.u * mu)
     return b, d
 
 
@@ -447,6 +489,9 @@ def average_supercurrent(p: Params, psi, links):
     """Eq. (35): J_av = 1/(2 N h_x) sum_m Im[ psi*_m (U_x psi_{i+1} - U_x* psi_{i-1}) ]  (plain 1/N
     mean, S18)."""
     xp, xm = _S(psi, links[0], 2, p.bc[0])
+    if p.sc_mask is not None:                       # only links that exist carry a current (S25); still the plain 1/N mean
+        ex = _link_exists(p, 2, p.bc[0])
+        xp, xm = ex[0] * xp, ex[1] * xm
     return float(np.sum(np.imag(np.conj(psi) * (xp - xm))) / (2.0 * p.n_sites * p.hx))
 
 
@@ -483,6 +528,8 @@ def solve_poisson(p: Params, rho):
     mirror ghost on open faces; S7: weighted zero mode removed).
     FFT along periodic axes and DCT-I along open axes diagonalise Delta_h; the zero mode (whose DCT-I/FFT
     coefficient is 2^{#open} sum_m w_m f_m) is set to zero."""
+    if p.sc_mask is not None:
+        raise ValueError("the transform solver does not apply with insulating inclusions (S25): use mu_solver='pseudotime'")
     f = rho.astype(np.complex128)
     for a, axis in ((0, 2), (1, 1), (2, 0)):
         if p.bc[a] == PERIODIC:
@@ -521,7 +568,7 @@ def solve_poisson_pseudotime(p: Params, rho, mu0, h_tau: float = 0.1, eps_mu: fl
     mu = np.array(mu0, dtype=np.float64)
     rho = np.asarray(rho, dtype=np.float64)
     zl = _zero_links(p)
-    d = 1.0 + h_tau * (p.cx + p.cy + p.cz)
+    d = 1.0 + 0.5 * h_tau * link_diagonal(p)        # N_mm = 1 + h_tau sum c; with S25 over the existing links
     log = []
     n_out = 0
     while True:
@@ -639,6 +686,8 @@ def free_energy(p: Params, psi, eps, links) -> float:
             sl = [slice(None)] * 3
             sl[axis] = -1
             wl[tuple(sl)] = 0.0
+        if p.sc_mask is not None:                   # a cut link stores no gradient energy (S25)
+            wl = wl * (p.sc_mask & np.roll(p.sc_mask, -1, axis))
         F += c * np.sum(wl * g2)
     return float(F * p.cell)
 
@@ -655,6 +704,9 @@ def plaquette_windings(p: Params, psi, links, Bz: float):
         n[:, :, -1] = 0.0
     if p.bc[1] == OPEN:
         n[:, -1, :] = 0.0
+    if p.sc_mask is not None:                       # a plaquette with a removed corner has no winding (S25)
+        m = p.sc_mask
+        n = np.where(m & np.roll(m, -1, 2) & np.roll(m, -1, 1) & np.roll(np.roll(m, -1, 1), -1, 2), n, 0.0)
     return n
 
 
@@ -675,5 +727,7 @@ def link_supercurrents(p: Params, psi, links):
             sl = [slice(None)] * 3
             sl[axis] = -1
             j[tuple(sl)] = 0.0
+        if p.sc_mask is not None:                   # no current across a cut link (S25)
+            j = j * (p.sc_mask & np.roll(p.sc_mask, -1, axis))
         out.append(j)
     return out

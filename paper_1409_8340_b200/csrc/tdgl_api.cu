@@ -481,7 +481,10 @@ extern "C" int tdgl_create(const tdgl_params *p, tdgl_t **out) {
       CKC(cudaStreamSynchronize(st));               // the host table dies at the end of this block
       continue;
     }
-    dv.bLB[a] = (bcs[a] == TDGL_BC_OPEN) ? dct_fast_lb(ns[a]) : 0;
+    // Bluestein DCT-I tables only for the axes that are transformed: x, and y of a 3D mesh (open z, and the open y of a
+    // film, which takes the z role, are solved by the Thomas algorithm)
+    const bool dct_axis = a == 0 || (a == 1 && !film);
+    dv.bLB[a] = (bcs[a] == TDGL_BC_OPEN && dct_axis) ? dct_fast_lb(ns[a]) : 0;
     if (dv.bLB[a]) {
       CKC(dct_fast_configure(dv.bLB[a]));
       launch_build_bluestein(dv.bT[a], dv.bC[a], dv.bH[a], ns[a], dv.bLB[a], st);

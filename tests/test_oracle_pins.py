@@ -778,3 +778,175 @@ def test_S5_the_printed_sign_has_no_fixed_point():
     c_stable = mu + h_tau * (0.5 * O.laplacian_real(p, mu) - rho)
     assert np.max(np.abs(Nmu - c_stable)) < 1e-12
     assert np.max(np.abs((Nmu - c_printed) + h_tau * rho)) < 1e-12 and np.max(np.abs(Nmu - c_printed)) > 0.1
+
+
+# ------------------------------------------------------------------------------------------------
+# S25: insulating inclusions = cut links (P:511 (ii): "no-current (open) boundary conditions across internal grid edges")
+# ------------------------------------------------------------------------------------------------
+def _mask_with_holes(p, seed):
+    """A cuboid hole, an L-shaped hole (re-entrant corners) and a few single removed sites; never the whole of a row."""
+    rng = np.random.default_rng(seed)
+    m = np.ones(p.shape, bool)
+    m[2:5, 1:4, 3:6] = False
+    m[5:7, 4:7, 0:2] = False
+    m[6:7, 6:8, 0:4] = False
+    for _ in range(6):
+        m[tuple(rng.integers(0, n) for n in p.shape)] = False
+    return m
+
+
+def _site_terms(p, i, j, k, K, Bx, Bz):
+    """The six neighbour terms of site (i, j, k) of the paper's operator, as (neighbour index, factor, c_alpha): the value
+    (S+-_alpha psi)_m = factor * psi[neighbour].  Written out from P:272-276 (Eq. 29a), P:449-455 (jump), P:471-505 (open
+    faces: S- := S+ at the first site, S+ := S- at the last) site by site -- independently of the oracle's array code."""
+    Ly = p.length("y")
+    ybar = j * p.hy - Ly / 2
+    Ux = np.exp(1j * p.hx * (K + Bz * ybar))
+    Uz = np.exp(-1j * p.hz * Bx * ybar)
+    Pik = np.exp(1j * (i * p.hx * Ly * Bz - k * p.hz * Ly * Bx))
+    out = []
+    n = (p.nx, p.ny, p.nz)
+    pos = (i, j, k)
+    for a, (U, c) in enumerate(((Ux, p.cx), (1.0, p.cy), (Uz, p.cz))):
+        fw = list(pos); fw[a] += 1
+        bw = list(pos); bw[a] -= 1
+        tf, tb = (tuple(fw), U), (tuple(bw), np.conj(U))
+        if p.bc[a] == P_:
+            if fw[a] == n[a]:
+                fw[a] = 0
+                tf = (tuple(fw), U * (np.conj(Pik) if a == 1 else 1.0))
+            if bw[a] < 0:
+                bw[a] = n[a] - 1
+                tb = (tuple(bw), np.conj(U) * (Pik if a == 1 else 1.0))
+        else:
+            if bw[a] < 0:
+                tb = tf                                        # S- := S+
+            if fw[a] == n[a]:
+                tf = tb                                        # S+ := S-
+        out += [(tf[0], tf[1], c), (tb[0], tb[1], c)]
+    return out
+
+
+def dense_M_cut(p, psi_prev, mu, eps, K, Bx, Bz, mask):
+    """Dense M of the implicit step with insulating inclusions: every term whose neighbour is a removed site is
+    dropped from the row AND from the diagonal's sum over links; rows of removed sites are the identity."""
+    N = p.n_sites
+    M = np.zeros((N, N), dtype=np.complex128)
+    idx = lambda i, j, k: i + p.nx * (j + p.ny * k)
+    ht = p.ht
+    for k in range(p.nz):
+        for j in range(p.ny):
+            for i in range(p.nx):
+                m = idx(i, j, k)
+                if not mask[k, j, i]:
+                    M[m, m] = 1.0
+                    continue
+                diag = abs(psi_prev[k, j, i]) ** 2 + 1j * p.u * mu[k, j, i] - eps[k, j, i]
+                for (ii, jj, kk), fac, c in _site_terms(p, i, j, k, K, Bx, Bz):
+                    if mask[kk, jj, ii]:
+                        M[m, idx(ii, jj, kk)] += -(ht / 2) * c * fac
+                        diag += c
+                M[m, m] = 1 + (ht / 2) * diag
+    return M
+
+
+@pytest.mark.parametrize("bc", [(P_, P_, P_), (P_, P_, O_), (O_, O_, O_), (O_, P_, P_)])
+def test_S25_implicit_step_with_cut_links_dense_solve(bc):
+    mask = _mask_with_holes(O.Params(8, 8, 8), 3)
+    p = O.Params(8, 8, 8, hx=0.5, hy=0.55, hz=0.45, g=1.1, u=1.7, bc=bc, eps_tol=1e-28, max_sweeps=5000, solve_mu=False,
+                 sc_mask=mask)
+    Bx, Bz, _, _ = O.snap_field(p, 0.12, 0.35)
+    K = 0.21 if bc[0] == P_ else 0.0
+    rng = np.random.default_rng(4)
+    psi0 = (1.0 + 0.4 * rand_psi(p, 7)) * mask
+    mu0 = rng.uniform(-0.2, 0.2, p.shape) * mask
+    eps = np.where(rng.uniform(size=p.shape) < 0.3, -1.0, 1.0)
+    # without holes the site-by-site assembly is the printed matrix (the function of the P9 pin)
+    pfull = O.Params(8, 8, 8, hx=0.5, hy=0.55, hz=0.45, g=1.1, u=1.7, bc=bc)
+    full = np.ones(p.shape, bool)
+    assert np.max(np.abs(dense_M_cut(pfull, psi0, mu0, eps, K, Bx, Bz, full) - dense_M(pfull, psi0, mu0, eps, K, Bx, Bz))) < 1e-14
+    M = dense_M_cut(p, psi0, mu0, eps, K, Bx, Bz, mask)
+    b_dense = 2 * psi0.ravel() - M @ psi0.ravel()
+    links = O.paper_links(p, K, Bx, Bz)
+    b, d = O.build_system(p, psi0, mu0, eps, links)
+    sc = mask.ravel()
+    assert np.max(np.abs(b.ravel() - b_dense)[sc]) < 1e-13 and np.max(np.abs(b.ravel()[~sc])) == 0.0
+    assert np.max(np.abs(d.ravel() - np.diag(M))[sc]) < 1e-15
+    off = np.sum(np.abs(M), axis=1) - np.abs(np.diag(M))
+    assert np.all(np.abs(np.diag(M)) > off)                              # still strictly diagonally dominant
+    x_dense = np.linalg.solve(M, b_dense)
+    st = O.State(psi=psi0.copy(), mu=mu0.copy(), K=K)
+    O.step(p, st, eps, Bx, Bz, 0.0)
+    assert np.max(np.abs(st.psi.ravel() - x_dense)) < 1e-12
+    assert np.all(st.psi[~mask] == 0.0)                                  # removed sites stay empty
+
+
+@pytest.mark.parametrize("bc", ALL_BC)
+def test_S25_cut_links_conserve_current_and_the_operator_is_hermitian(bc):
+    """With cut links the covariant Laplacian is Hermitian in the weighted inner product (the mirror rule applied at
+    the re-entrant corners of a voxelised hole would not be), so the weighted sum of rho = div j_s vanishes exactly:
+    the Neumann problem for mu stays solvable.  And div(j_s + j_n) = rho - Delta_h mu on the links that exist (P7)."""
+    mask = _mask_with_holes(O.Params(8, 8, 8), 5)
+    p = O.Params(8, 8, 8, hx=0.5, hy=0.4, hz=0.6, g=1.2, bc=bc, sc_mask=mask)
+    Bx, Bz, _, _ = O.snap_field(p, 0.1, 0.3)
+    links = O.paper_links(p, 0.2 if bc[0] == P_ else 0.0, Bx, Bz)
+    w = O.site_weights(p)
+    f, g_ = rand_psi(p, 1) * mask, rand_psi(p, 2) * mask
+    lhs = np.sum(w * np.conj(f) * O.covariant_laplacian(p, g_, links))
+    rhs = np.sum(w * np.conj(O.covariant_laplacian(p, f, links)) * g_)
+    assert abs(lhs - rhs) < 1e-11
+    rho = O.supercurrent_divergence(p, f, links)
+    assert abs(np.sum(w * rho)) < 1e-12 and np.all(rho[~mask] == 0.0)
+    # discrete divergence of the link currents = rho - Delta_h mu, site by site (open faces: weight 1/2 doubles the link)
+    mu = np.random.default_rng(3).standard_normal(p.shape) * mask
+    js = O.link_supercurrents(p, f, links)
+    div = np.zeros(p.shape)
+    for a, axis, h, c in ((0, 2, p.hx, p.cx), (1, 1, p.hy, p.cy), (2, 0, p.hz, p.cz)):
+        exist = (mask & np.roll(mask, -1, axis)).astype(float)
+        if p.bc[a] == O_:
+            sl = [slice(None)] * 3
+            sl[axis] = -1
+            exist[tuple(sl)] = 0.0
+        gg = p.g ** 2 if a == 2 else 1.0
+        jn = -(np.roll(mu, -1, axis) - mu) / (h * gg) * exist
+        flux = (js[a] + jn) / h                                          # through the forward link
+        wa = np.ones(p.shape)
+        if p.bc[a] == O_:
+            sl = [slice(None)] * 3
+            sl[axis] = 0
+            wa[tuple(sl)] = 0.5
+            sl[axis] = -1
+            wa[tuple(sl)] = 0.5
+        div += (flux - np.roll(flux, 1, axis)) / wa
+    assert np.max(np.abs(div - (rho - O.laplacian_real(p, mu)))[mask]) < 1e-11
+
+
+def test_S25_pseudo_time_solver_with_holes_and_gauge_invariance():
+    mask = _mask_with_holes(O.Params(8, 8, 8), 7)
+    p = O.Params(8, 8, 8, bc=(P_, P_, O_), sc_mask=mask, mu_solver="pseudotime", h_tau=1.0, eps_mu=1e-26, eps_mu_in=1e-28,
+                 mu_max_outer=4000, mu_max_inner=4000, eps_tol=1e-26, max_sweeps=4000)
+    Bx, Bz, _, _ = O.snap_field(p, 0.0, 0.3)
+    psi0 = nonzero_psi(p, 4) * mask
+    eps = np.ones(p.shape)
+    # the direct solver refuses; the iteration reaches Delta_h mu = rho on every superconducting site
+    with pytest.raises(ValueError):
+        O.solve_poisson(p, np.zeros(p.shape))
+    st = O.State(psi=psi0.copy(), mu=np.zeros(p.shape), K=0.1)
+    O.step(p, st, eps, Bx, Bz, 0.02)
+    links = O.paper_links(p, st.K, Bx, Bz)
+    res = O.laplacian_real(p, st.mu) - O.supercurrent_divergence(p, st.psi, links)
+    assert np.max(np.abs(res[mask])) < 1e-10 and np.all(st.mu[~mask] == 0.0) and np.all(st.psi[~mask] == 0.0)
+    assert abs(np.sum(O.site_weights(p) * st.mu)) < 1e-10
+    # gauge invariance (P8) with holes: psi -> psi e^{i chi}, th(m) -> th(m) + chi(m) - chi(m + alpha)
+    chi = np.random.default_rng(9).uniform(-3, 3, p.shape)
+
+    def gauged(K):
+        thx, thy, thz = O.paper_links(p, K, Bx, Bz)
+        return (thx + chi - np.roll(chi, -1, 2), thy + chi - np.roll(chi, -1, 1), thz + chi - np.roll(chi, -1, 0))
+    st2 = O.State(psi=psi0 * np.exp(1j * chi), mu=np.zeros(p.shape), K=0.1)
+    O.step(p, st2, eps, Bx, Bz, 0.02, links_fn=gauged)
+    assert np.max(np.abs(np.abs(st2.psi) - np.abs(st.psi))) < 1e-11
+    assert np.max(np.abs(st2.mu - st.mu)) < 1e-9 and abs(st2.K - st.K) < 1e-12
+    F1 = O.free_energy(p, st.psi, eps, links)
+    F2 = O.free_energy(p, st2.psi, eps, gauged(st2.K))
+    assert abs(F1 - F2) < 1e-10 * abs(F1)
