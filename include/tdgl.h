@@ -52,6 +52,11 @@ extern "C" {
                                    psi, b, d, mu in double (104 B/site of workspace), every kernel of the step in fp64;
                                    mu is solved by the pseudo-time iteration (the direct solver is fp32 only).  psi / mu
                                    buffers of tdgl_get_psi_mu, tdgl_set_state, tdgl_debug_* are then double (pairs). */
+#define TDGL_FLAG_INSULATORS 128u /* insulating inclusions (P:511 (ii), reading S25): tdgl_set_insulators removes the sites
+                                   inside a list of spheres and CUTS every link between a superconducting and a removed
+                                   site ("no-current boundary conditions across internal grid edges").  Needs
+                                   TDGL_FLAG_FP64 (the cut links are implemented in the precision-generic kernels; mu is
+                                   then solved by the pseudo-time iteration, the transform solver does not apply). */
 #define TDGL_FLAG_HOST_LOOP 2u  /* test/diagnostic: host-driven sweep loop instead of the CUDA-graph
                                    WHILE node (identical arithmetic)                                     */
 
@@ -115,6 +120,14 @@ int tdgl_destroy(tdgl_t *h);
  * axes), else eps_out (P:245, P:511 (i), S19).  `spheres_host` is copied during the call; n may be 0.
  * The workspace scratch array holds the device copy, so n <= N/4. */
 int tdgl_set_pinning(tdgl_t *h, const tdgl_sphere *spheres_host, int64_t n, float eps_in, float eps_out);
+
+/* Insulating inclusions (TDGL_FLAG_INSULATORS only, else TDGL_EINCOMPAT): every site within distance r of a sphere centre
+ * (the inside test of tdgl_set_pinning) is REMOVED -- psi = 0 and mu = 0 there for good -- and every link between a
+ * remaining and a removed site is cut: it carries no supercurrent and no normal current, and drops out of the covariant
+ * Laplacian (Eq. 29), of M (the diagonal sums c_alpha over the links that exist), of rho and of the
+ * Laplacian of mu.  External open faces keep the paper's mirror rule.  Replaces any earlier list; n may be 0.
+ * J_av keeps the plain 1/N mean of Eq. (35) over the links that exist. */
+int tdgl_set_insulators(tdgl_t *h, const tdgl_sphere *spheres_host, int64_t n);
 
 /* Applied field and transport current J_ext along x (Eq. 21).  The Landau gauge is fixed at create (S23):
  * xz gauge (default; Eq. 24a): B = (Bx, 0, Bz); yz gauge (TDGL_FLAG_GAUGE_YZ; Eq. 24b): B = (0, By, Bz).

@@ -6,7 +6,7 @@ torch is used for device memory and streams.  There is no CPU path: loading fail
 library has not been built (`python -m paper_1409_8340_b200.build`).
 """
 from .binding import (  # noqa: F401
-    TDGL_BC_OPEN, TDGL_BC_PERIODIC, TDGL_FLAG_FP64, TDGL_FLAG_GAUGE_YZ, TDGL_FLAG_HOST_LOOP, TDGL_FLAG_MU_ITERATIVE, TDGL_FLAG_SOLVE_MU, TdglError, TdglObs, TdglParams,
+    TDGL_BC_OPEN, TDGL_BC_PERIODIC, TDGL_FLAG_FP64, TDGL_FLAG_GAUGE_YZ, TDGL_FLAG_HOST_LOOP, TDGL_FLAG_INSULATORS, TDGL_FLAG_MU_ITERATIVE, TDGL_FLAG_SOLVE_MU, TdglError, TdglObs, TdglParams,
     TdglSphere, Solver, lib, tdgl_create, tdgl_destroy, tdgl_get_psi_mu, tdgl_observables, tdgl_set_field_current,
     tdgl_set_pinning, tdgl_step, tdgl_strerror, tdgl_workspace_bytes,
 )

@@ -13,14 +13,14 @@ _LIB_PATH = os.environ.get("TDGL_LIB") or os.path.join(_HERE, "libtdgl.so")     
 TDGL_OK, TDGL_EINVAL, TDGL_ENOMEM, TDGL_EINCOMPAT, TDGL_ECUDA, TDGL_WMAXSWEEPS = 0, -1, -2, -3, -4, 1
 TDGL_BC_PERIODIC, TDGL_BC_OPEN = 0, 1
 TDGL_FLAG_SOLVE_MU, TDGL_FLAG_HOST_LOOP, TDGL_FLAG_GAUGE_YZ, TDGL_FLAG_MU_REFINE, TDGL_FLAG_MU_NOREFINE = 1, 2, 4, 8, 16
-TDGL_FLAG_MU_ITERATIVE, TDGL_FLAG_FP64 = 32, 64
+TDGL_FLAG_MU_ITERATIVE, TDGL_FLAG_FP64, TDGL_FLAG_INSULATORS = 32, 64, 128
 
 EXPORTS = (
     "tdgl_workspace_bytes", "tdgl_create", "tdgl_destroy", "tdgl_set_pinning", "tdgl_set_field_current", "tdgl_step",
     "tdgl_get_psi_mu", "tdgl_observables", "tdgl_strerror", "tdgl_last_cuda_error", "tdgl_set_state", "tdgl_set_solver",
     "tdgl_set_sweep_schedule", "tdgl_get_sweep_log", "tdgl_get_eps", "tdgl_debug_noise", "tdgl_debug_poisson",
     "tdgl_debug_rho", "tdgl_launch_count", "tdgl_sweep_timing", "tdgl_mu_gain", "tdgl_mu_refine_enabled",
-    "tdgl_set_mu_solver", "tdgl_get_mu_log",
+    "tdgl_set_mu_solver", "tdgl_get_mu_log", "tdgl_set_insulators",
 )
 
 
@@ -94,6 +94,7 @@ def lib() -> C.CDLL:
     L.tdgl_mu_gain.argtypes = [C.POINTER(TdglParams)]
     L.tdgl_mu_refine_enabled.argtypes = [vp]
     L.tdgl_set_mu_solver.argtypes = [vp, f32, f32, f32, i32, i32]
+    L.tdgl_set_insulators.argtypes = [vp, C.POINTER(TdglSphere), i64]
     L.tdgl_get_mu_log.argtypes = [vp, i32, C.POINTER(i32), C.POINTER(i32), i32, C.POINTER(i32)]
     _lib = L
     return L
@@ -161,7 +162,7 @@ class Solver:
                  u: float = 1.0, g: float = 1.0, eps_tol: float = 1e-6, max_sweeps: int = 100, fixed_sweeps: int = 0,
                  temperature: float = 0.0, seed: int = 0, init_amp: float = 0.01, solve_mu: bool = True,
                  host_loop: bool = False, hxyz: Optional[Sequence[float]] = None, device: Optional[str] = None,
-                 gauge_yz: bool = False, mu_refine: Optional[bool] = None, mu_iterative: bool = False, fp64: bool = False):
+                 gauge_yz: bool = False, mu_refine: Optional[bool] = None, mu_iterative: bool = False, fp64: bool = False, insulators: bool = False):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1409_8340_b200 needs a CUDA device (sm_100a); there is no CPU path")
@@ -179,7 +180,8 @@ class Solver:
         p.flags = ((TDGL_FLAG_SOLVE_MU if solve_mu else 0) | (TDGL_FLAG_HOST_LOOP if host_loop else 0)
                    | (TDGL_FLAG_GAUGE_YZ if gauge_yz else 0)
                    | (0 if mu_refine is None else (TDGL_FLAG_MU_REFINE if mu_refine else TDGL_FLAG_MU_NOREFINE))
-                   | (TDGL_FLAG_MU_ITERATIVE if mu_iterative else 0) | (TDGL_FLAG_FP64 if fp64 else 0))
+                   | (TDGL_FLAG_MU_ITERATIVE if mu_iterative else 0) | (TDGL_FLAG_FP64 if fp64 else 0)
+                   | (TDGL_FLAG_INSULATORS if insulators else 0))
         self.fp64 = bool(fp64)
         nbytes = tdgl_workspace_bytes(p)
         if nbytes == 0:
@@ -207,6 +209,12 @@ class Solver:
     # the boundary
     def set_pinning(self, spheres, eps_in=-1.0, eps_out=1.0):
         tdgl_set_pinning(self.h, np.asarray(spheres, dtype=np.float32), eps_in, eps_out)
+
+    def set_insulators(self, spheres):
+        """spheres: float32 array (n, 4) = (cx, cy, cz, r), HOST memory (TDGL_FLAG_INSULATORS)."""
+        s = np.ascontiguousarray(spheres, dtype=np.float32).reshape(-1, 4)
+        ptr = s.ctypes.data_as(C.POINTER(TdglSphere)) if len(s) else None
+        _check(lib().tdgl_set_insulators(self.h, ptr, len(s)), "tdgl_set_insulators", self.h)
 
     def set_field_current(self, Bx=0.0, By=0.0, Bz=0.0, Jx=0.0):
         tdgl_set_field_current(self.h, Bx, By, Bz, Jx)

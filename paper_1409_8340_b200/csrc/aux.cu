@@ -104,7 +104,9 @@ __global__ void k_fill_f32(float *p, long long n, float v) {
 // Inside test (P:245, 511 (i), S19): d_x^2 + d_y^2 + d_z^2 <= r^2 with d the minimum-image distance on
 // periodic axes, evaluated in fp64 with every product and sum rounded separately (no contraction), so
 // the mask does not depend on how the compiler fuses operations.
-__global__ void __launch_bounds__(128) k_spheres(const __grid_constant__ Dev dv, const float4 *__restrict__ sph, float eps_in) {
+// mask != nullptr: the sphere REMOVES its sites instead (insulating inclusion, S25): mask[m] = 0.
+__global__ void __launch_bounds__(128) k_spheres(const __grid_constant__ Dev dv, const float4 *__restrict__ sph, float eps_in,
+                                                 unsigned char *mask) {
   const float4 s = sph[blockIdx.x];
   const int n[3] = {dv.nx, dv.ny, dv.nz};
   const int bc[3] = {dv.bcx, dv.bcy, dv.bcz};
@@ -139,8 +141,11 @@ __global__ void __launch_bounds__(128) k_spheres(const __grid_constant__ Dev dv,
       }
       d2[a] = __dmul_rn(d, d);
     }
-    if (__dadd_rn(__dadd_rn(d2[0], d2[1]), d2[2]) <= r2)
-      dv.eps[idx[0] + (long long)dv.nx * (idx[1] + (long long)dv.ny * idx[2])] = eps_in;
+    if (__dadd_rn(__dadd_rn(d2[0], d2[1]), d2[2]) <= r2) {
+      const long long m = idx[0] + (long long)dv.nx * (idx[1] + (long long)dv.ny * idx[2]);
+      if (mask) mask[m] = 0;
+      else dv.eps[m] = eps_in;
+    }
   }
 }
 
@@ -279,11 +284,15 @@ void launch_ctl_sched(const Dev &dv, int n, cudaStream_t st) { k_ctl_sched<<<1, 
 void launch_ctl_state(const Dev &dv, double K, cudaStream_t st) { k_ctl_state<<<1, 1, 0, st>>>(dv, K); }
 void launch_set_field(const Dev &dv, double Bx, double Bz, double J, cudaStream_t st) { k_set_field<<<1, 256, 0, st>>>(dv, Bx, Bz, J); }
 void launch_fill(float *p, long long n, float v, cudaStream_t st) { k_fill_f32<<<grid_for(n, 256, 148 * 16), 256, 0, st>>>(p, n, v); }
-void launch_spheres(const Dev &dv, const float4 *sph, long long n, float eps_in, cudaStream_t st) {
+static void spheres_impl(const Dev &dv, const float4 *sph, long long n, float eps_in, cudaStream_t st, unsigned char *mask) {
   for (long long off = 0; off < n; off += 1 << 20) {
     const unsigned g = (unsigned)((n - off) < (1 << 20) ? (n - off) : (1 << 20));
-    k_spheres<<<g, 128, 0, st>>>(dv, sph + off, eps_in);
+    k_spheres<<<g, 128, 0, st>>>(dv, sph + off, eps_in, mask);
   }
+}
+void launch_spheres(const Dev &dv, const float4 *sph, long long n, float eps_in, cudaStream_t st) { spheres_impl(dv, sph, n, eps_in, st, nullptr); }
+void launch_spheres_mask(const Dev &dv, const float4 *sph, long long n, unsigned char *mask, cudaStream_t st) {
+  spheres_impl(dv, sph, n, 0.f, st, mask);
 }
 void launch_copy_psi(const Dev &dv, float2 *out, cudaStream_t st) { k_copy_psi<<<grid_for(dv.N / 2, 256, 148 * 16), 256, 0, st>>>(dv, out); }
 void launch_noise(const Dev &dv, long long step, float2 *out, cudaStream_t st) { k_noise<<<grid_for(dv.N, 256, 148 * 16), 256, 0, st>>>(dv, step, out); }

@@ -45,8 +45,39 @@ __device__ __forceinline__ Site site_of(const Dev &dv, int i, int j, int k) {
   return s;
 }
 
-// sum_alpha c_alpha (S+_alpha x + S-_alpha x)_m in fp64 (Eq. 29a / 29b without the -2 x term), fp64 link variables
-__device__ __forceinline__ cd neighbour_sum(const Dev &dv, const double2 *__restrict__ x, const Site &s) {
+// Insulating inclusions (S25): which of the six neighbour terms of a superconducting site exist.  A link to a removed
+// site is cut; on an external open face the mirrored term exists iff the link it mirrors does.  bit 0/1: x +/-, 2/3: y, 4/5: z.
+__device__ __forceinline__ unsigned link_bits(const Dev &dv, const Site &s) {
+  if (!dv.sc) return 63u;
+  const int nx = dv.nx, ny = dv.ny;
+  const long long plane = (long long)nx * ny;
+  const long long rowb = (long long)s.k * plane + (long long)s.j * nx;
+  unsigned b = 0u;
+  bool fw = dv.sc[rowb + s.ie] != 0, bw = dv.sc[rowb + s.iw] != 0;
+  if (s.xlo) bw = fw;
+  if (s.xhi) fw = bw;
+  b |= (fw ? 1u : 0u) | (bw ? 2u : 0u);
+  fw = dv.sc[(long long)s.k * plane + (long long)s.jn * nx + s.i] != 0; bw = dv.sc[(long long)s.k * plane + (long long)s.js * nx + s.i] != 0;
+  if (s.ylo) bw = fw;
+  if (s.yhi) fw = bw;
+  b |= (fw ? 4u : 0u) | (bw ? 8u : 0u);
+  if (dv.nz > 1) {
+    fw = dv.sc[(long long)s.kt * plane + (long long)s.j * nx + s.i] != 0; bw = dv.sc[(long long)s.kb * plane + (long long)s.j * nx + s.i] != 0;
+    if (s.zlo) bw = fw;
+    if (s.zhi) fw = bw;
+    b |= (fw ? 16u : 0u) | (bw ? 32u : 0u);
+  }
+  return b;
+}
+// sum over the existing links of site m of c_alpha: 2 (c_x + c_y + c_z) without inclusions (the "2 sum c" of M_mm)
+__device__ __forceinline__ double link_diag(const Dev &dv, unsigned lb) {
+  if (lb == 63u) return dv.csum2_64;
+  return dv.cx64 * (double)__popc(lb & 3u) + dv.cy64 * (double)__popc(lb & 12u) + (dv.nz > 1 ? dv.cz64 * (double)__popc(lb & 48u) : 0.0);
+}
+
+// sum_alpha c_alpha (S+_alpha x + S-_alpha x)_m in fp64 (Eq. 29a / 29b without the -2 x term), fp64 link variables;
+// `lb`: the terms that exist (link_bits)
+__device__ __forceinline__ cd neighbour_sum(const Dev &dv, const double2 *__restrict__ x, const Site &s, unsigned lb = 63u) {
   const int nx = dv.nx, ny = dv.ny;
   const long long plane = (long long)nx * ny;
   const bool film = dv.nz == 1, yz = dv.gauge_yz != 0;
@@ -61,6 +92,8 @@ __device__ __forceinline__ cd neighbour_sum(const Dev &dv, const double2 *__rest
   cd sp = cm(Ux, e), sm = cmc(Ux, w);
   if (s.xlo) sm = sp;
   if (s.xhi) sp = sm;
+  if (!(lb & 1u)) sp = mk(0.0, 0.0);
+  if (!(lb & 2u)) sm = mk(0.0, 0.0);
   cd acc = mk(dv.cx64 * (sp.x + sm.x), dv.cx64 * (sp.y + sm.y));
   cd n = ldc(x + (long long)s.k * plane + (long long)s.jn * nx + s.i), so = ldc(x + (long long)s.k * plane + (long long)s.js * nx + s.i);
   if (!yz && dv.bcy == 0 && (s.j == ny - 1 || s.j == 0)) {         // jump in y: psi_{i,-1,k} = P_{i,k} psi_{i,ny-1,k}
@@ -72,6 +105,8 @@ __device__ __forceinline__ cd neighbour_sum(const Dev &dv, const double2 *__rest
   else { sp = n; sm = so; }
   if (s.ylo) sm = sp;
   if (s.yhi) sp = sm;
+  if (!(lb & 4u)) sp = mk(0.0, 0.0);
+  if (!(lb & 8u)) sm = mk(0.0, 0.0);
   acc.x += dv.cy64 * (sp.x + sm.x); acc.y += dv.cy64 * (sp.y + sm.y);
   if (!film) {
     const cd Uz = yz ? ldt(dv.Uzx64 + s.i) : ldt(dv.Uz64 + s.j);
@@ -79,6 +114,8 @@ __device__ __forceinline__ cd neighbour_sum(const Dev &dv, const double2 *__rest
     sp = cm(Uz, t); sm = cmc(Uz, b);
     if (s.zlo) sm = sp;
     if (s.zhi) sp = sm;
+    if (!(lb & 16u)) sp = mk(0.0, 0.0);
+    if (!(lb & 32u)) sm = mk(0.0, 0.0);
     acc.x += dv.cz64 * (sp.x + sm.x); acc.y += dv.cz64 * (sp.y + sm.y);
   }
   return acc;
@@ -132,8 +169,14 @@ __global__ void __launch_bounds__(128) k_march64(const __grid_constant__ Dev dv)
   for (int j = ch.j0; j < ch.j1; ++j) {
     const Site s = site_of(dv, i, j, k);
     const long long m = (long long)i + (long long)dv.nx * (j + (long long)dv.ny * k);
+    if (dv.sc && !dv.sc[m]) {                                             // a removed site (S25): psi = 0, rho = 0
+      if (MODE == MODE_RHO) dv.mu64[m] = 0.0;
+      else xout[m] = make_double2(0.0, 0.0);
+      continue;
+    }
+    const unsigned lb = link_bits(dv, s);
     const cd c = ldc(xin + m);
-    const cd ns = neighbour_sum(dv, xin, s);
+    const cd ns = neighbour_sum(dv, xin, s, lb);
     if (MODE == MODE_RHO) {
       dv.mu64[m] = c.x * ns.y - c.y * ns.x;                                 // rho_m = Im[psi*_m sum (S+ + S-) psi]
     } else {
@@ -143,7 +186,7 @@ __global__ void __launch_bounds__(128) k_march64(const __grid_constant__ Dev dv)
         // d_m = 1 + (h_t/2)[|psi|^2 + 2 sum c - eps + i u mu];  b_m = psi (2 - d) + (h_t/2)(nsum + 2 zeta)  (Eq. 31)
         const double a = c.x * c.x + c.y * c.y;
         const double mu = dv.solve_mu ? dv.mu64[m] : 0.0;
-        d = mk(1.0 + ht2 * (a + dv.csum2_64 - (double)dv.eps[m]), ht2 * dv.u64 * mu);
+        d = mk(1.0 + ht2 * (a + link_diag(dv, lb) - (double)dv.eps[m]), ht2 * dv.u64 * mu);
         cd z = mk(0.0, 0.0);
         if (dv.zeta_max64 > 0.0) {                                          // Langevin term, Eq. (39), S11
           const unsigned long long mm = (unsigned long long)m;
@@ -193,8 +236,10 @@ __global__ void __launch_bounds__(256) k_jav64(const __grid_constant__ Dev dv) {
     const int i = (int)(m % nx);
     const long long row = m / nx;
     const int j = (int)(row % ny), k = (int)(row / ny);
+    const long long me = row * nx + (i + 1 == nx ? 0 : i + 1);
+    if (dv.sc && !(dv.sc[m] && dv.sc[me])) continue;            // a cut link carries no current (S25)
     const cd a = ldc(x + m);
-    cd b = ldc(x + row * nx + (i + 1 == nx ? 0 : i + 1));
+    cd b = ldc(x + me);
     if (dv.gauge_yz && i + 1 == nx) b = cmc(cm(ldt(dv.Pj64 + j), ldt(dv.Pk64 + k)), b);
     const cd ub = cm(ldt(dv.Ux64 + j), b);
     acc += a.x * ub.y - a.y * ub.x;
@@ -249,7 +294,7 @@ __global__ void __launch_bounds__(256) k_obs64(const __grid_constant__ Dev dv) {
     const long long rest = m / nx;
     const int j = (int)(rest % ny), k = (int)(rest / ny);
     const int ip = (i + 1 == nx) ? 0 : i + 1, jp = (j + 1 == ny) ? 0 : j + 1, kp = (k + 1 == nz) ? 0 : k + 1;
-    const bool hasx = dv.bcx == 0 || i + 1 < nx, hasy = dv.bcy == 0 || j + 1 < ny, hasz = !film && (dv.bcz == 0 || k + 1 < nz);
+    const bool hasx0 = dv.bcx == 0 || i + 1 < nx, hasy0 = dv.bcy == 0 || j + 1 < ny, hasz0 = !film && (dv.bcz == 0 || k + 1 < nz);
     const double wx = face_w64(i, nx, dv.bcx), wy = face_w64(j, ny, dv.bcy), wz = film ? 1.0 : face_w64(k, nz, dv.bcz);
     const cd Pk = ldt(dv.Pk64 + k);
     auto at = [&](int ii, int jj, int kk) { return ldc(x + (long long)kk * plane + (long long)jj * nx + ii); };
@@ -266,6 +311,9 @@ __global__ void __launch_bounds__(256) k_obs64(const __grid_constant__ Dev dv) {
       if (dv.bcy == 0 && jj + 1 == ny) return cmc(cmc(Pk, ldt(dv.Pi64 + ii)), v);
       return v;
     };
+    auto sc = [&](int ii, int jj, int kk) { return !dv.sc || dv.sc[(long long)kk * plane + (long long)jj * nx + ii] != 0; };
+    if (!sc(i, j, k)) continue;                                  // removed sites and cut links carry nothing (S25)
+    const bool hasx = hasx0 && sc(ip, j, k), hasy = hasy0 && sc(i, jp, k), hasz = hasz0 && sc(i, j, kp);
     const cd c = at(i, j, k);
     const double ab = c.x * c.x + c.y * c.y;
     const cd e = xlink(i, j), n = ylink(i, j);
@@ -279,7 +327,7 @@ __global__ void __launch_bounds__(256) k_obs64(const __grid_constant__ Dev dv) {
     a0 += ab;
     a1 += wx * wy * wz * (-(double)dv.eps[m] * ab + 0.5 * ab * ab);
     a2 += g;
-    if (hasx && hasy) {                                          // winding of the z-plaquette with corner (i, j)
+    if (hasx && hasy && sc(ip, jp, k)) {                         // winding of the z-plaquette with corner (i, j)
       const cd cn = at(i, jp, k), ce = at(ip, j, k);
       const cd q0 = cmc(c, e), q1 = cmc(ce, ylink(ip, j)), q2 = cmc(cn, xlink(i, jp)), q3 = cmc(c, n);
       a3 += rint((atan2(q0.y, q0.x) + atan2(q1.y, q1.x) - atan2(q2.y, q2.x) - atan2(q3.y, q3.x) + flux) / twopi);
@@ -305,15 +353,18 @@ __global__ void __launch_bounds__(256) k_obs64(const __grid_constant__ Dev dv) {
 template <class T> struct MuArrays { T *mu, *rho, *c, *xa, *xb; };
 
 template <class T>
-__device__ __forceinline__ double real_nsum(const Dev &dv, const T *__restrict__ x, const Site &s, double &centre) {
+__device__ __forceinline__ double real_nsum(const Dev &dv, const T *__restrict__ x, const Site &s, double &centre, unsigned lb = 63u) {
   const int nx = dv.nx, ny = dv.ny;
   const long long plane = (long long)nx * ny;
   const long long rowb = (long long)s.k * plane + (long long)s.j * nx;
   centre = (double)x[rowb + s.i];
-  double acc = dv.cx64 * ((double)x[rowb + s.ie] + (double)x[rowb + s.iw]) +
-               dv.cy64 * ((double)x[(long long)s.k * plane + (long long)s.jn * nx + s.i] + (double)x[(long long)s.k * plane + (long long)s.js * nx + s.i]);
+  // mirror ghost on external open faces (the clamped neighbour index IS the mirrored site); cut links contribute nothing
+  double acc = dv.cx64 * (((lb & 1u) ? (double)x[rowb + s.ie] : 0.0) + ((lb & 2u) ? (double)x[rowb + s.iw] : 0.0)) +
+               dv.cy64 * (((lb & 4u) ? (double)x[(long long)s.k * plane + (long long)s.jn * nx + s.i] : 0.0) +
+                          ((lb & 8u) ? (double)x[(long long)s.k * plane + (long long)s.js * nx + s.i] : 0.0));
   if (dv.nz > 1)
-    acc += dv.cz64 * ((double)x[(long long)s.kt * plane + (long long)s.j * nx + s.i] + (double)x[(long long)s.kb * plane + (long long)s.j * nx + s.i]);
+    acc += dv.cz64 * (((lb & 16u) ? (double)x[(long long)s.kt * plane + (long long)s.j * nx + s.i] : 0.0) +
+                      ((lb & 32u) ? (double)x[(long long)s.kb * plane + (long long)s.j * nx + s.i] : 0.0));
   return acc;
 }
 
@@ -329,9 +380,11 @@ __global__ void __launch_bounds__(128) k_mu_rhs(const __grid_constant__ Dev dv, 
   for (int j = ch.j0; j < ch.j1; ++j) {
     const Site s = site_of(dv, i, j, k);
     const long long m = (long long)i + (long long)dv.nx * (j + (long long)dv.ny * k);
+    if (dv.sc && !dv.sc[m]) { A.c[m] = (T)0; continue; }
+    const unsigned lb = link_bits(dv, s);
     double ctr;
-    const double ns = real_nsum(dv, A.mu, s, ctr);
-    const double lap = ns - dv.csum2_64 * ctr;
+    const double ns = real_nsum(dv, A.mu, s, ctr, lb);
+    const double lap = ns - link_diag(dv, lb) * ctr;
     A.c[m] = (T)(ctr + (double)ctl->h_tau * (0.5 * lap - (double)A.rho[m]));
   }
   if (blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0 && threadIdx.x == 0) {
@@ -355,9 +408,11 @@ __global__ void __launch_bounds__(128) k_mu_sweep(const __grid_constant__ Dev dv
   for (int j = ch.j0; j < ch.j1; ++j) {
     const Site s = site_of(dv, i, j, k);
     const long long m = (long long)i + (long long)dv.nx * (j + (long long)dv.ny * k);
+    if (dv.sc && !dv.sc[m]) { xout[m] = (T)0; continue; }
+    const unsigned lb = link_bits(dv, s);
     double ctr;
-    const double ns = real_nsum(dv, xin, s, ctr);
-    const double ht = (double)ctl->h_tau, d = 1.0 + 0.5 * ht * dv.csum2_64;
+    const double ns = real_nsum(dv, xin, s, ctr, lb);
+    const double ht = (double)ctl->h_tau, d = 1.0 + 0.5 * ht * link_diag(dv, lb);
     const T xn = (T)(((double)A.c[m] + 0.5 * ht * ns) / d);
     xout[m] = xn;
     const double r = d * ((double)xn - ctr);
@@ -443,6 +498,16 @@ __global__ void k_mu_controls(const __grid_constant__ Dev dv, float h_tau, float
 }
 __global__ void k_mu_sched(const __grid_constant__ Dev dv, int n) { dv.ctl->mu_sched_n = n; dv.ctl->mu_sched_pos = 0; }
 
+// zero psi and mu on the removed sites (after tdgl_set_insulators / tdgl_set_state)
+__global__ void k_apply_mask64(const __grid_constant__ Dev dv) {
+  double2 *x = dv.psi64[dv.ctl->xbuf & 1];
+  for (long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x; m < dv.N; m += (long long)gridDim.x * blockDim.x)
+    if (!dv.sc[m]) { x[m] = make_double2(0.0, 0.0); dv.mu64[m] = 0.0; }
+}
+__global__ void k_fill_u8(unsigned char *p, long long n, unsigned char v) {
+  for (long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x; m < n; m += (long long)gridDim.x * blockDim.x) p[m] = v;
+}
+
 template <class T> __global__ void k_fill_t(T *p, long long n, T v) {
   for (long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x; m < n; m += (long long)gridDim.x * blockDim.x) p[m] = v;
 }
@@ -483,6 +548,8 @@ int launch_obs64(const Dev &dv, cudaStream_t st) {                 // followed b
   k_obs64<<<g, 256, 0, st>>>(dv);
   return (int)g;
 }
+void launch_apply_mask64(const Dev &dv, cudaStream_t st) { k_apply_mask64<<<grid1(dv.N, 256, 148 * 16), 256, 0, st>>>(dv); }
+void launch_fill_u8(unsigned char *p, long long n, unsigned char v, cudaStream_t st) { k_fill_u8<<<grid1(n, 256, 148 * 16), 256, 0, st>>>(p, n, v); }
 void launch_fill64(double *p, long long n, double v, cudaStream_t st) { k_fill_t<double><<<grid1(n, 256, 148 * 16), 256, 0, st>>>(p, n, v); }
 
 // the pieces of one pseudo-time solve; `mu` = the array that holds mu^- and receives mu (T = double iff dv.fp64)

@@ -52,6 +52,9 @@ void launch_mu_sweep(const Dev &dv, void *mu, cudaStream_t st);
 void launch_mu_finish(const Dev &dv, void *mu, cudaStream_t st);
 void launch_mu_controls(const Dev &dv, float h_tau, float eps_mu, float eps_in, int max_outer, int max_inner, cudaStream_t st);
 void launch_mu_sched(const Dev &dv, int n, cudaStream_t st);
+void launch_spheres_mask(const Dev &dv, const float4 *sph, long long n, unsigned char *mask, cudaStream_t st);
+void launch_apply_mask64(const Dev &dv, cudaStream_t st);
+void launch_fill_u8(unsigned char *p, long long n, unsigned char v, cudaStream_t st);
 void launch_mu_add(const Dev &dv, float *mu, const float *delta, cudaStream_t st);
 
 #define MODE_SWEEP 0
@@ -138,6 +141,7 @@ static bool params_ok(const tdgl_params *p) {
   if (!(p->temperature >= 0.f)) return false;
   if ((p->flags & TDGL_FLAG_GAUGE_YZ) && p->nz == 1) return false;          // films use the xz gauge
   if ((p->flags & TDGL_FLAG_MU_REFINE) && (p->flags & (TDGL_FLAG_MU_ITERATIVE | TDGL_FLAG_FP64))) return false;
+  if ((p->flags & TDGL_FLAG_INSULATORS) && !(p->flags & TDGL_FLAG_FP64)) return false;   // cut links: plain kernels only
   return true;
 }
 
@@ -239,6 +243,7 @@ static size_t carve(const tdgl_params *p, char *base, Dev *dv) {
     q = take(N * sizeof(double)); if (dv) dv->mu64 = (double *)q;
     q = take(N * sizeof(float)); if (dv) dv->eps = (float *)q;
     q = take(N * sizeof(float)); if (dv) dv->scratch = (float *)q;          // sphere list of tdgl_set_pinning
+    if (p->flags & TDGL_FLAG_INSULATORS) { q = take(N); if (dv) dv->sc = (unsigned char *)q; }
   } else {
     q = take(N * sizeof(float2)); if (dv) dv->psi[0] = (float2 *)q;
     q = take(N * sizeof(float2)); if (dv) dv->psi[1] = (float2 *)q;
@@ -504,6 +509,7 @@ extern "C" int tdgl_create(const tdgl_params *p, tdgl_t **out) {
   }
   if (dv.fp64) launch_init_state64(dv, (double)p->init_amp, st);
   else launch_init_state(dv, p->init_amp, st);
+  if (dv.sc) { launch_fill_u8(dv.sc, dv.N, 1, st); h->launches += 1; }      // no site removed yet
   launch_set_field(dv, 0.0, 0.0, 0.0, st);
   launch_step_begin(dv, st);
   h->launches += 7;
@@ -541,6 +547,23 @@ extern "C" int tdgl_set_pinning(tdgl_t *h, const tdgl_sphere *sph, int64_t n, fl
     launch_spheres(h->dv, (const float4 *)h->dv.scratch, n, eps_in, h->stream);
     h->launches += (n + (1 << 20) - 1) >> 20;
   }
+  CKL();
+  return TDGL_OK;
+}
+
+extern "C" int tdgl_set_insulators(tdgl_t *h, const tdgl_sphere *sph, int64_t n) {
+  if (!h || n < 0 || (n > 0 && !sph) || n > h->dv.N / 4) return TDGL_EINVAL;
+  if (!h->dv.sc) return TDGL_EINCOMPAT;                       // created without TDGL_FLAG_INSULATORS
+  launch_fill_u8(h->dv.sc, h->dv.N, 1, h->stream);
+  h->launches += 1;
+  if (n > 0) {
+    CK(cudaMemcpyAsync(h->dv.scratch, sph, (size_t)n * sizeof(tdgl_sphere), cudaMemcpyHostToDevice, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
+    launch_spheres_mask(h->dv, (const float4 *)h->dv.scratch, n, h->dv.sc, h->stream);
+    h->launches += (n + (1 << 20) - 1) >> 20;
+  }
+  launch_apply_mask64(h->dv, h->stream);                      // psi = 0, mu = 0 on the removed sites
+  h->launches += 1;
   CKL();
   return TDGL_OK;
 }
@@ -675,7 +698,7 @@ extern "C" const char *tdgl_strerror(int code) {
     case TDGL_OK: return "ok";
     case TDGL_EINVAL: return "invalid argument (size, mesh, boundary type, pointer or struct_size)";
     case TDGL_ENOMEM: return "workspace too small or misaligned";
-    case TDGL_EINCOMPAT: return "incompatible request (open x with a current, or a field component the chosen Landau gauge cannot carry)";
+    case TDGL_EINCOMPAT: return "incompatible request (open x with a current, a field component the chosen Landau gauge cannot carry, or a call the mode chosen at create does not support)";
     case TDGL_ECUDA: return "CUDA runtime error";
     case TDGL_WMAXSWEEPS: return "warning: Jacobi iteration hit max_sweeps";
     default: return "unknown code";
@@ -733,6 +756,7 @@ extern "C" int tdgl_set_state(tdgl_t *h, const void *psi_dev, const void *mu_dev
   launch_ctl_state(h->dv, K, h->stream);
   launch_step_begin(h->dv, h->stream);
   h->launches += 2;
+  if (h->dv.sc) { launch_apply_mask64(h->dv, h->stream); h->launches += 1; }
   CKL();
   return TDGL_OK;
 }

@@ -88,6 +88,8 @@ struct Dev {
   double2 *psi64[2], *b64, *d64;
   double *mu64;
   double cx64, cy64, cz64, csum2_64, ht2_64, u64, zeta_max64;
+  // insulating inclusions (TDGL_FLAG_INSULATORS, reading S25): 1 = superconducting site, 0 = removed; nullptr = none
+  unsigned char *sc;
   // pseudo-time mu iteration (TDGL_FLAG_MU_ITERATIVE): rho, c, two Jacobi iterates (float or double), logs
   int mu_iterative;
   void *mu_rho, *mu_c, *mu_xa, *mu_xb;

@@ -230,3 +230,86 @@ def test_mode_flags_are_validated():
         s.set_mu_solver()                                          # direct solver: no iteration to control
     assert e.value.code == -1
     s.close()
+
+
+# ---------------------------------------------------------------------------------------------------
+# insulating inclusions: removed sites and cut links (TDGL_FLAG_INSULATORS, reading S25; fp64 build)
+# ---------------------------------------------------------------------------------------------------
+def insulator_pair(cfg, holes, psi0, mu0, K0, fixed_sweeps=0, eps_tol=1e-6):
+    """Oracle (sc_mask from the same inside test as the epsilon pattern) and Solver with identical inputs."""
+    from dataclasses import replace
+    from paper_1409_8340_b200 import Solver
+    p = oracle_params(cfg, fp64=True, eps_tol=eps_tol)
+    mask = O.epsilon_from_spheres(p, holes, 0.0, 1.0) > 0.5
+    p = replace(p, sc_mask=mask)
+    s = Solver(cfg.nx, cfg.ny, cfg.nz, bc=cfg.bc, h=cfg.h, dt=cfg.dt, eps_tol=eps_tol, fixed_sweeps=fixed_sweeps,
+               temperature=cfg.temperature, seed=cfg.seed, fp64=True, insulators=True)
+    spheres = I.sphere_list(cfg)
+    eps = O.epsilon_from_spheres(p, spheres, cfg.eps_in, cfg.eps_out)
+    s.set_pinning(spheres, cfg.eps_in, cfg.eps_out)
+    s.set_insulators(holes)
+    bx_req, bz_req = cfg.requested_field()
+    Bx, Bz, _, _ = O.snap_field(p, f32(bx_req), f32(bz_req))
+    s.set_field_current(Bx=bx_req, Bz=bz_req, Jx=cfg.Jx)
+    st = O.State(psi=psi0.astype(np.complex128) * mask, mu=mu0.astype(np.float64) * mask, K=float(K0))
+    s.set_state(torch.from_numpy(psi0), torch.from_numpy(mu0), float(K0))       # the library empties the removed sites
+    return p, st, eps, (Bx, Bz), s, mask
+
+
+@pytest.mark.parametrize("bc", ALL_BC)
+def test_insulating_inclusions_two_steps(bc):
+    cfg = cfg_of(36, 14, 10, bc, Bx=0.05, Bz=0.3, Jx=0.02 if bc[0] == P_ else 0.0, temperature=1e-3,
+                 incl_fraction=0.1, incl_rmin=1.0, incl_rmax=2.0, seed=2)
+    holes = np.array([[4.0, 3.0, 2.0, 1.6], [12.0, 5.0, 3.5, 2.1], [17.5, 0.5, 0.0, 1.3], [9.0, 6.5, 4.5, 0.9]], np.float32)
+    psi0, mu0 = I.random_state(cfg, seed=21, amp=0.8)
+    K0 = 0.11 if bc[0] == P_ else 0.0
+    p, st, eps, (Bx, Bz), s, mask = insulator_pair(cfg, holes, psi0, mu0, K0, fixed_sweeps=5)
+    assert 0.03 < 1.0 - mask.mean() < 0.3
+    s.step(2)
+    psi, mu = s.get_psi_mu()
+    outer, inner = s.mu_log(2)
+    for n in range(2):
+        O.step(p, st, eps, Bx, Bz, f32(cfg.Jx), fixed_sweeps=5, mu_inner_counts=inner[n])
+    psi, mu = psi.cpu().numpy(), mu.cpu().numpy()
+    assert np.all(psi[~mask] == 0.0) and np.all(mu[~mask] == 0.0)
+    assert np.max(np.abs(psi - st.psi)) < 1e-12
+    assert np.max(np.abs(mu - st.mu)) < 1e-12 * max(1.0, np.max(np.abs(st.mu)))
+    ob = s.observables()
+    assert abs(ob.K - st.K) < 1e-13 and abs(ob.Jav - st.Jav) < 1e-13
+    links = O.paper_links(p, st.K, Bx, Bz)
+    F = O.free_energy(p, st.psi, eps, links)
+    assert abs(ob.free_energy - F) < 1e-12 * abs(F)
+    assert abs(ob.mean_abs2 - O.mean_abs2(st.psi)) < 1e-14
+    assert ob.vortices_per_slice == O.vortices_per_slice(p, st.psi, links, Bz)
+    s.close()
+
+
+def test_insulating_inclusions_film_run_and_conservation():
+    """A film with holes, 30 steps with the GPU's own decisions, replayed by the oracle; the weighted sum of rho vanishes
+    (the cut-link operator is Hermitian: the Neumann problem for mu stays solvable) and no current enters a hole."""
+    cfg = cfg_of(96, 64, 1, (P_, P_, P_), nz_flux=6, Jx=0.02, seed=4)
+    holes = np.array([[10.0, 8.0, 0.0, 3.0], [30.0, 20.0, 0.0, 4.2], [40.0, 5.0, 0.0, 2.0]], np.float32)
+    psi0 = I.initial_psi(cfg)
+    p, st, eps, (Bx, Bz), s, mask = insulator_pair(cfg, holes, psi0, np.zeros((1, 64, 96), np.float32), 0.0)
+    s.step(30)
+    psi, mu = s.get_psi_mu()
+    counts, _ = s.sweep_log(30)
+    outer, inner = s.mu_log(30)
+    O.run(p, st, eps, Bx, Bz, f32(cfg.Jx), 30, sweep_counts=counts, mu_schedule=inner)
+    assert np.max(np.abs(psi.cpu().numpy() - st.psi)) < 1e-10
+    assert np.max(np.abs(mu.cpu().numpy() - st.mu)) < 1e-10
+    rho = s.debug_rho().cpu().numpy()
+    assert abs(rho.sum()) < 1e-10 * np.abs(rho).sum() and np.all(rho[~mask] == 0.0)
+    s.close()
+
+
+def test_insulators_need_the_flag():
+    from paper_1409_8340_b200 import Solver
+    from paper_1409_8340_b200.binding import TdglError
+    s = Solver(16, 8, 4, fp64=True)
+    with pytest.raises(TdglError) as e:
+        s.set_insulators(np.array([[1.0, 1.0, 1.0, 1.0]], np.float32))
+    assert e.value.code == -3
+    s.close()
+    with pytest.raises(TdglError):
+        Solver(16, 8, 4, insulators=True)                          # fp32 path has no cut links
