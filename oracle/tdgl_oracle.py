@@ -431,6 +431,109 @@ def epsilon_brute_force(p: Params, spheres, eps_in: float, eps_out: float):
     return eps
 
 
+# Further generator shapes ("ellipsoids ... cylinders", Fig. 2(d) elliptical inclusions, Fig. 2(e) +-45 degree
+# columnar defects; reading S26).  A shape is a row of 10 float32 numbers
+#     (kind, c_x, c_y, c_z, a_0, a_1, a_2, n_x, n_y, n_z)
+# kind 0 SPHERE    radius a_0                              : d_x^2 + d_y^2 + d_z^2 <= a_0^2
+# kind 1 ELLIPSOID semi-axes (a_0, a_1, a_2) along x, y, z : (d_x/a_0)^2 + (d_y/a_1)^2 + (d_z/a_2)^2 <= 1
+# kind 2 CYLINDER  radius a_0, half-length a_1, axis n (any non-zero vector, normalised in fp64):
+#                  t = d.n_hat, |t| <= a_1 and |d|^2 - t^2 <= a_0^2
+# d = site position minus centre, minimum image on periodic axes, exactly as for spheres; every product, quotient and
+# sum is a separately rounded fp64 operation in the order written (no contraction), so that a mask is reproducible.
+SHAPE_SPHERE, SHAPE_ELLIPSOID, SHAPE_CYLINDER = 0, 1, 2
+
+
+def _shape_inside(kind: int, a, nhat, dx, dy, dz):
+    """The inside test of one shape on broadcastable fp64 displacement arrays."""
+    if kind == SHAPE_SPHERE:
+        return (dx * dx + dy * dy) + dz * dz <= a[0] * a[0]
+    if kind == SHAPE_ELLIPSOID:
+        ex, ey, ez = dx / a[0], dy / a[1], dz / a[2]
+        return (ex * ex + ey * ey) + ez * ez <= 1.0
+    if kind == SHAPE_CYLINDER:
+        t = (dx * nhat[0] + dy * nhat[1]) + dz * nhat[2]
+        q = ((dx * dx + dy * dy) + dz * dz) - t * t
+        return (np.abs(t) <= a[1]) & (q <= a[0] * a[0])
+    raise ValueError(f"unknown shape kind {kind}")
+
+
+def _shape_unpack(row):
+    row = np.asarray(row, dtype=np.float32)
+    kind = int(row[0])
+    c = [float(row[1]), float(row[2]), float(row[3])]
+    a = [float(row[4]), float(row[5]), float(row[6])]
+    n = [float(row[7]), float(row[8]), float(row[9])]
+    nhat = [0.0, 0.0, 0.0]
+    if kind == SHAPE_CYLINDER:
+        nn = math.sqrt((n[0] * n[0] + n[1] * n[1]) + n[2] * n[2])
+        nhat = [n[0] / nn, n[1] / nn, n[2] / nn]
+    return kind, c, a, nhat
+
+
+def shape_half_extent(kind: int, a, nhat):
+    """Half-width of the axis-aligned bounding box of a shape along x, y, z."""
+    if kind == SHAPE_SPHERE:
+        return [a[0], a[0], a[0]]
+    if kind == SHAPE_ELLIPSOID:
+        return [a[0], a[1], a[2]]
+    # capped cylinder: |n_a| * half-length + r sqrt(1 - n_a^2)
+    return [abs(nhat[q]) * a[1] + a[0] * math.sqrt(max(0.0, 1.0 - nhat[q] * nhat[q])) for q in range(3)]
+
+
+def epsilon_from_shapes(p: Params, shapes, eps_in: float, eps_out: float):
+    """eps_m = eps_in if site m lies inside any shape of the list, else eps_out (P:511 (i), 513; S26).  Each shape is
+    tested on the sites of its bounding box only."""
+    eps = np.full(p.shape, float(eps_out))
+    n = (p.nx, p.ny, p.nz)
+    h = (float(np.float32(p.hx)), float(np.float32(p.hy)), float(np.float32(p.hz)))
+    L = tuple(n[q] * h[q] for q in range(3))
+    for row in np.asarray(shapes, dtype=np.float32).reshape(-1, 10):
+        kind, c, a, nhat = _shape_unpack(row)
+        ext = shape_half_extent(kind, a, nhat)
+        idx, dd = [], []
+        for q in range(3):
+            lo = int(math.floor((c[q] - ext[q]) / h[q])) - 1
+            hi = int(math.ceil((c[q] + ext[q]) / h[q])) + 1
+            if p.bc[q] == OPEN:
+                lo, hi = max(lo, 0), min(hi, n[q] - 1)
+            elif hi - lo + 1 >= n[q]:
+                lo, hi = 0, n[q] - 1
+            r = np.arange(lo, hi + 1)
+            ii = np.mod(r, n[q])
+            d = ii.astype(np.float64) * h[q] - c[q]
+            if p.bc[q] == PERIODIC:
+                d = d - L[q] * np.rint(d / L[q])
+            idx.append(ii)
+            dd.append(d)
+        if min(len(i) for i in idx) == 0:
+            continue
+        inside = _shape_inside(kind, a, nhat, dd[0][None, None, :], dd[1][None, :, None], dd[2][:, None, None])
+        sub = eps[np.ix_(idx[2], idx[1], idx[0])]
+        sub[inside] = float(eps_in)
+        eps[np.ix_(idx[2], idx[1], idx[0])] = sub
+    return eps
+
+
+def epsilon_shapes_brute_force(p: Params, shapes, eps_in: float, eps_out: float):
+    """The same definition as a loop over every site and every shape (tiny inputs only)."""
+    h = (float(np.float32(p.hx)), float(np.float32(p.hy)), float(np.float32(p.hz)))
+    n = (p.nx, p.ny, p.nz)
+    kk, jj, ii = np.meshgrid(np.arange(p.nz), np.arange(p.ny), np.arange(p.nx), indexing="ij")
+    pos = (ii * h[0], jj * h[1], kk * h[2])
+    eps = np.full(p.shape, float(eps_out))
+    for row in np.asarray(shapes, dtype=np.float32).reshape(-1, 10):
+        kind, c, a, nhat = _shape_unpack(row)
+        d = []
+        for q in range(3):
+            dq = pos[q] - c[q]
+            if p.bc[q] == PERIODIC:
+                Lq = n[q] * h[q]
+                dq = dq - Lq * np.rint(dq / Lq)
+            d.append(dq)
+        eps[_shape_inside(kind, a, nhat, d[0], d[1], d[2])] = float(eps_in)
+    return eps
+
+
 # --------------------------------------------------------------------------------------------------
 # the psi solve
 # --------------------------------------------------------------------------------------------------

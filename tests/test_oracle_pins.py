@@ -532,6 +532,86 @@ def test_epsilon_bounding_box_equals_brute_force(bc):
     assert int(np.sum(one < 0)) == 33          # |n|^2 <= 4 on the cubic lattice h = 0.5: 1+6+12+8+6
 
 
+def _mixed_shapes(rng, n, box):
+    sh = np.zeros((n, 10), dtype=np.float32)
+    sh[:, 0] = rng.integers(0, 3, n)
+    for q in range(3):
+        sh[:, 1 + q] = rng.uniform(0, box[q], n)
+        sh[:, 4 + q] = rng.uniform(0.4, 2.2, n)
+        sh[:, 7 + q] = rng.normal(size=n)
+    return sh
+
+
+@pytest.mark.parametrize("bc", [(P_, P_, P_), (P_, P_, O_), (O_, P_, O_), (O_, O_, O_)])
+def test_shapes_bounding_box_equals_brute_force(bc):
+    # S26 (Fig. 2d/e): spheres, axis-aligned ellipsoids, capped cylinders with any axis
+    p = O.Params(18, 14, 12, bc=bc)
+    sh = _mixed_shapes(np.random.default_rng(61), 14, (9.0, 7.0, 6.0))
+    sh[0, :7] = (2, 0.1, 0.2, 0.1, 0.8, 3.0, 0.0)          # a cylinder through the corner: minimum image
+    sh[1, :7] = (1, 8.9, 0.1, 5.9, 2.0, 1.0, 1.5)          # an ellipsoid through the opposite corner
+    e1 = O.epsilon_from_shapes(p, sh, -1.0, 1.0)
+    e2 = O.epsilon_shapes_brute_force(p, sh, -1.0, 1.0)
+    assert np.array_equal(e1, e2)
+    assert 0.05 < np.mean(e1 < 0) < 0.95
+    for kind in (0, 1, 2):                                  # and each kind on its own
+        one = sh[sh[:, 0] == kind]
+        assert len(one) > 0
+        assert np.array_equal(O.epsilon_from_shapes(p, one, -1.0, 1.0), O.epsilon_shapes_brute_force(p, one, -1.0, 1.0))
+
+
+def test_shapes_reduce_to_spheres_and_lattice_counts():
+    p = O.Params(20, 16, 14, bc=(P_, P_, O_))
+    rng = np.random.default_rng(62)
+    sph = np.stack([rng.uniform(0, 10, 7), rng.uniform(0, 8, 7), rng.uniform(0, 7, 7), rng.uniform(0.45, 2.3, 7)], 1).astype(np.float32)
+    sh = np.zeros((7, 10), dtype=np.float32)
+    sh[:, 1:5] = sph
+    ref = O.epsilon_from_spheres(p, sph, -1.0, 1.0)
+    assert np.array_equal(O.epsilon_from_shapes(p, sh, -1.0, 1.0), ref)         # kind 0 = the sphere generator
+    el = sh.copy()
+    el[:, 0] = 1
+    el[:, 5] = el[:, 4]
+    el[:, 6] = el[:, 4]
+    assert np.array_equal(O.epsilon_from_shapes(p, el, -1.0, 1.0), ref)         # equal semi-axes = a sphere
+    # ellipsoid centred on a site, semi-axes (1, 0.5, 1.5), h = 0.5: lattice points with 9 i^2 + 36 j^2 + 4 k^2 <= 36
+    want = sum(1 for i in range(-3, 4) for j in range(-3, 4) for k in range(-4, 5) if 9 * i * i + 36 * j * j + 4 * k * k <= 36)
+    one = O.epsilon_from_shapes(p, np.array([[1, 5.0, 4.0, 3.5, 1.0, 0.5, 1.5, 0, 0, 0]]), -1.0, 1.0)
+    assert int(np.sum(one < 0)) == want == 21
+    # cylinder along z through the whole (open) thickness: every slice is the disc i^2 + j^2 <= 4 (13 lattice points)
+    col = O.epsilon_from_shapes(p, np.array([[2, 5.0, 4.0, 3.0, 1.0, 50.0, 0.0, 0, 0, 2.5]]), -1.0, 1.0)
+    assert np.all(np.sum(col < 0, axis=(1, 2)) == 13)
+    assert np.all(col == col[0][None])
+    # capped: half-length 1.0 keeps the slices |k h - 3.0| <= 1.0 only
+    cap = O.epsilon_from_shapes(p, np.array([[2, 5.0, 4.0, 3.0, 1.0, 1.0, 0.0, 0, 0, 1.0]]), -1.0, 1.0)
+    assert [int(v) for v in np.sum(cap < 0, axis=(1, 2))] == [13 if abs(k * 0.5 - 3.0) <= 1.0 else 0 for k in range(14)]
+
+
+def test_shapes_cylinder_axis_covariance_and_volume():
+    # the same cylinder with its axis along x, y: the masks are transposes of each other
+    p = O.Params(24, 24, 10, bc=(P_, P_, P_))
+    cx = O.epsilon_from_shapes(p, np.array([[2, 6.0, 5.0, 2.0, 1.3, 3.1, 0, 1, 0, 0]]), -1.0, 1.0)
+    cy = O.epsilon_from_shapes(p, np.array([[2, 5.0, 6.0, 2.0, 1.3, 3.1, 0, 0, 1, 0]]), -1.0, 1.0)
+    assert np.array_equal(cx, np.swapaxes(cy, 1, 2))
+    # +-45 degree columns (Fig. 2e): a column along (1, 0, 1) is invariant under the lattice shift (i, k) -> (i+1, k+1)
+    # (x periodic, half-length far beyond the box); the -45 degree column is its mirror image i -> -i
+    p = O.Params(32, 12, 16, bc=(P_, P_, O_))
+    a = O.epsilon_from_shapes(p, np.array([[2, 8.0, 3.0, 4.0, 1.3, 100.0, 0, 1, 0, 1]]), -1.0, 1.0) < 0
+    assert 0 < a.sum()
+    assert np.array_equal(a[1:], np.roll(a, 1, axis=2)[:-1])
+    b = O.epsilon_from_shapes(p, np.array([[2, 8.0, 3.0, 4.0, 1.3, 100.0, 0, -1, 0, 1]]), -1.0, 1.0) < 0
+    assert np.array_equal(b, np.roll(a[:, :, ::-1], 2 * 16 + 1, axis=2))
+    # each slice of a 45 degree column is an ellipse of area pi r^2 sqrt(2): site count within 5 %
+    assert abs(a[8].sum() * 0.25 / (math.pi * 1.3 ** 2 * math.sqrt(2.0)) - 1.0) < 0.05
+    # volume of a tilted capped cylinder / of an ellipsoid on a fine mesh
+    pf = O.Params(64, 64, 64, hx=0.125, hy=0.125, hz=0.125, bc=(O_, O_, O_))
+    cyl = O.epsilon_from_shapes(pf, np.array([[2, 4.0, 4.0, 4.0, 1.5, 2.0, 0, 1.0, 2.0, -0.5]]), -1.0, 1.0) < 0
+    assert abs(cyl.sum() * 0.125 ** 3 / (math.pi * 1.5 ** 2 * 4.0) - 1.0) < 0.01
+    ell = O.epsilon_from_shapes(pf, np.array([[1, 4.0, 4.0, 4.0, 3.0, 1.5, 2.5, 0, 0, 0]]), -1.0, 1.0) < 0
+    assert abs(ell.sum() * 0.125 ** 3 / (4.0 / 3.0 * math.pi * 3.0 * 1.5 * 2.5) - 1.0) < 0.01
+    # point symmetry about a centre that sits on a site
+    c = O.epsilon_from_shapes(pf, np.array([[2, 4.0, 4.0, 4.0, 1.1, 1.7, 0, 0.3, -1.0, 0.8]]), -1.0, 1.0) < 0
+    assert np.array_equal(c[1:, 1:, 1:], c[1:, 1:, 1:][::-1, ::-1, ::-1])
+
+
 # ------------------------------------------------------------------------------------------------
 # single-sweep amplification of the checkerboard mode
 # ------------------------------------------------------------------------------------------------
