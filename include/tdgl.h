@@ -129,6 +129,21 @@ int tdgl_set_pinning(tdgl_t *h, const tdgl_sphere *spheres_host, int64_t n, floa
  * J_av keeps the plain 1/N mean of Eq. (35) over the links that exist. */
 int tdgl_set_insulators(tdgl_t *h, const tdgl_sphere *spheres_host, int64_t n);
 
+/* Further generator shapes ("ellipsoids ... cylinders", Fig. 2(d) elliptical inclusions, Fig. 2(e) +-45 degree
+ * columnar defects; reading S26).  Lengths in xi_0, domain coordinates; d = site position - c, minimum image on
+ * periodic axes.  Inside tests, every operation a separately rounded fp64 operation in the order written:
+ *   kind 0 sphere    : (d_x^2 + d_y^2) + d_z^2 <= a[0]^2
+ *   kind 1 ellipsoid : ((d_x/a[0])^2 + (d_y/a[1])^2) + (d_z/a[2])^2 <= 1     (semi-axes along x, y, z)
+ *   kind 2 cylinder  : t = (d_x n_x + d_y n_y) + d_z n_z with n = the given axis / its fp64 norm;
+ *                      |t| <= a[1] (half-length) and ((d_x^2 + d_y^2) + d_z^2) - t^2 <= a[0]^2 (radius)
+ * `kind` is stored as a float (0, 1, 2) so that a list is a plain float32 array of 10 columns. */
+typedef struct { float kind; float c[3]; float a[3]; float n[3]; } tdgl_shape;
+
+/* tdgl_set_pinning / tdgl_set_insulators with a list of shapes.  Same ownership and error rules; n <= N/10;
+ * TDGL_EINVAL for an unknown kind, a non-positive radius / semi-axis / half-length or a zero cylinder axis. */
+int tdgl_set_pinning_shapes(tdgl_t *h, const tdgl_shape *shapes_host, int64_t n, float eps_in, float eps_out);
+int tdgl_set_insulator_shapes(tdgl_t *h, const tdgl_shape *shapes_host, int64_t n);
+
 /* Applied field and transport current J_ext along x (Eq. 21).  The Landau gauge is fixed at create (S23):
  * xz gauge (default; Eq. 24a): B = (Bx, 0, Bz); yz gauge (TDGL_FLAG_GAUGE_YZ; Eq. 24b): B = (0, By, Bz).
  * B_z is snapped to 2 pi n_z/(Lx Ly) iff x and y are periodic; B_x to 2 pi n_x/(Ly Lz) iff y and z are; B_y to

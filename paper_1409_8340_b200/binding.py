@@ -20,7 +20,7 @@ EXPORTS = (
     "tdgl_get_psi_mu", "tdgl_observables", "tdgl_strerror", "tdgl_last_cuda_error", "tdgl_set_state", "tdgl_set_solver",
     "tdgl_set_sweep_schedule", "tdgl_get_sweep_log", "tdgl_get_eps", "tdgl_debug_noise", "tdgl_debug_poisson",
     "tdgl_debug_rho", "tdgl_launch_count", "tdgl_sweep_timing", "tdgl_mu_gain", "tdgl_mu_refine_enabled",
-    "tdgl_set_mu_solver", "tdgl_get_mu_log", "tdgl_set_insulators",
+    "tdgl_set_mu_solver", "tdgl_get_mu_log", "tdgl_set_insulators", "tdgl_set_pinning_shapes", "tdgl_set_insulator_shapes",
 )
 
 
@@ -95,6 +95,8 @@ def lib() -> C.CDLL:
     L.tdgl_mu_refine_enabled.argtypes = [vp]
     L.tdgl_set_mu_solver.argtypes = [vp, f32, f32, f32, i32, i32]
     L.tdgl_set_insulators.argtypes = [vp, C.POINTER(TdglSphere), i64]
+    L.tdgl_set_pinning_shapes.argtypes = [vp, vp, i64, f32, f32]
+    L.tdgl_set_insulator_shapes.argtypes = [vp, vp, i64]
     L.tdgl_get_mu_log.argtypes = [vp, i32, C.POINTER(i32), C.POINTER(i32), i32, C.POINTER(i32)]
     _lib = L
     return L
@@ -133,6 +135,17 @@ def tdgl_set_pinning(h, spheres: np.ndarray, eps_in: float, eps_out: float) -> N
     s = np.ascontiguousarray(spheres, dtype=np.float32).reshape(-1, 4)
     ptr = s.ctypes.data_as(C.POINTER(TdglSphere)) if len(s) else None
     _check(lib().tdgl_set_pinning(h, ptr, len(s), eps_in, eps_out), "tdgl_set_pinning", h)
+
+
+def tdgl_set_pinning_shapes(h, shapes: np.ndarray, eps_in: float, eps_out: float) -> None:
+    """shapes: float32 array (n, 10) = (kind, c[3], a[3], n[3]) (tdgl_shape), HOST memory."""
+    s = np.ascontiguousarray(shapes, dtype=np.float32).reshape(-1, 10)
+    _check(lib().tdgl_set_pinning_shapes(h, s.ctypes.data if len(s) else None, len(s), eps_in, eps_out), "tdgl_set_pinning_shapes", h)
+
+
+def tdgl_set_insulator_shapes(h, shapes: np.ndarray) -> None:
+    s = np.ascontiguousarray(shapes, dtype=np.float32).reshape(-1, 10)
+    _check(lib().tdgl_set_insulator_shapes(h, s.ctypes.data if len(s) else None, len(s)), "tdgl_set_insulator_shapes", h)
 
 
 def tdgl_set_field_current(h, Bx: float, By: float, Bz: float, Jx: float) -> None:
@@ -215,6 +228,12 @@ class Solver:
         s = np.ascontiguousarray(spheres, dtype=np.float32).reshape(-1, 4)
         ptr = s.ctypes.data_as(C.POINTER(TdglSphere)) if len(s) else None
         _check(lib().tdgl_set_insulators(self.h, ptr, len(s)), "tdgl_set_insulators", self.h)
+
+    def set_pinning_shapes(self, shapes, eps_in=-1.0, eps_out=1.0):
+        tdgl_set_pinning_shapes(self.h, shapes, eps_in, eps_out)
+
+    def set_insulator_shapes(self, shapes):
+        tdgl_set_insulator_shapes(self.h, shapes)
 
     def set_field_current(self, Bx=0.0, By=0.0, Bz=0.0, Jx=0.0):
         tdgl_set_field_current(self.h, Bx, By, Bz, Jx)

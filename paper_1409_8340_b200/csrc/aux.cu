@@ -149,6 +149,78 @@ __global__ void __launch_bounds__(128) k_spheres(const __grid_constant__ Dev dv,
   }
 }
 
+// Further generator shapes (Fig. 2d/e; reading S26): one CTA per shape walks the shape's bounding box.
+// A shape is 10 floats (kind, c[3], a[3], n[3]): 0 sphere (radius a0), 1 axis-aligned ellipsoid (semi-axes a),
+// 2 capped cylinder (radius a0, half-length a1, axis n normalised here in fp64).  As in k_spheres every fp64
+// operation of the inside test is rounded separately, in the order of include/tdgl.h.
+__global__ void __launch_bounds__(128) k_shapes(const __grid_constant__ Dev dv, const float *__restrict__ shp, float eps_in,
+                                                unsigned char *mask) {
+  const float *s = shp + 10ll * blockIdx.x;
+  const int kind = (int)s[0];
+  const int n[3] = {dv.nx, dv.ny, dv.nz};
+  const int bc[3] = {dv.bcx, dv.bcy, dv.bcz};
+  const double h[3] = {dv.hx, dv.hy, dv.hz};
+  const double cc[3] = {(double)s[1], (double)s[2], (double)s[3]};
+  const double a[3] = {(double)s[4], (double)s[5], (double)s[6]};
+  double nh[3] = {0.0, 0.0, 0.0};
+  double ext[3] = {a[0], a[0], a[0]};
+  if (kind == 1) { ext[1] = a[1]; ext[2] = a[2]; }
+  if (kind == 2) {
+    const double v[3] = {(double)s[7], (double)s[8], (double)s[9]};
+    const double nn = __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(v[0], v[0]), __dmul_rn(v[1], v[1])), __dmul_rn(v[2], v[2])));
+    for (int q = 0; q < 3; ++q) {
+      nh[q] = __ddiv_rn(v[q], nn);
+      ext[q] = fabs(nh[q]) * a[1] + a[0] * sqrt(fmax(0.0, 1.0 - nh[q] * nh[q])) + 1e-9;   // box only: any cover will do
+    }
+  }
+  if (kind < 0 || kind > 2) return;
+  int lo[3], cnt3[3];
+  for (int q = 0; q < 3; ++q) {
+    int l = (int)floor((cc[q] - ext[q]) / h[q]) - 1, u = (int)ceil((cc[q] + ext[q]) / h[q]) + 1;
+    if (bc[q] == 1) { l = max(l, 0); u = min(u, n[q] - 1); }
+    else if (u - l + 1 >= n[q]) { l = 0; u = n[q] - 1; }
+    lo[q] = l;
+    cnt3[q] = max(0, u - l + 1);
+  }
+  const double r2 = __dmul_rn(a[0], a[0]);
+  const long long cnt = (long long)cnt3[0] * cnt3[1] * cnt3[2];
+  for (long long t = threadIdx.x; t < cnt; t += blockDim.x) {
+    const int qx = (int)(t % cnt3[0]);
+    const long long rest = t / cnt3[0];
+    const int qq[3] = {lo[0] + qx, lo[1] + (int)(rest % cnt3[1]), lo[2] + (int)(rest / cnt3[1])};
+    int idx[3];
+    double d[3];
+    for (int q = 0; q < 3; ++q) {
+      int ii = qq[q] % n[q];
+      if (ii < 0) ii += n[q];
+      idx[q] = ii;
+      double dd = __dsub_rn(__dmul_rn((double)ii, h[q]), cc[q]);
+      if (bc[q] == 0) {
+        const double L = __dmul_rn((double)n[q], h[q]);
+        dd = __dsub_rn(dd, __dmul_rn(L, rint(__ddiv_rn(dd, L))));
+      }
+      d[q] = dd;
+    }
+    bool in;
+    if (kind == 1) {
+      const double ex = __ddiv_rn(d[0], a[0]), ey = __ddiv_rn(d[1], a[1]), ez = __ddiv_rn(d[2], a[2]);
+      in = __dadd_rn(__dadd_rn(__dmul_rn(ex, ex), __dmul_rn(ey, ey)), __dmul_rn(ez, ez)) <= 1.0;
+    } else {
+      const double dsq = __dadd_rn(__dadd_rn(__dmul_rn(d[0], d[0]), __dmul_rn(d[1], d[1])), __dmul_rn(d[2], d[2]));
+      if (kind == 0) in = dsq <= r2;
+      else {
+        const double tt = __dadd_rn(__dadd_rn(__dmul_rn(d[0], nh[0]), __dmul_rn(d[1], nh[1])), __dmul_rn(d[2], nh[2]));
+        in = fabs(tt) <= a[1] && __dsub_rn(dsq, __dmul_rn(tt, tt)) <= r2;
+      }
+    }
+    if (in) {
+      const long long m = idx[0] + (long long)dv.nx * (idx[1] + (long long)dv.ny * idx[2]);
+      if (mask) mask[m] = 0;
+      else dv.eps[m] = eps_in;
+    }
+  }
+}
+
 // zeta_m of step `step` (Eq. 39; S11) exactly as the init kernel draws it.
 __global__ void k_noise(const __grid_constant__ Dev dv, long long step, float2 *out) {
   for (long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x; m < dv.N; m += (long long)gridDim.x * blockDim.x) {
@@ -293,6 +365,12 @@ static void spheres_impl(const Dev &dv, const float4 *sph, long long n, float ep
 void launch_spheres(const Dev &dv, const float4 *sph, long long n, float eps_in, cudaStream_t st) { spheres_impl(dv, sph, n, eps_in, st, nullptr); }
 void launch_spheres_mask(const Dev &dv, const float4 *sph, long long n, unsigned char *mask, cudaStream_t st) {
   spheres_impl(dv, sph, n, 0.f, st, mask);
+}
+void launch_shapes(const Dev &dv, const float *shp, long long n, float eps_in, unsigned char *mask, cudaStream_t st) {
+  for (long long off = 0; off < n; off += 1 << 20) {
+    const unsigned g = (unsigned)((n - off) < (1 << 20) ? (n - off) : (1 << 20));
+    k_shapes<<<g, 128, 0, st>>>(dv, shp + 10 * off, eps_in, mask);
+  }
 }
 void launch_copy_psi(const Dev &dv, float2 *out, cudaStream_t st) { k_copy_psi<<<grid_for(dv.N / 2, 256, 148 * 16), 256, 0, st>>>(dv, out); }
 void launch_noise(const Dev &dv, long long step, float2 *out, cudaStream_t st) { k_noise<<<grid_for(dv.N, 256, 148 * 16), 256, 0, st>>>(dv, step, out); }

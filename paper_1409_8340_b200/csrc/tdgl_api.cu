@@ -53,6 +53,7 @@ void launch_mu_finish(const Dev &dv, void *mu, cudaStream_t st);
 void launch_mu_controls(const Dev &dv, float h_tau, float eps_mu, float eps_in, int max_outer, int max_inner, cudaStream_t st);
 void launch_mu_sched(const Dev &dv, int n, cudaStream_t st);
 void launch_spheres_mask(const Dev &dv, const float4 *sph, long long n, unsigned char *mask, cudaStream_t st);
+void launch_shapes(const Dev &dv, const float *shp, long long n, float eps_in, unsigned char *mask, cudaStream_t st);
 void launch_apply_mask64(const Dev &dv, cudaStream_t st);
 void launch_fill_u8(unsigned char *p, long long n, unsigned char v, cudaStream_t st);
 void launch_mu_add(const Dev &dv, float *mu, const float *delta, cudaStream_t st);
@@ -560,6 +561,47 @@ extern "C" int tdgl_set_insulators(tdgl_t *h, const tdgl_sphere *sph, int64_t n)
     CK(cudaMemcpyAsync(h->dv.scratch, sph, (size_t)n * sizeof(tdgl_sphere), cudaMemcpyHostToDevice, h->stream));
     CK(cudaStreamSynchronize(h->stream));
     launch_spheres_mask(h->dv, (const float4 *)h->dv.scratch, n, h->dv.sc, h->stream);
+    h->launches += (n + (1 << 20) - 1) >> 20;
+  }
+  launch_apply_mask64(h->dv, h->stream);                      // psi = 0, mu = 0 on the removed sites
+  h->launches += 1;
+  CKL();
+  return TDGL_OK;
+}
+
+static bool shapes_ok(const tdgl_shape *shp, int64_t n) {
+  for (int64_t q = 0; q < n; ++q) {
+    const tdgl_shape &s = shp[q];
+    if (s.kind < 0.f || s.kind > 2.f || s.kind != (float)(int)s.kind || !(s.a[0] > 0.f)) return false;
+    if (s.kind == 1.f && (!(s.a[1] > 0.f) || !(s.a[2] > 0.f))) return false;
+    if (s.kind == 2.f && (!(s.a[1] > 0.f) || !(s.n[0] * s.n[0] + s.n[1] * s.n[1] + s.n[2] * s.n[2] > 0.f))) return false;
+  }
+  return true;
+}
+
+extern "C" int tdgl_set_pinning_shapes(tdgl_t *h, const tdgl_shape *shp, int64_t n, float eps_in, float eps_out) {
+  if (!h || n < 0 || (n > 0 && !shp) || n > h->dv.N / 10 || !shapes_ok(shp, n)) return TDGL_EINVAL;
+  launch_fill(h->dv.eps, h->dv.N, eps_out, h->stream);
+  h->launches += 1;
+  if (n > 0) {
+    CK(cudaMemcpyAsync(h->dv.scratch, shp, (size_t)n * sizeof(tdgl_shape), cudaMemcpyHostToDevice, h->stream));
+    CK(cudaStreamSynchronize(h->stream));       // the host list may be freed on return
+    launch_shapes(h->dv, (const float *)h->dv.scratch, n, eps_in, nullptr, h->stream);
+    h->launches += (n + (1 << 20) - 1) >> 20;
+  }
+  CKL();
+  return TDGL_OK;
+}
+
+extern "C" int tdgl_set_insulator_shapes(tdgl_t *h, const tdgl_shape *shp, int64_t n) {
+  if (!h || n < 0 || (n > 0 && !shp) || n > h->dv.N / 10 || !shapes_ok(shp, n)) return TDGL_EINVAL;
+  if (!h->dv.sc) return TDGL_EINCOMPAT;                       // created without TDGL_FLAG_INSULATORS
+  launch_fill_u8(h->dv.sc, h->dv.N, 1, h->stream);
+  h->launches += 1;
+  if (n > 0) {
+    CK(cudaMemcpyAsync(h->dv.scratch, shp, (size_t)n * sizeof(tdgl_shape), cudaMemcpyHostToDevice, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
+    launch_shapes(h->dv, (const float *)h->dv.scratch, n, 0.f, h->dv.sc, h->stream);
     h->launches += (n + (1 << 20) - 1) >> 20;
   }
   launch_apply_mask64(h->dv, h->stream);                      // psi = 0, mu = 0 on the removed sites

@@ -155,3 +155,27 @@ def sphere_list(cfg: Config, seed: Optional[int] = None) -> np.ndarray:
     out[:, 2] = rng.uniform(0.0, lz, n_s)
     out[:, 3] = rng.uniform(a, b, n_s) if b > a else a
     return out
+
+
+def shape_list(cfg: Config, n_ellipsoids: int, n_columns: int, seed: Optional[int] = None) -> np.ndarray:
+    """Seeded list of the further generator shapes (Fig. 2d/e), float32 array (n, 10) =
+    (kind, c_x, c_y, c_z, a_0, a_1, a_2, n_x, n_y, n_z): `n_ellipsoids` axis-aligned ellipsoids (kind 1) with semi-axes
+    uniform in [rmin, 2 rmax] at uniform random centres, then `n_columns` columnar defects (kind 2) of radius uniform
+    in [rmin, rmax] through the whole thickness, tilted by +45 or -45 degrees from z in the xz plane with equal
+    probability (Fig. 2e)."""
+    lx, ly, lz = cfg.lengths()
+    a, b = max(cfg.incl_rmin, 0.5), max(cfg.incl_rmax, 1.0)
+    rng = np.random.default_rng((cfg.seed if seed is None else seed) + 104729)
+    n = n_ellipsoids + n_columns
+    out = np.zeros((n, 10), dtype=np.float32)
+    out[:, 1] = rng.uniform(0.0, lx, n)
+    out[:, 2] = rng.uniform(0.0, ly, n)
+    out[:, 3] = rng.uniform(0.0, lz, n)
+    out[:n_ellipsoids, 0] = 1
+    out[:n_ellipsoids, 4:7] = rng.uniform(a, 2.0 * b, (n_ellipsoids, 3))
+    out[n_ellipsoids:, 0] = 2
+    out[n_ellipsoids:, 4] = rng.uniform(a, b, n_columns)
+    out[n_ellipsoids:, 5] = 2.0 * (lx + ly + lz)                    # half-length: beyond the box
+    out[n_ellipsoids:, 7] = rng.choice([-1.0, 1.0], n_columns)
+    out[n_ellipsoids:, 9] = 1.0
+    return out

@@ -84,6 +84,70 @@ def test_epsilon_mask_sphere_larger_than_box():
     s.close()
 
 
+@pytest.mark.parametrize("bc", [(P_, P_, P_), (P_, P_, O_), (O_, O_, O_), (O_, P_, O_)])
+def test_shape_mask_identical(bc):
+    """Further generator shapes (S26; Fig. 2d/e): ellipsoids, +-45 degree columns, a few spheres and
+    arbitrarily oriented capped cylinders -- the mask must be the oracle's bit for bit."""
+    cfg = cfg_of(44, 30, 20, bc, incl_rmin=0.8, incl_rmax=1.7, seed=8)
+    p = oracle_params(cfg)
+    s = make_solver(cfg)
+    sh = I.shape_list(cfg, 9, 5)
+    rng = np.random.default_rng(3)
+    extra = np.zeros((6, 10), np.float32)
+    extra[:3, 0] = 2                                                 # capped cylinders with any axis
+    extra[:, 1:4] = rng.uniform(0, 10, (6, 3))
+    extra[:, 4:7] = rng.uniform(0.6, 2.5, (6, 3))
+    extra[:, 7:10] = rng.normal(size=(6, 3))
+    extra[5, 1:5] = (0.1, 0.2, 0.1, 3.0)                             # a sphere through the corner (kind 0)
+    sh = np.concatenate([sh, extra])
+    s.set_pinning_shapes(sh, -1.0, 1.0)
+    eps = s.get_eps().cpu().numpy()
+    ref = O.epsilon_from_shapes(p, sh, -1.0, 1.0)
+    assert np.array_equal(eps, ref.astype(np.float32))
+    assert 0.05 < (eps < 0).mean() < 0.7
+    for kind in (0, 1, 2):
+        one = sh[sh[:, 0] == kind]
+        s.set_pinning_shapes(one, -0.5, 1.0)
+        assert np.array_equal(s.get_eps().cpu().numpy(), O.epsilon_from_shapes(p, one, -0.5, 1.0).astype(np.float32))
+    s.set_pinning_shapes(np.zeros((0, 10), np.float32), -1.0, 0.5)  # empty list
+    assert np.all(s.get_eps().cpu().numpy() == np.float32(0.5))
+    from paper_1409_8340_b200.binding import TdglError
+    bad = sh[:2].copy()
+    bad[1, 0] = 3                                                    # unknown kind
+    with pytest.raises(TdglError):
+        s.set_pinning_shapes(bad)
+    bad = sh[-8:-7].copy()
+    bad[0, 7:10] = 0                                                 # a column without an axis
+    assert bad[0, 0] == 2
+    with pytest.raises(TdglError):
+        s.set_pinning_shapes(bad)
+    s.close()
+
+
+def test_columnar_defects_run():
+    """Fig. 2(e): +-45 degree columnar defects in a vertical field, 40 noisy driven steps against the oracle."""
+    cfg = cfg_of(64, 32, 24, (P_, P_, O_), Bz=0.3, Jx=0.02, temperature=1e-3, incl_rmin=1.0, incl_rmax=1.5, seed=12)
+    p = oracle_params(cfg)
+    s = make_solver(cfg)
+    sh = I.shape_list(cfg, 3, 6)
+    eps = O.epsilon_from_shapes(p, sh, -1.0, 1.0)
+    s.set_pinning_shapes(sh, -1.0, 1.0)
+    bx_req, bz_req = cfg.requested_field()
+    Bx, Bz, _, _ = O.snap_field(p, f32(bx_req), f32(bz_req))
+    s.set_field_current(Bx=bx_req, Bz=bz_req, Jx=cfg.Jx)
+    psi0 = I.initial_psi(cfg)
+    st = O.State(psi=psi0.astype(np.complex128), mu=np.zeros(p.shape))
+    s.set_state(torch.from_numpy(psi0), torch.zeros(p.shape, dtype=torch.float32), 0.0)
+    s.step(40)
+    counts, _ = s.sweep_log(40)
+    O.run(p, st, eps, Bx, Bz, f32(cfg.Jx), 40, sweep_counts=counts)
+    psi, mu = s.get_psi_mu()
+    assert np.max(np.abs(psi.cpu().numpy() - st.psi)) <= 1e-4
+    assert rel_l2(psi.cpu().numpy(), st.psi) <= 1e-5
+    assert np.max(np.abs(mu.cpu().numpy() - st.mu)) <= 1e-4 * max(1.0, np.max(np.abs(st.mu)))
+    s.close()
+
+
 # ---------------------------------------------------------------------------------------------------
 # a6: rho = div j_s
 # ---------------------------------------------------------------------------------------------------

@@ -240,14 +240,15 @@ def insulator_pair(cfg, holes, psi0, mu0, K0, fixed_sweeps=0, eps_tol=1e-6):
     from dataclasses import replace
     from paper_1409_8340_b200 import Solver
     p = oracle_params(cfg, fp64=True, eps_tol=eps_tol)
-    mask = O.epsilon_from_spheres(p, holes, 0.0, 1.0) > 0.5
+    shapes = np.asarray(holes).shape[-1] == 10               # a tdgl_shape list (S26) instead of spheres
+    mask = (O.epsilon_from_shapes if shapes else O.epsilon_from_spheres)(p, holes, 0.0, 1.0) > 0.5
     p = replace(p, sc_mask=mask)
     s = Solver(cfg.nx, cfg.ny, cfg.nz, bc=cfg.bc, h=cfg.h, dt=cfg.dt, eps_tol=eps_tol, fixed_sweeps=fixed_sweeps,
                temperature=cfg.temperature, seed=cfg.seed, fp64=True, insulators=True)
     spheres = I.sphere_list(cfg)
     eps = O.epsilon_from_spheres(p, spheres, cfg.eps_in, cfg.eps_out)
     s.set_pinning(spheres, cfg.eps_in, cfg.eps_out)
-    s.set_insulators(holes)
+    (s.set_insulator_shapes if shapes else s.set_insulators)(holes)
     bx_req, bz_req = cfg.requested_field()
     Bx, Bz, _, _ = O.snap_field(p, f32(bx_req), f32(bz_req))
     s.set_field_current(Bx=bx_req, Bz=bz_req, Jx=cfg.Jx)
@@ -281,6 +282,29 @@ def test_insulating_inclusions_two_steps(bc):
     assert abs(ob.free_energy - F) < 1e-12 * abs(F)
     assert abs(ob.mean_abs2 - O.mean_abs2(st.psi)) < 1e-14
     assert ob.vortices_per_slice == O.vortices_per_slice(p, st.psi, links, Bz)
+    s.close()
+
+
+@pytest.mark.parametrize("bc", [(P_, P_, O_), (O_, O_, O_)])
+def test_insulating_shapes_two_steps(bc):
+    """Insulating ellipsoids and +-45 degree columns (S25 with the shapes of S26)."""
+    cfg = cfg_of(40, 16, 12, bc, Bz=0.3, Jx=0.02 if bc[0] == P_ else 0.0, temperature=1e-3, seed=6)
+    holes = np.array([[1, 5.0, 3.0, 2.0, 2.2, 1.1, 1.6, 0, 0, 0],
+                      [2, 12.0, 5.0, 3.0, 1.2, 100.0, 0, 1, 0, 1],
+                      [2, 16.0, 2.0, 3.0, 0.9, 100.0, 0, -1, 0, 1],
+                      [0, 0.2, 0.1, 5.9, 1.4, 0, 0, 0, 0, 0]], np.float32)
+    psi0, mu0 = I.random_state(cfg, seed=22, amp=0.8)
+    p, st, eps, (Bx, Bz), s, mask = insulator_pair(cfg, holes, psi0, mu0, 0.07 if bc[0] == P_ else 0.0, fixed_sweeps=4)
+    assert 0.03 < 1.0 - mask.mean() < 0.4
+    s.step(2)
+    psi, mu = s.get_psi_mu()
+    outer, inner = s.mu_log(2)
+    for n in range(2):
+        O.step(p, st, eps, Bx, Bz, f32(cfg.Jx), fixed_sweeps=4, mu_inner_counts=inner[n])
+    psi, mu = psi.cpu().numpy(), mu.cpu().numpy()
+    assert np.all(psi[~mask] == 0.0) and np.all(mu[~mask] == 0.0)
+    assert np.max(np.abs(psi - st.psi)) < 1e-12
+    assert np.max(np.abs(mu - st.mu)) < 1e-12 * max(1.0, np.max(np.abs(st.mu)))
     s.close()
 
 
