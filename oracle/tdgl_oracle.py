@@ -346,16 +346,23 @@ def zeta_max(p: Params) -> float:
 
 def langevin_noise(p: Params, step: int):
     """zeta_m = zeta_max (r1 + i r2), r uniform in (-1, 1), independent per site and step (P:353);
-    Philox stream 0, counter (m, step) (S11)."""
+    Philox stream 0, one call per site PAIR (reading S11'; see langevin_noise_at)."""
     return langevin_noise_at(p, step, np.arange(p.n_sites, dtype=np.uint64)).reshape(p.shape)
 
 
 def langevin_noise_at(p: Params, step: int, m):
-    """The Langevin term of `langevin_noise` at the global site indices m = i + nx (j + ny k) (any shape)."""
+    """The Langevin term of `langevin_noise` at the global site indices m = i + nx (j + ny k) (any shape).
+    Reading S11': the four words of ONE Philox4x32-10 call serve the two sites of a pair -- key = seed,
+    counter = (m_e lo, m_e hi, step, stream 0) with m_e = m - (m mod 2) the even site of the pair; site m_e takes
+    the words (x0, x1) as (re, im), site m_e + 1 the words (x2, x3).  nx is even, so a pair never straddles a row.
+    The four output words of a Philox call are as independent as the words of different calls (Salmon et al., SC'11)."""
     m = np.asarray(m, dtype=np.uint64)
-    x0, x1, _, _ = philox.philox4x32_10(m & np.uint64(0xFFFFFFFF), m >> np.uint64(32), step, 0,
-                                        p.seed & 0xFFFFFFFF, (p.seed >> 32) & 0xFFFFFFFF)
-    return zeta_max(p) * (philox.uniform_pm1(x0) + 1j * philox.uniform_pm1(x1))
+    me = m & ~np.uint64(1)
+    x0, x1, x2, x3 = philox.philox4x32_10(me & np.uint64(0xFFFFFFFF), me >> np.uint64(32), step, 0,
+                                          p.seed & 0xFFFFFFFF, (p.seed >> 32) & 0xFFFFFFFF)
+    odd = (m & np.uint64(1)) == np.uint64(1)
+    re, im = np.where(odd, x2, x0), np.where(odd, x3, x1)
+    return zeta_max(p) * (philox.uniform_pm1(re) + 1j * philox.uniform_pm1(im))
 
 
 def box_muller(x0, x1):

@@ -65,25 +65,48 @@ __device__ __forceinline__ float4 cmulc4(float2 a, const float4 &v) {     // con
   return make_float4(p.x, p.y, q.x, q.y);
 }
 
-// per-thread link constants, already scaled:  f c_x U_x(j),  f c_z U_z(j),  f c_y   (f = h_t/2 or 1)
-struct Links { float2 ux, uz; float cy; };
+// packed fp32x2 arithmetic of sm_100 (one instruction for the (re, im) pair of a site: FADD2 / FMUL2 / FFMA2)
+typedef unsigned long long u64;
+__device__ __forceinline__ u64 pk2(float a, float b) { u64 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a), "f"(b)); return r; }
+__device__ __forceinline__ u64 pk2(float2 a) { return pk2(a.x, a.y); }
+__device__ __forceinline__ float2 upk2(u64 a) { float2 r; asm("mov.b64 {%0, %1}, %2;" : "=f"(r.x), "=f"(r.y) : "l"(a)); return r; }
+__device__ __forceinline__ u64 add2(u64 a, u64 b) { u64 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ u64 sub2(u64 a, u64 b) { u64 r; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ u64 mul2(u64 a, u64 b) { u64 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c) { u64 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
 
-// s += f [ c_x (U_x E + U_x* W) + c_y (N + S) + c_z (U_z T + U_z* B) ]  for the two sites of a pair:
-//   U E + U* W = U.re (E + W) + i U.im (E - W): 10 adds and 10 FMAs per site (Eq. 29a)
+// per-thread link constants, already scaled:  f c_x U_x(j),  f c_z U_z(j),  f c_y   (f = h_t/2 or 1), each component
+// broadcast to both halves of a packed pair
+struct Links { u64 uxr, uxi, uzr, uzi, cy; };
+__device__ __forceinline__ Links make_links(float2 ux, float2 uz, float cy) {
+  Links L;
+  L.uxr = pk2(ux.x, ux.x); L.uxi = pk2(ux.y, ux.y);
+  L.uzr = pk2(uz.x, uz.x); L.uzi = pk2(uz.y, uz.y);
+  L.cy = pk2(cy, cy);
+  return L;
+}
+
+// s += f [ c_x (U_x E + U_x* W) + c_y (N + S) + c_z (U_z T + U_z* B) ]  for one site (Eq. 29a):
+//   U E + U* W = U.re (E + W) + i U.im (E - W);  the real multiples are gathered in a1 (which starts from s), the
+//   multiples of i in a2, on (re, im) pairs: 5 packed adds, 1 packed product, 4 packed FMAs and the final
+//   s = a1 + i a2 (2 scalar adds) per site
+__device__ __forceinline__ float2 nsum_site(const Links &L, float2 s, float2 W, float2 E, float2 N, float2 S, float2 T,
+                                            float2 B) {
+  const u64 e = pk2(E), w = pk2(W), t = pk2(T), b = pk2(B);
+  u64 a1 = fma2(L.uxr, add2(e, w), pk2(s));
+  u64 a2 = mul2(L.uxi, sub2(e, w));
+  a1 = fma2(L.cy, add2(pk2(N), pk2(S)), a1);
+  a1 = fma2(L.uzr, add2(t, b), a1);
+  a2 = fma2(L.uzi, sub2(t, b), a2);
+  const float2 r = upk2(a1), q = upk2(a2);
+  return make_float2(r.x - q.y, r.y + q.x);
+}
 __device__ __forceinline__ void nsum_pair(const Links &L, const float4 &C, const float2 &W, const float2 &E,
                                           const float4 &Nn, const float4 &Ss, const float4 &T, const float4 &B,
                                           float2 &s0, float2 &s1) {
   // site 0: west W, east C.hi;  site 1: west C.lo, east E
-  s0.x = fmaf(L.ux.x, C.z + W.x, s0.x);  s0.x = fmaf(-L.ux.y, C.w - W.y, s0.x);
-  s0.y = fmaf(L.ux.x, C.w + W.y, s0.y);  s0.y = fmaf(L.ux.y, C.z - W.x, s0.y);
-  s1.x = fmaf(L.ux.x, E.x + C.x, s1.x);  s1.x = fmaf(-L.ux.y, E.y - C.y, s1.x);
-  s1.y = fmaf(L.ux.x, E.y + C.y, s1.y);  s1.y = fmaf(L.ux.y, E.x - C.x, s1.y);
-  s0.x = fmaf(L.cy, Nn.x + Ss.x, s0.x);  s0.y = fmaf(L.cy, Nn.y + Ss.y, s0.y);
-  s1.x = fmaf(L.cy, Nn.z + Ss.z, s1.x);  s1.y = fmaf(L.cy, Nn.w + Ss.w, s1.y);
-  s0.x = fmaf(L.uz.x, T.x + B.x, s0.x);  s0.x = fmaf(-L.uz.y, T.y - B.y, s0.x);
-  s0.y = fmaf(L.uz.x, T.y + B.y, s0.y);  s0.y = fmaf(L.uz.y, T.x - B.x, s0.y);
-  s1.x = fmaf(L.uz.x, T.z + B.z, s1.x);  s1.x = fmaf(-L.uz.y, T.w - B.w, s1.x);
-  s1.y = fmaf(L.uz.x, T.w + B.w, s1.y);  s1.y = fmaf(L.uz.y, T.z - B.z, s1.y);
+  s0 = nsum_site(L, s0, W, hi(C), lo(Nn), lo(Ss), lo(T), lo(B));
+  s1 = nsum_site(L, s1, lo(C), E, hi(Nn), hi(Ss), hi(T), hi(B));
 }
 
 // x^{l+1} = n / d for both sites of a pair (Eq. 33) and |r^l|^2 = |d|^2 |x^{l+1} - x^l|^2 (S8)
@@ -92,10 +115,11 @@ __device__ __forceinline__ float4 divide_pair(const float2 &n0, const float2 &n1
   const float m0 = d.x * d.x + d.y * d.y, m1 = d.z * d.z + d.w * d.w;
   const float i0 = rcp_approx(m0), i1 = rcp_approx(m1);
   const float2 y0 = cmulc(lo(d), n0), y1 = cmulc(hi(d), n1);
-  const float4 out = make_float4(y0.x * i0, y0.y * i0, y1.x * i1, y1.y * i1);
-  const float e0x = out.x - C.x, e0y = out.y - C.y, e1x = out.z - C.z, e1y = out.w - C.w;
-  rmax = fmaxf(rmax, fmaxf((e0x * e0x + e0y * e0y) * m0, (e1x * e1x + e1y * e1y) * m1));
-  return out;
+  const u64 o0 = mul2(pk2(y0), pk2(i0, i0)), o1 = mul2(pk2(y1), pk2(i1, i1));
+  const float2 e0 = upk2(sub2(o0, pk2(lo(C)))), e1 = upk2(sub2(o1, pk2(hi(C))));
+  rmax = fmaxf(rmax, fmaxf((e0.x * e0.x + e0.y * e0.y) * m0, (e1.x * e1.x + e1.y * e1.y) * m1));
+  const float2 a = upk2(o0), b = upk2(o1);
+  return make_float4(a.x, a.y, b.x, b.y);
 }
 
 // The decision taken by the last CTA of a sweep (Eq. 34; S8: residual of the input iterate,

@@ -160,13 +160,9 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_march_tma(const __grid_constant
   const bool xopen = !px && (i0 == 0 || i0 + nv == nx);             // CTA-uniform
 
   const float f = (MODE == MODE_RHO) ? 1.f : dv.ht2;
-  Links L;
-  {
-    const float2 Ux = dv.Ux[jc], Uz = dv.Uz[jc];
-    L.ux = make_float2(f * dv.cx * Ux.x, f * dv.cx * Ux.y);
-    L.uz = make_float2(f * dv.cz * Uz.x, f * dv.cz * Uz.y);
-    L.cy = f * dv.cy;
-  }
+  const float2 Uxj = dv.Ux[jc], Uzj = dv.Uz[jc];
+  const float2 Lux = make_float2(f * dv.cx * Uxj.x, f * dv.cx * Uxj.y);
+  const Links L = make_links(Lux, make_float2(f * dv.cz * Uzj.x, f * dv.cz * Uzj.y), f * dv.cy);
   const int icA = min(iA, nx - 2), icB = min(iB, nx - 2);
   float4 uyA, uyB, uzA, uzB;                                         // yz gauge: scaled U_y(i), U_z(i) of the four sites
   if (YZ) {
@@ -183,7 +179,6 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_march_tma(const __grid_constant
   // J_av (Eq. 35): x links of the NEW iterate that lie inside this tile row (step_ctl.cu, k_jav_edges
   // adds the links that cross a tile edge); only with x periodic and the mu / K part active
   const bool jact = (MODE != MODE_RHO) && dv.solve_mu && px;
-  const float2 Uraw = dv.Ux[jc];
   const bool lkA0 = actA, lkA1 = actA && 2 * lane + 2 < nv;
   const bool lkB0 = actB, lkB1 = actB && 64 + 2 * lane + 2 < nv && lane < 31;
   double jacc = 0.0;
@@ -200,6 +195,16 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_march_tma(const __grid_constant
     const long long ob = (long long)zwrap(k0 - 1) * plane + rowoff;
     rA[0] = actA ? __ldg(reinterpret_cast<const float4 *>(xin + ob)) : make_float4(0, 0, 0, 0);
     rB[0] = actB ? __ldg(reinterpret_cast<const float4 *>(xin + ob + 64)) : make_float4(0, 0, 0, 0);
+  }
+  const bool ztop = !pz && k1 == nz;                  // this chunk ends at the open top face
+  if (!pz && k0 == 0) {                               // open bottom face: psi_{-1} = U_z^2 psi_1 (plane 1 is what was loaded)
+    if (YZ) {
+      const float4 ua = *reinterpret_cast<const float4 *>(dv.Uzx + icA), ub = *reinterpret_cast<const float4 *>(dv.Uzx + icB);
+      rA[0] = sq_mul4(ua, rA[0], false); rB[0] = sq_mul4(ub, rB[0], false);
+    } else {
+      const float2 U2 = cmul(Uzj, Uzj);
+      rA[0] = cmul4(U2, rA[0]); rB[0] = cmul4(U2, rB[0]);
+    }
   }
   mbar_wait(sbase, 0u);
   rA[1] = lds128(stage0 + oA);
@@ -255,7 +260,6 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_march_tma(const __grid_constant
     if (eA_h) EA = lds64(prv + oEA);
     if (eB_h) EB = lds64(prv + oEB);
 
-    float4 TA = TvA, TB = TvB, BA = BvA, BB = BvB;
     if (YZ) {
       if (xedge) {                                     // quasi-periodic jump in x: psi_{-1} = P_{j,k} psi_{nx-1}
         const float2 P = cmul(dv.Pj[jc], dv.Pk[k]);
@@ -287,33 +291,29 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_march_tma(const __grid_constant
       }
     }
     if (xopen) {                                       // open x faces: W' = U^2 E, E' = U*^2 W
-      const float2 Ux = dv.Ux[jc];
-      const float2 U2 = cmul(Ux, Ux);
+      const float2 U2 = cmul(Uxj, Uxj);
       if (xloA) WA = cmul(U2, hi(CvA));
       if (xhiA) EA = cmulc(U2, lo(CvA));
       if (xhiB) EB = cmulc(U2, lo(CvB));
     }
-    if (!pz && (k == 0 || k == nz - 1)) {              // open z faces, uniform over the CTA
-      if (YZ) {
+    if (ztop && t == nk) {                             // open top face: psi_{nz} = U_z*^2 psi_{nz-2}; the stage
+      if (YZ) {                                        // holds plane nz - 2 (mirror), nobody reads Tv after this plane
         const float4 ua = *reinterpret_cast<const float4 *>(dv.Uzx + icA), ub = *reinterpret_cast<const float4 *>(dv.Uzx + icB);
-        if (k == 0) { BA = sq_mul4(ua, TA, false); BB = sq_mul4(ub, TB, false); }
-        else { TA = sq_mul4(ua, BA, true); TB = sq_mul4(ub, BB, true); }
+        TvA = sq_mul4(ua, TvA, true); TvB = sq_mul4(ub, TvB, true);
       } else {
-        const float2 Uz = dv.Uz[jc];
-        const float2 U2 = cmul(Uz, Uz);
-        if (k == 0) { BA = cmul4(U2, TA); BB = cmul4(U2, TB); }
-        else { TA = cmulc4(U2, BA); TB = cmulc4(U2, BB); }
+        const float2 U2 = cmul(Uzj, Uzj);
+        TvA = cmulc4(U2, TvA); TvB = cmulc4(U2, TvB);
       }
     }
 
     float2 sA0 = make_float2(0.f, 0.f), sA1 = sA0, sB0 = sA0, sB1 = sA0;
     if (MODE == MODE_SWEEP) { sA0 = lo(bA); sA1 = hi(bA); sB0 = lo(bB); sB1 = hi(bB); }
     if (YZ) {
-      nsum_pair_yz(L.ux, uyA, uzA, CvA, WA, EA, NA, SA, TA, BA, sA0, sA1);
-      nsum_pair_yz(L.ux, uyB, uzB, CvB, WB, EB, NB, SB_, TB, BB, sB0, sB1);
+      nsum_pair_yz(Lux, uyA, uzA, CvA, WA, EA, NA, SA, TvA, BvA, sA0, sA1);
+      nsum_pair_yz(Lux, uyB, uzB, CvB, WB, EB, NB, SB_, TvB, BvB, sB0, sB1);
     } else {
-      nsum_pair(L, CvA, WA, EA, NA, SA, TA, BA, sA0, sA1);
-      nsum_pair(L, CvB, WB, EB, NB, SB_, TB, BB, sB0, sB1);
+      nsum_pair(L, CvA, WA, EA, NA, SA, TvA, BvA, sA0, sA1);
+      nsum_pair(L, CvB, WB, EB, NB, SB_, TvB, BvB, sB0, sB1);
     }
 
     if (MODE == MODE_RHO) {
@@ -370,7 +370,7 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_march_tma(const __grid_constant
         const float rBx = __shfl_sync(0xffffffffu, outB.x, (lane + 1) & 31), rBy = __shfl_sync(0xffffffffu, outB.y, (lane + 1) & 31);
         const float2 nxA = (lane == 31) ? make_float2(rBx, rBy) : make_float2(nAx, nAy);
         auto link = [&](float ar, float ai, float br, float bi) {
-          return ar * (Uraw.x * bi + Uraw.y * br) - ai * (Uraw.x * br - Uraw.y * bi);
+          return ar * (Uxj.x * bi + Uxj.y * br) - ai * (Uxj.x * br - Uxj.y * bi);
         };
         float tsum = 0.f;
         if (lkA0) tsum += link(outA.x, outA.y, outA.z, outA.w);

@@ -690,6 +690,53 @@ def test_S13_initial_state_is_one_plus_complex_gaussian(seed):
     assert abs(np.mean(z.real * g1)) < 5.0 / math.sqrt(3 * n) * 1.2 and abs(np.mean(z.imag * g2)) < 5.0 / math.sqrt(3 * n) * 1.2
 
 
+def test_S11_langevin_pair_by_hand_from_the_known_answer_vector():
+    """Reading S11': one Philox call per site pair.  Seed 0, step 0, pair (0, 1): counter (0, 0, 0, 0), key (0, 0) is the
+    first published known-answer vector (tests/golden/philox4x32_10_kat.txt): 6627e8d5 e169c58d bc57ac4c 9b00dbd8.
+    Site 0 takes the first two words, site 1 the last two; r = ((x >> 9) + 1/2) 2^-22 - 1."""
+    p = O.Params(4, 2, 2, seed=0, temperature=1e-3)
+    z = O.langevin_noise(p, 0).ravel() / O.zeta_max(p)
+    r = [((w >> 9) + 0.5) / 4194304.0 - 1.0 for w in (0x6627e8d5, 0xe169c58d, 0xbc57ac4c, 0x9b00dbd8)]
+    assert abs(z[0] - complex(r[0], r[1])) < 1e-15 and abs(z[1] - complex(r[2], r[3])) < 1e-15   # (one product, one quotient)
+    # the next pair is another counter: sites 2, 3 come from the call with counter word 0 = 2
+    from oracle import philox
+    w = [int(v) for v in philox.philox4x32_10(2, 0, 0, 0, 0, 0)]
+    r = [((v >> 9) + 0.5) / 4194304.0 - 1.0 for v in w]
+    assert abs(z[2] - complex(r[0], r[1])) < 1e-15 and abs(z[3] - complex(r[2], r[3])) < 1e-15
+    # step and seed enter as counter word 2 and as the key
+    w = [int(v) for v in philox.philox4x32_10(6, 0, 9, 0, 77, 1)]
+    p2 = O.Params(4, 2, 2, seed=(1 << 32) + 77, temperature=1e-3)
+    z2 = O.langevin_noise(p2, 9).ravel() / O.zeta_max(p2)
+    assert abs(z2[7] - complex(((w[2] >> 9) + 0.5) / 4194304.0 - 1.0, ((w[3] >> 9) + 0.5) / 4194304.0 - 1.0)) < 1e-15
+
+
+def test_S11_langevin_field_is_white():
+    """Eq. (38)-(39): <zeta> = 0, <zeta_m zeta*_m'> = (2/3) zeta_max^2 delta_mm' delta_tt'; both components uniform in
+    (-zeta_max, zeta_max); nothing correlates -- not the two components of a site, not the two sites of a Philox pair,
+    not neighbouring pairs, rows, or steps."""
+    p = O.Params(64, 64, 64, seed=7, temperature=1e-3)
+    n = p.n_sites
+    z = O.langevin_noise(p, 3).ravel() / O.zeta_max(p)
+    a, b = z.real, z.imag
+    tol = 5.0 / 3.0 / math.sqrt(n)                                         # 5 sigma of a mean of products of U(-1,1) pairs
+    for c in (a, b):
+        assert abs(c.mean()) < 5.0 / math.sqrt(3 * n)
+        assert abs((c ** 2).mean() - 1.0 / 3.0) < 5.0 * math.sqrt(4.0 / 45.0 / n)
+        assert abs((c ** 4).mean() - 0.2) < 5.0 * math.sqrt((1.0 / 9.0 - 1.0 / 25.0) / n)
+        assert np.max(np.abs(c)) < 1.0
+        assert abs(np.mean(c[0::2] * c[1::2])) < tol * math.sqrt(2)     # the two sites of a pair
+        assert abs(np.mean(c[1:-1:2] * c[2::2])) < tol * math.sqrt(2)   # neighbouring pairs
+        assert abs(np.mean(c[:-64] * c[64:])) < tol                        # neighbouring rows
+        hist = np.histogram(c, bins=32, range=(-1, 1))[0]
+        assert np.max(np.abs(hist - n / 32)) < 5.0 * math.sqrt(n / 32)
+    assert abs(np.mean(a * b)) < tol
+    assert abs(np.mean(a[0::2] * b[1::2])) < tol * math.sqrt(2) and abs(np.mean(b[0::2] * a[1::2])) < tol * math.sqrt(2)
+    assert abs(np.mean(a[0::2] ** 2 * a[1::2] ** 2) - 1.0 / 9.0) < 5.0 * math.sqrt(2.0 / n) * 0.2   # independence, not just no correlation
+    z4 = O.langevin_noise(p, 4).ravel() / O.zeta_max(p)
+    assert abs(np.mean(z.real * z4.real)) < tol and abs(np.mean(z.imag * z4.imag)) < tol
+    assert abs(np.mean(np.abs(z) ** 2) - 2.0 / 3.0) < 5.0 * math.sqrt(2 * 4.0 / 45.0 / n)      # P:360
+
+
 def test_S13_box_muller_two_sites_by_hand():
     """Sites m = 0, 1 of seed 0, evaluated by hand from the Philox words (whose generator is pinned by the
     published known-answer vectors): u = ((x >> 9) + 1/2) 2^-23, g1 + i g2 = sqrt(-2 ln u1) e^{2 pi i u2}."""
