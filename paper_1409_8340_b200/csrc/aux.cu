@@ -221,11 +221,12 @@ __global__ void __launch_bounds__(128) k_shapes(const __grid_constant__ Dev dv, 
   }
 }
 
-// zeta_m of step `step` (Eq. 39; S11) exactly as the init kernel draws it.
+// zeta_m of step `step` (Eq. 39; S11') exactly as the init kernel draws it.
 __global__ void k_noise(const __grid_constant__ Dev dv, long long step, float2 *out) {
   for (long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x; m < dv.N; m += (long long)gridDim.x * blockDim.x) {
-    const PhiloxOut p = philox4x32_10((uint32_t)m, (uint32_t)((unsigned long long)m >> 32), (uint32_t)step, 0u, dv.seed_lo, dv.seed_hi);
-    out[m] = make_float2(dv.zeta_max * u32_to_pm1(p.x0), dv.zeta_max * u32_to_pm1(p.x1));
+    uint32_t wr, wi;
+    langevin_words((unsigned long long)m, (uint32_t)step, dv.seed_lo, dv.seed_hi, wr, wi);
+    out[m] = make_float2(dv.zeta_max * u32_to_pm1(wr), dv.zeta_max * u32_to_pm1(wi));
   }
 }
 

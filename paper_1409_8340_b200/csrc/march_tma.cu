@@ -336,11 +336,10 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_march_tma(const __grid_constant
           float2 z0 = make_float2(0.f, 0.f), z1 = z0;
           if (dv.zeta_max > 0.f) {                     // Langevin term, Eq. (39), S11
             const unsigned long long m = (unsigned long long)ix;
-            const PhiloxOut p0 = philox4x32_10((uint32_t)m, (uint32_t)(m >> 32), nstep, 0u, dv.seed_lo, dv.seed_hi);
-            const PhiloxOut p1 = philox4x32_10((uint32_t)(m + 1), (uint32_t)((m + 1) >> 32), nstep, 0u, dv.seed_lo, dv.seed_hi);
-            const float zs = 2.f * ht2 * dv.zeta_max;
+            const PhiloxOut p0 = philox4x32_10((uint32_t)m, (uint32_t)(m >> 32), nstep, 0u, dv.seed_lo, dv.seed_hi);   // m is even:
+            const float zs = 2.f * ht2 * dv.zeta_max;                                     // one call per site pair (S11')
             z0 = make_float2(zs * u32_to_pm1(p0.x0), zs * u32_to_pm1(p0.x1));
-            z1 = make_float2(zs * u32_to_pm1(p1.x0), zs * u32_to_pm1(p1.x1));
+            z1 = make_float2(zs * u32_to_pm1(p0.x2), zs * u32_to_pm1(p0.x3));
           }
           const float2 q0 = cmul(lo(C), make_float2(2.f - d0.x, -d0.y)), q1 = cmul(hi(C), make_float2(2.f - d1.x, -d1.y));
           const float2 b0 = make_float2(q0.x + s0.x + z0.x, q0.y + s0.y + z0.y);

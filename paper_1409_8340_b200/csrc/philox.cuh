@@ -1,7 +1,8 @@
 // Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11, Sec. 3.3), counter-based, in registers.
-// The paper names no generator; BASELINE.json fixes Philox; reading S11 fixes the
-// counter/key assignment: key = (seed_lo, seed_hi), counter = (m_lo, m_hi, step, stream) with the
-// global site index m, stream 0 = Langevin noise, stream 1 = initial condition.
+// The paper names no generator; BASELINE.json fixes Philox; readings S11' / S13 fix the
+// counter/key assignment: key = (seed_lo, seed_hi), counter = (m_lo, m_hi, step, stream) with a
+// global site index m; stream 0 = Langevin noise (ONE call per site pair: m = the even site, words
+// (x0, x1) -> even site, (x2, x3) -> odd site), stream 1 = initial condition (one call per site).
 #pragma once
 #include <stdint.h>
 
@@ -30,4 +31,14 @@ __device__ __forceinline__ float u32_to_pm1(uint32_t x) {
 // uint32 -> uniform in (0, 1): ((x >> 9) + 0.5) 2^-23 (S13), as a double.
 __device__ __forceinline__ double u32_to_01(uint32_t x) {
   return ((double)(x >> 9) + 0.5) * (1.0 / 8388608.0);
+}
+
+// Langevin words of ONE site (reading S11'): the call of its pair, the words picked by the parity of m.  For kernels
+// that own one site per thread; the marching kernels own whole pairs and use all four words of a call.
+__device__ __forceinline__ void langevin_words(unsigned long long m, uint32_t step, uint32_t k0, uint32_t k1,
+                                               uint32_t &re, uint32_t &im) {
+  const unsigned long long me = m & ~1ull;
+  const PhiloxOut p = philox4x32_10((uint32_t)me, (uint32_t)(me >> 32), step, 0u, k0, k1);
+  re = (m & 1ull) ? p.x2 : p.x0;
+  im = (m & 1ull) ? p.x3 : p.x1;
 }

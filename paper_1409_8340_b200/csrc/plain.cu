@@ -190,8 +190,9 @@ __global__ void __launch_bounds__(128) k_march64(const __grid_constant__ Dev dv)
         cd z = mk(0.0, 0.0);
         if (dv.zeta_max64 > 0.0) {                                          // Langevin term, Eq. (39), S11
           const unsigned long long mm = (unsigned long long)m;
-          const PhiloxOut p = philox4x32_10((uint32_t)mm, (uint32_t)(mm >> 32), (unsigned)ctl->n, 0u, dv.seed_lo, dv.seed_hi);
-          z = mk(dv.zeta_max64 * (double)u32_to_pm1(p.x0), dv.zeta_max64 * (double)u32_to_pm1(p.x1));
+          uint32_t wr, wi;
+          langevin_words(mm, (unsigned)ctl->n, dv.seed_lo, dv.seed_hi, wr, wi);
+          z = mk(dv.zeta_max64 * (double)u32_to_pm1(wr), dv.zeta_max64 * (double)u32_to_pm1(wi));
         }
         const cd q = cm(c, mk(2.0 - d.x, -d.y));
         b = mk(q.x + ht2 * (ns.x + 2.0 * z.x), q.y + ht2 * (ns.y + 2.0 * z.y));
@@ -270,8 +271,9 @@ __global__ void k_init_state64(const __grid_constant__ Dev dv, double amp) {
 }
 __global__ void k_noise64(const __grid_constant__ Dev dv, long long step, double2 *out) {
   for (long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x; m < dv.N; m += (long long)gridDim.x * blockDim.x) {
-    const PhiloxOut p = philox4x32_10((uint32_t)m, (uint32_t)((unsigned long long)m >> 32), (uint32_t)step, 0u, dv.seed_lo, dv.seed_hi);
-    out[m] = make_double2(dv.zeta_max64 * (double)u32_to_pm1(p.x0), dv.zeta_max64 * (double)u32_to_pm1(p.x1));
+    uint32_t wr, wi;
+    langevin_words((unsigned long long)m, (uint32_t)step, dv.seed_lo, dv.seed_hi, wr, wi);
+    out[m] = make_double2(dv.zeta_max64 * (double)u32_to_pm1(wr), dv.zeta_max64 * (double)u32_to_pm1(wi));
   }
 }
 __global__ void k_copy_psi64(const __grid_constant__ Dev dv, double2 *__restrict__ out) {
