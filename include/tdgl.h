@@ -212,10 +212,21 @@ int tdgl_debug_poisson(tdgl_t *h, const void *rho_dev, void *mu_dev);
 int tdgl_debug_rho(tdgl_t *h, void *rho_dev);
 /* Number of kernels the library has launched on this handle since create (bench: gpu_launches). */
 int64_t tdgl_launch_count(const tdgl_t *h);
-/* CUDA-event timing of the Jacobi sweep kernel: when enabled, every launch of the plain sweep kernel
- * in HOST_LOOP mode is bracketed by events on the stream; read back the accumulated milliseconds and
- * launch count.  Used by bench.py for the roofline figure. */
+/* CUDA-event timing of the sweep kernels in HOST_LOOP mode: enable = 1 brackets every launch of the plain sweep kernel
+ * by events on the stream, enable = 2 every launch of the fused two-sweep kernel (see tdgl_set_pair_mode); one kernel
+ * at a time while timing is on.  The call returns the milliseconds and launches accumulated so far and, with enable > 0,
+ * clears them.  Used by bench.py for the roofline figures. */
 int tdgl_sweep_timing(tdgl_t *h, int32_t enable, double *ms_total_host, int64_t *launches_host);
+
+/* Fused sweep pairs (temporal blocking of Eq. 33; march_pair.cu).  On meshes that admit it (xz gauge, fp32, nx % 128 == 0,
+ * ny % 16 == 0, ny >= 32, nz >= 4) two Jacobi sweeps run as ONE pass over HBM whenever two more sweeps are certain
+ * (prescribed counts) or predicted from the residual history.  Criterion (34) stays exact: both residuals are reduced,
+ * and a pair whose first sweep already met the criterion is discarded and redone as a plain sweep, so psi, the sweep
+ * counts, the residual log and J_av are bit-identical to plain sweeps.  mode: 0 never, 1 automatic (default), 2 whenever
+ * the cap max_sweeps allows (tests: forces the redo path).  tdgl_get_pair_stats: whether the mesh is eligible, pairs
+ * launched, pairs discarded since create. */
+int tdgl_set_pair_mode(tdgl_t *h, int32_t mode);
+int tdgl_get_pair_stats(tdgl_t *h, int32_t *eligible_host, int64_t *pairs_host, int64_t *redone_host);
 
 #ifdef __cplusplus
 }

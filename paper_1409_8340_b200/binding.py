@@ -20,7 +20,7 @@ EXPORTS = (
     "tdgl_get_psi_mu", "tdgl_observables", "tdgl_strerror", "tdgl_last_cuda_error", "tdgl_set_state", "tdgl_set_solver",
     "tdgl_set_sweep_schedule", "tdgl_get_sweep_log", "tdgl_get_eps", "tdgl_debug_noise", "tdgl_debug_poisson",
     "tdgl_debug_rho", "tdgl_launch_count", "tdgl_sweep_timing", "tdgl_mu_gain", "tdgl_mu_refine_enabled",
-    "tdgl_set_mu_solver", "tdgl_get_mu_log", "tdgl_set_insulators", "tdgl_set_pinning_shapes", "tdgl_set_insulator_shapes",
+    "tdgl_set_mu_solver", "tdgl_get_mu_log", "tdgl_set_insulators", "tdgl_set_pinning_shapes", "tdgl_set_insulator_shapes", "tdgl_set_pair_mode", "tdgl_get_pair_stats",
 )
 
 
@@ -97,6 +97,8 @@ def lib() -> C.CDLL:
     L.tdgl_set_insulators.argtypes = [vp, C.POINTER(TdglSphere), i64]
     L.tdgl_set_pinning_shapes.argtypes = [vp, vp, i64, f32, f32]
     L.tdgl_set_insulator_shapes.argtypes = [vp, vp, i64]
+    L.tdgl_set_pair_mode.argtypes = [vp, i32]
+    L.tdgl_get_pair_stats.argtypes = [vp, C.POINTER(i32), C.POINTER(i64), C.POINTER(i64)]
     L.tdgl_get_mu_log.argtypes = [vp, i32, C.POINTER(i32), C.POINTER(i32), i32, C.POINTER(i32)]
     _lib = L
     return L
@@ -337,7 +339,18 @@ class Solver:
     def launch_count(self) -> int:
         return int(lib().tdgl_launch_count(self.h))
 
-    def sweep_timing(self, enable: bool):
+    def set_pair_mode(self, mode: int):
+        """Fused sweep pairs: 0 never, 1 automatic (default), 2 whenever the cap allows (forces the redo path)."""
+        _check(lib().tdgl_set_pair_mode(self.h, int(mode)), "tdgl_set_pair_mode", self.h)
+
+    def pair_stats(self):
+        """(mesh eligible, pairs launched, pairs discarded and redone as plain sweeps)."""
+        e, a, b = C.c_int32(), C.c_int64(), C.c_int64()
+        _check(lib().tdgl_get_pair_stats(self.h, C.byref(e), C.byref(a), C.byref(b)), "tdgl_get_pair_stats", self.h)
+        return bool(e.value), a.value, b.value
+
+    def sweep_timing(self, enable):
+        """enable: 0 / False off, 1 / True plain sweeps, 2 fused pairs."""
         ms, n = C.c_double(), C.c_int64()
         _check(lib().tdgl_sweep_timing(self.h, int(enable), C.byref(ms), C.byref(n)), "tdgl_sweep_timing", self.h)
         return ms.value, n.value

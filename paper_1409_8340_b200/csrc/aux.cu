@@ -21,7 +21,8 @@ __global__ void k_ctl_reset(const __grid_constant__ Dev dv, float eps_tol, int m
   Ctl *c = dv.ctl;
   c->K = 0.0; c->Ex = 0.0; c->Jav = 0.0; c->Ex_sum = 0.0; c->Ex_cnt = 0; c->n = 0; c->sweeps_total = 0;
   c->sweeps = 0; c->done = 0; c->xbuf = 0; c->status = 0; c->sweeps_last = 0; c->resid_last = 0.f;
-  c->ticket = 0u; c->ticket2 = 0u;
+  c->ticket = 0u; c->ticket2 = 0u; c->use_pair = 0; c->pair_mode = 1; c->r_hist = 0.f;
+  c->pair_launches = 0; c->pair_redone = 0; c->body_launches = 0;
   c->eps_tol = eps_tol; c->max_sweeps = max_sweeps; c->fixed_sweeps = fixed_sweeps;
   c->sched_n = 0; c->sched_pos = 0; c->Jext = 0.0; c->Bx = 0.0; c->Bz = 0.0;
   c->h_tau = 0.1f; c->eps_mu = 1e-6f; c->eps_mu_in = 1e-6f; c->mu_max_outer = 1000; c->mu_max_inner = 100;   // S20
@@ -33,6 +34,7 @@ __global__ void k_ctl_solver(const __grid_constant__ Dev dv, float eps_tol, int 
   dv.ctl->eps_tol = eps_tol; dv.ctl->max_sweeps = max_sweeps; dv.ctl->fixed_sweeps = fixed_sweeps;
 }
 __global__ void k_ctl_sched(const __grid_constant__ Dev dv, int n) { dv.ctl->sched_n = n; dv.ctl->sched_pos = 0; }
+__global__ void k_ctl_pair_mode(const __grid_constant__ Dev dv, int mode) { dv.ctl->pair_mode = mode; }
 __global__ void k_ctl_state(const __grid_constant__ Dev dv, double K) { dv.ctl->K = K; dv.ctl->xbuf = 0; }
 
 // a1: the K-independent phase tables of the xz Landau gauge (Eq. 24a, 27):
@@ -354,6 +356,7 @@ void launch_init_state(const Dev &dv, float amp, cudaStream_t st) { k_init_state
 void launch_ctl_reset(const Dev &dv, float tol, int maxs, int fixed, cudaStream_t st) { k_ctl_reset<<<1, 1, 0, st>>>(dv, tol, maxs, fixed); }
 void launch_ctl_solver(const Dev &dv, float tol, int maxs, int fixed, cudaStream_t st) { k_ctl_solver<<<1, 1, 0, st>>>(dv, tol, maxs, fixed); }
 void launch_ctl_sched(const Dev &dv, int n, cudaStream_t st) { k_ctl_sched<<<1, 1, 0, st>>>(dv, n); }
+void launch_ctl_pair_mode(const Dev &dv, int mode, cudaStream_t st) { k_ctl_pair_mode<<<1, 1, 0, st>>>(dv, mode); }
 void launch_ctl_state(const Dev &dv, double K, cudaStream_t st) { k_ctl_state<<<1, 1, 0, st>>>(dv, K); }
 void launch_set_field(const Dev &dv, double Bx, double Bz, double J, cudaStream_t st) { k_set_field<<<1, 256, 0, st>>>(dv, Bx, Bz, J); }
 void launch_fill(float *p, long long n, float v, cudaStream_t st) { k_fill_f32<<<grid_for(n, 256, 148 * 16), 256, 0, st>>>(p, n, v); }

@@ -112,18 +112,44 @@ __device__ __forceinline__ void nsum_pair(const Links &L, const float4 &C, const
 // x^{l+1} = n / d for both sites of a pair (Eq. 33) and |r^l|^2 = |d|^2 |x^{l+1} - x^l|^2 (S8)
 __device__ __forceinline__ float4 divide_pair(const float2 &n0, const float2 &n1, const float4 &d, const float4 &C,
                                               float &rmax) {
-  const float m0 = d.x * d.x + d.y * d.y, m1 = d.z * d.z + d.w * d.w;
+  const float m0 = __fmaf_rn(d.x, d.x, __fmul_rn(d.y, d.y)), m1 = __fmaf_rn(d.z, d.z, __fmul_rn(d.w, d.w));
   const float i0 = rcp_approx(m0), i1 = rcp_approx(m1);
   const float2 y0 = cmulc(lo(d), n0), y1 = cmulc(hi(d), n1);
   const u64 o0 = mul2(pk2(y0), pk2(i0, i0)), o1 = mul2(pk2(y1), pk2(i1, i1));
   const float2 e0 = upk2(sub2(o0, pk2(lo(C)))), e1 = upk2(sub2(o1, pk2(hi(C))));
-  rmax = fmaxf(rmax, fmaxf((e0.x * e0.x + e0.y * e0.y) * m0, (e1.x * e1.x + e1.y * e1.y) * m1));
+  const float q0 = __fmul_rn(__fmaf_rn(e0.x, e0.x, __fmul_rn(e0.y, e0.y)), m0);
+  const float q1 = __fmul_rn(__fmaf_rn(e1.x, e1.x, __fmul_rn(e1.y, e1.y)), m1);
+  rmax = fmaxf(rmax, fmaxf(q0, q1));
   const float2 a = upk2(o0), b = upk2(o1);
   return make_float4(a.x, a.y, b.x, b.y);
 }
 
+// Im[a* U b] of one x link (Eq. 35), contraction spelled out (the plain sweep and the fused pair must agree)
+__device__ __forceinline__ float jlink(float2 U, float ar, float ai, float br, float bi) {
+  const float p = __fmaf_rn(U.x, bi, __fmul_rn(U.y, br)), q = __fmaf_rn(U.x, br, -__fmul_rn(U.y, bi));
+  return __fmaf_rn(ar, p, -__fmul_rn(ai, q));
+}
+
 // The decision taken by the last CTA of a sweep (Eq. 34; S8: residual of the input iterate,
 // keep the new one; S9/S10: prescribed counts, cap).
+// Which kernel of the loop body acts next: the fused pair (march_pair.cu) only when two more sweeps are certain
+// (prescribed counts) or predicted from the residual history (criterion (34) stays exact either way: a pair whose
+// FIRST sweep already met it is discarded and redone as a plain sweep, see pair_decide).
+__device__ __forceinline__ void choose_next(const Dev &dv, Ctl *c, int sweeps, int target, float r_last, float r_prev) {
+  int up = 0;
+  if (dv.pair_ok && c->pair_mode > 0) {
+    if (target > 0) up = target - sweeps >= 2;
+    else if (sweeps + 2 <= c->max_sweeps) {
+      if (c->pair_mode == 2) up = 1;
+      else if (r_prev > 0.f) {                           // geometric decay: next residual ~ r_last * (r_last / r_prev)
+        const float q = fminf(1.f, r_last / r_prev);
+        up = r_last * q >= 3.f * c->eps_tol;
+      } else up = c->sweeps_last >= sweeps + 2;           // first decision of a step: the previous step's count
+    }
+  }
+  c->use_pair = up;
+}
+
 __device__ __noinline__ void sweep_decide(const Dev &dv, int l) {
   Ctl *c = dv.ctl;
   const float r2 = __uint_as_float(atomicMax(&c->resid_bits[l], 0u));
@@ -139,10 +165,50 @@ __device__ __noinline__ void sweep_decide(const Dev &dv, int l) {
     done = (r2 < c->eps_tol) || sweeps >= c->max_sweeps;
     if (!(r2 < c->eps_tol) && sweeps >= c->max_sweeps) c->status = 1;
   }
+  choose_next(dv, c, sweeps, target, r2, l > 0 ? c->r_hist : 0.f);
+  c->r_hist = r2;
   if (done) {
     c->done = 1;
+    c->use_pair = 0;
     c->sweeps_last = sweeps;
     c->resid_last = r2;
+  }
+  if (dv.use_cond) cudaGraphSetConditional((cudaGraphConditionalHandle)dv.cond_handle, done ? 0u : 1u);
+  __threadfence();
+}
+
+// The decision after a fused pair of sweeps l+1, l+2 (residuals r^l, r^{l+1} of their input iterates, S8).  If r^l
+// already meets criterion (34) the answer is x^{l+1}, which the pair did not keep: nothing is committed (x^l is
+// intact in its buffer) and the next kernel is the plain sweep, which recomputes x^{l+1} and stops.
+__device__ __noinline__ void pair_decide(const Dev &dv, int l) {
+  Ctl *c = dv.ctl;
+  const float r1 = __uint_as_float(atomicMax(&c->resid_bits[l], 0u));
+  const float r2 = __uint_as_float(atomicMax(&c->resid_bits[l + 1], 0u));
+  int target = c->fixed_sweeps;
+  if (c->sched_pos < c->sched_n) target = dv.sched[c->sched_pos];
+  c->pair_launches += 1;
+  bool done = false;
+  if (target <= 0 && r1 < c->eps_tol) {
+    c->use_pair = 0;
+    c->pair_redone += 1;
+  } else {
+    const int sweeps = l + 2;
+    c->sweeps = sweeps;
+    c->xbuf ^= 1;
+    if (target > 0) {
+      done = sweeps >= target;
+    } else {
+      done = (r2 < c->eps_tol) || sweeps >= c->max_sweeps;
+      if (!(r2 < c->eps_tol) && sweeps >= c->max_sweeps) c->status = 1;
+    }
+    choose_next(dv, c, sweeps, target, r2, r1);
+    c->r_hist = r2;
+    if (done) {
+      c->done = 1;
+      c->use_pair = 0;
+      c->sweeps_last = sweeps;
+      c->resid_last = r2;
+    }
   }
   if (dv.use_cond) cudaGraphSetConditional((cudaGraphConditionalHandle)dv.cond_handle, done ? 0u : 1u);
   __threadfence();

@@ -74,8 +74,10 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_march_tma(const __grid_constant
   extern __shared__ __align__(128) unsigned char smem_raw[];
   Ctl *ctl = dv.ctl;
   int l = 0;
+  if (MODE == MODE_SWEEP && (blockIdx.x | blockIdx.y | blockIdx.z | threadIdx.x) == 0) ctl->body_launches += 1;
   if (MODE != MODE_RHO) {
     if (ctl->done) return;
+    if (MODE == MODE_SWEEP && ctl->use_pair) return;   // this iteration belongs to the fused pair kernel (march_pair.cu)
     l = ctl->sweeps;
   }
   const int xb = ctl->xbuf;
@@ -368,9 +370,7 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_march_tma(const __grid_constant
         const float nAx = __shfl_down_sync(0xffffffffu, outA.x, 1), nAy = __shfl_down_sync(0xffffffffu, outA.y, 1);
         const float rBx = __shfl_sync(0xffffffffu, outB.x, (lane + 1) & 31), rBy = __shfl_sync(0xffffffffu, outB.y, (lane + 1) & 31);
         const float2 nxA = (lane == 31) ? make_float2(rBx, rBy) : make_float2(nAx, nAy);
-        auto link = [&](float ar, float ai, float br, float bi) {
-          return ar * (Uxj.x * bi + Uxj.y * br) - ai * (Uxj.x * br - Uxj.y * bi);
-        };
+        auto link = [&](float ar, float ai, float br, float bi) { return jlink(Uxj, ar, ai, br, bi); };
         float tsum = 0.f;
         if (lkA0) tsum += link(outA.x, outA.y, outA.z, outA.w);
         if (lkA1) tsum += link(outA.z, outA.w, nxA.x, nxA.y);

@@ -58,6 +58,7 @@ __global__ void k_step_begin(const __grid_constant__ Dev dv) {
   if (tid == 0) {
     c->sweeps = 0;
     c->done = 0;
+    c->use_pair = 0;
     c->ticket = 0u;
   }
   write_Ux(dv, c->K, tid, blockDim.x);

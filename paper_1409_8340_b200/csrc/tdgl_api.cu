@@ -4,7 +4,10 @@
 #include "tdgl_dev.cuh"
 #include "march_tma.h"
 #include "march_film.h"
+#include "march_pair.h"
 #include <cmath>
+#include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -28,6 +31,7 @@ void launch_init_state(const Dev &dv, float amp, cudaStream_t st);
 void launch_ctl_reset(const Dev &dv, float tol, int maxs, int fixed, cudaStream_t st);
 void launch_ctl_solver(const Dev &dv, float tol, int maxs, int fixed, cudaStream_t st);
 void launch_ctl_sched(const Dev &dv, int n, cudaStream_t st);
+void launch_ctl_pair_mode(const Dev &dv, int mode, cudaStream_t st);
 void launch_ctl_state(const Dev &dv, double K, cudaStream_t st);
 void launch_set_field(const Dev &dv, double Bx, double Bz, double J, cudaStream_t st);
 void launch_fill(float *p, long long n, float v, cudaStream_t st);
@@ -68,6 +72,7 @@ struct tdgl {
   cudaStream_t stream;
   dim3 mgrid;                  // grid of the marching kernels: 128 x 8 tiles x z chunks
   MarchMaps maps;              // TMA tensor maps of psi[0], psi[1], b, d
+  PairMaps pmaps;              // ... of the fused two-sweep kernel (march_pair.cu), when dv.pair_ok
   bool film;                   // nz = 1: the paper's 2D mode (S22), kernels of march_film.cu
   Dev dvp;                     // the Poisson solver's view of the grid (film: y takes the role of z)
   int jav_blocks;
@@ -83,10 +88,10 @@ struct tdgl {
   cudaStream_t cap_stream;
   // host loop
   int *h_flag;                 // pinned: [0] done, [1] sweeps
-  int pred_sweeps;
+  int pred_units;              // predicted iterations of the sweep loop (host loop: enqueued before the first flag read)
   int pred_mu_inner;           // pseudo-time mu iteration: predicted Jacobi sweeps per outer iteration
   // sweep timing
-  bool timing;
+  int timing;                  // 0 off, 1 plain sweeps, 2 fused pairs
   double t_ms;
   int64_t t_launches;
   cudaEvent_t ev0, ev1;
@@ -268,6 +273,7 @@ static size_t carve(const tdgl_params *p, char *base, Dev *dv) {
 }
 
 static int cuda_fail(tdgl_t *h, cudaError_t e) {
+  if (getenv("TDGL_DEBUG")) fprintf(stderr, "libtdgl: CUDA error %d: %s\n", (int)e, cudaGetErrorString(e));
   if (h) h->last_cuda = (int)e;
   return TDGL_ECUDA;
 }
@@ -283,6 +289,15 @@ static void march(tdgl_t *h, int mode, const Dev &dv, cudaStream_t st) {
   if (dv.fp64) launch_march64(mode, dv, st);
   else if (h->film) launch_march_film(mode, dv, h->mgrid, st);
   else launch_march_tma(mode, dv, h->maps, h->mgrid, st);
+}
+
+// one iteration of the sweep loop: the fused pair kernel (acts only when the device-side choice says so) and the plain
+// sweep (acts otherwise); a kernel whose turn it is not returns at once
+static int sweep_unit(tdgl_t *h, const Dev &dv, cudaStream_t st) {
+  int n = 0;
+  if (dv.pair_ok) { launch_march_pair(dv, h->pmaps, st); ++n; }
+  march(h, MODE_SWEEP, dv, st); ++n;
+  return n;
 }
 
 // One solve of the paper's pseudo-time mu iteration (Eq. 40; plain.cu), host-driven: per outer iteration the right side c,
@@ -385,7 +400,7 @@ static int build_graph(tdgl_t *h) {
   CK(cudaGraphAddNode(&cond, h->graph, tail.data(), tail.size(), &np));
   cudaGraph_t body = np.conditional.phGraph_out[0];
   CK(cudaStreamBeginCaptureToGraph(cs, body, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal));
-  march(h, MODE_SWEEP, h->dv, cs);
+  sweep_unit(h, h->dv, cs);
   CKCAP(cudaSuccess);
   CK(cudaStreamEndCapture(cs, &g2));
   // segment B: everything after the psi solve
@@ -398,8 +413,12 @@ static int build_graph(tdgl_t *h) {
 }
 
 // inside tdgl_create a failing CUDA call releases the half-built handle (pinned flag word, events, graph objects)
-#define CKC(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { tdgl_destroy(h); return TDGL_ECUDA; } } while (0)
-#define CKCL() do { cudaError_t e_ = cudaGetLastError(); if (e_ != cudaSuccess) { tdgl_destroy(h); return TDGL_ECUDA; } } while (0)
+// (TDGL_DEBUG in the environment: say which call failed; tdgl_create has no handle to leave the code in)
+static void create_fail(cudaError_t e, int line) {
+  if (getenv("TDGL_DEBUG")) fprintf(stderr, "tdgl_create: %s (tdgl_api.cu:%d)\n", cudaGetErrorString(e), line);
+}
+#define CKC(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { create_fail(e_, __LINE__); tdgl_destroy(h); return TDGL_ECUDA; } } while (0)
+#define CKCL() do { cudaError_t e_ = cudaGetLastError(); if (e_ != cudaSuccess) { create_fail(e_, __LINE__); tdgl_destroy(h); return TDGL_ECUDA; } } while (0)
 extern "C" int tdgl_destroy(tdgl_t *h);
 
 extern "C" int tdgl_create(const tdgl_params *p, tdgl_t **out) {
@@ -457,7 +476,7 @@ extern "C" int tdgl_create(const tdgl_params *p, tdgl_t **out) {
     h->mgrid = dim3(gx, gy, gz);
   }
   h->jav_blocks = jav_edge_blocks(dv, march_tma_tile_w());
-  h->pred_sweeps = 1;
+  h->pred_units = 0;
   h->pred_mu_inner = 1;
   if (dv.fp64) {
     // plain kernels: nothing to configure
@@ -466,6 +485,11 @@ extern "C" int tdgl_create(const tdgl_params *p, tdgl_t **out) {
   } else {
     CKC(march_tma_configure());
     if (march_tma_build_maps(dv, &h->maps) != 0) { tdgl_destroy(h); return TDGL_ECUDA; }
+    if (march_pair_ok(p->nx, p->ny, p->nz, dv.gauge_yz != 0)) {
+      CKC(march_pair_configure());
+      { const int rc_ = march_pair_build_maps(dv, &h->pmaps); if (rc_ != 0) { create_fail(cudaErrorUnknown, -rc_); tdgl_destroy(h); return TDGL_ECUDA; } }
+      dv.pair_ok = 1;
+    }
   }
   if (film) CKC(poisson_configure(p->nx, 1, p->ny));
   else CKC(poisson_configure(p->nx, p->ny, p->nz));
@@ -648,31 +672,40 @@ static int step_host_loop(tdgl_t *h) {
   launch_step_begin(dv, st);
   march(h, MODE_INIT, dv, st);
   h->launches += 2;
-  int launched = 1;
+  int launched = 0;                             // loop iterations (sweep units) enqueued
   const int cap = TDGL_MAX_RESID_SLOTS;
   for (;;) {
-    // speculative sweeps (they return at once when the solve is already done), then one flag read
-    int burst = h->timing ? 0 : h->pred_sweeps - launched;
+    // speculative iterations (their kernels return at once when the solve is already done), then one flag read
+    int burst = h->timing ? 0 : h->pred_units - launched;
     for (int s = 0; s < burst && launched < cap; ++s) {
-      march(h, MODE_SWEEP, dv, st);
-      ++launched; ++h->launches;
+      h->launches += sweep_unit(h, dv, st);
+      ++launched;
     }
-    CK(cudaMemcpyAsync(h->h_flag, &dv.ctl->sweeps, 2 * sizeof(int), cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(h->h_flag, &dv.ctl->sweeps, 3 * sizeof(int), cudaMemcpyDeviceToHost, st));   // sweeps, done, use_pair
     CK(cudaStreamSynchronize(st));
     if (h->h_flag[1] || launched >= cap) break;
-    if (h->timing) CK(cudaEventRecord(h->ev0, st));
-    march(h, MODE_SWEEP, dv, st);
-    ++launched; ++h->launches;
-    if (h->timing) {
-      CK(cudaEventRecord(h->ev1, st));
-      CK(cudaEventSynchronize(h->ev1));
-      float ms = 0.f;
-      CK(cudaEventElapsedTime(&ms, h->ev0, h->ev1));
-      h->t_ms += ms;
-      h->t_launches += 1;
+    if (!h->timing) {
+      h->launches += sweep_unit(h, dv, st);
+    } else {
+      // timing mode: exactly the kernel whose turn it is, bracketed by events (kind 1: plain sweeps, kind 2: pairs)
+      const bool pair = dv.pair_ok && h->h_flag[2];
+      const bool timed = pair ? h->timing == 2 : h->timing == 1;
+      if (timed) CK(cudaEventRecord(h->ev0, st));
+      if (pair) launch_march_pair(dv, h->pmaps, st);
+      else march(h, MODE_SWEEP, dv, st);
+      ++h->launches;
+      if (timed) {
+        CK(cudaEventRecord(h->ev1, st));
+        CK(cudaEventSynchronize(h->ev1));
+        float ms = 0.f;
+        CK(cudaEventElapsedTime(&ms, h->ev0, h->ev1));
+        h->t_ms += ms;
+        h->t_launches += 1;
+      }
     }
+    ++launched;
   }
-  h->pred_sweeps = h->h_flag[0] < 1 ? 1 : h->h_flag[0];
+  h->pred_units = launched < 1 ? 1 : launched;
   {
     const int m = enqueue_after_solve(h, st);
     if (m < 0) return cuda_fail(h, cudaGetLastError());
@@ -902,22 +935,40 @@ extern "C" int64_t tdgl_launch_count(const tdgl_t *h) {
   if (!h) return 0;
   int64_t n = h->launches;
   if (h->use_graph && h->graph_steps > 0) {
-    long long tot = 0, steps = 0;
-    if (cudaMemcpyAsync(&tot, &h->dv.ctl->sweeps_total, sizeof(long long), cudaMemcpyDeviceToHost, h->stream) != cudaSuccess ||
-        cudaMemcpyAsync(&steps, &h->dv.ctl->n, sizeof(long long), cudaMemcpyDeviceToHost, h->stream) != cudaSuccess ||
+    long long body = 0;
+    if (cudaMemcpyAsync(&body, &h->dv.ctl->body_launches, sizeof(long long), cudaMemcpyDeviceToHost, h->stream) != cudaSuccess ||
         cudaStreamSynchronize(h->stream) != cudaSuccess)
       return -1;
-    // per graph step: fixed_per_step kernels (begin, init+sweep 1, ...) + the further sweeps
-    n += h->graph_steps * (int64_t)h->fixed_per_step + (tot - steps);
+    // per graph step: fixed_per_step kernels (begin, init+sweep 1, ...) + the kernels of the sweep loop (counted on the device)
+    n += h->graph_steps * (int64_t)h->fixed_per_step + body;
   }
   return n;
+}
+
+extern "C" int tdgl_set_pair_mode(tdgl_t *h, int32_t mode) {
+  if (!h || mode < 0 || mode > 2) return TDGL_EINVAL;
+  launch_ctl_pair_mode(h->dv, mode, h->stream);
+  h->launches += 1;
+  CKL();
+  return TDGL_OK;
+}
+
+extern "C" int tdgl_get_pair_stats(tdgl_t *h, int32_t *eligible, int64_t *pairs, int64_t *redone) {
+  if (!h) return TDGL_EINVAL;
+  long long v[2] = {0, 0};
+  CK(cudaMemcpyAsync(v, &h->dv.ctl->pair_launches, 2 * sizeof(long long), cudaMemcpyDeviceToHost, h->stream));
+  CK(cudaStreamSynchronize(h->stream));
+  if (eligible) *eligible = h->dv.pair_ok;
+  if (pairs) *pairs = v[0];
+  if (redone) *redone = v[1];
+  return TDGL_OK;
 }
 
 extern "C" int tdgl_sweep_timing(tdgl_t *h, int32_t enable, double *ms_total, int64_t *launches) {
   if (!h) return TDGL_EINVAL;
   if (ms_total) *ms_total = h->t_ms;
   if (launches) *launches = h->t_launches;
-  h->timing = enable != 0;
+  h->timing = enable < 0 ? 0 : (enable > 2 ? 1 : enable);
   if (enable) { h->t_ms = 0.0; h->t_launches = 0; }
   return TDGL_OK;
 }

@@ -19,12 +19,18 @@ struct Ctl {
   long long sweeps_total;
   int sweeps;               // sweeps done in the current step
   int done;                 // psi solve of the current step finished
+  int use_pair;             // the next loop-body kernel to act is the fused two-sweep kernel (march_pair.cu), else the plain sweep
   int xbuf;                 // which psi buffer holds the latest iterate
   int status;               // latched TDGL_WMAXSWEEPS
   int sweeps_last;
   float resid_last;
   unsigned int ticket;      // last-block election of the sweep kernel
   unsigned int ticket2;     // ... of the reduction kernels
+  // fused sweep pairs (march_pair.cu): 0 never, 1 when the residual history predicts that both sweeps are needed,
+  // 2 whenever the cap allows (tests: exercises the redo path); residual of the previous sweep; statistics
+  int pair_mode;
+  float r_hist;
+  long long pair_launches, pair_redone, body_launches;
   // solver controls (changed by tdgl_set_solver / tdgl_set_sweep_schedule)
   float eps_tol;
   int max_sweeps;
@@ -94,13 +100,16 @@ struct Dev {
   int mu_iterative;
   void *mu_rho, *mu_c, *mu_xa, *mu_xb;
   int *mu_log, *mu_outer_log, *mu_sched;
+  int pair_ok;              // the mesh admits the fused two-sweep kernel (march_pair.cu)
   unsigned long long cond_handle;   // cudaGraphConditionalHandle of the WHILE node (graph mode)
   int use_cond;
 };
 
+// complex products with the contraction spelled out (one product, one FMA per component): the plain sweep and the
+// fused pair kernel must round identically, whatever the compiler would choose in either context
 __device__ __forceinline__ float2 cmul(float2 a, float2 b) {
-  return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+  return make_float2(__fmaf_rn(a.x, b.x, -__fmul_rn(a.y, b.y)), __fmaf_rn(a.x, b.y, __fmul_rn(a.y, b.x)));
 }
 __device__ __forceinline__ float2 cmulc(float2 a, float2 b) {   // conj(a) * b
-  return make_float2(a.x * b.x + a.y * b.y, a.x * b.y - a.y * b.x);
+  return make_float2(__fmaf_rn(a.x, b.x, __fmul_rn(a.y, b.y)), __fmaf_rn(a.x, b.y, -__fmul_rn(a.y, b.x)));
 }
