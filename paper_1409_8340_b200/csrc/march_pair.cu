@@ -3,10 +3,10 @@
 // and not re-reading b, d for sweep l+2.  Per site this kernel reads x^l, b, d once (plus the halo of its tile) and
 // writes x^{l+2}: 32 B instead of 64 B for the two sweeps.
 //
-// A CTA of 19 warps owns a 128 x 16 tile of the xy plane and marches through a chunk of z planes, two pipeline
+// A CTA of 20 warps owns a 128 x 16 tile of the xy plane and marches through a chunk of z planes, two pipeline
 // stages per iteration t:
 //   stage 1  x^{l+1} of plane p1 = k0 - 1 + t on the tile grown by one site (rows -1 .. 16: warps 0 .. 17, one row
-//            each; columns -1 and 128: the column warp, 18), from x^l planes p1 - 1, p1 (registers) and p1 + 1 (TMA
+//            each; columns -1 and 128: one warp each, 18 and 19), from x^l planes p1 - 1, p1 (registers) and p1 + 1 (TMA
 //            stage), written to a three-plane shared-memory ring Y;
 //   stage 2  x^{l+2} of plane p2 = p1 - 1 on the tile itself (warps 1 .. 16) from x^{l+1} planes p2 - 1, p2 and the
 //            in-plane neighbours (all in Y) and p2 + 1 (just computed, registers), written to HBM.
@@ -17,20 +17,20 @@
 //
 // TMA: one stage = x^l rows -2 .. 17 of plane p1 + 1 (three boxes: centre 16 rows, two rows below, two above;
 // wrapped rows for tiles at a periodic seam) and the b, d rows -1 .. 16 of plane p1; ring of 3 stages (56 KB each).
-// The column warp feeds itself with plain 16-byte loads one plane ahead and hands the x^l halo columns to the row
-// warps through a small shared array; it also issues the TMA copies.
+// The column warps feed themselves with plain 16-byte loads one plane ahead and hand the x^l halo columns to the row
+// warps through a small shared array; warp 0 (a halo row: half the work of a centre row) issues the TMA copies.
 // Eligible meshes: xz gauge, nx % 128 == 0, ny % 16 == 0, ny >= 32, nz >= 4 (march_pair_ok); everything else runs
 // plain sweeps only.
 #include "march_common.cuh"
 #include "march_pair.h"
+#include <type_traits>
 
 namespace {
 
 constexpr int TW = 128;                              // tile width (sites)
 constexpr int PH = 16;                               // tile height (rows)
 constexpr int NROWW = PH + 2;                        // row warps: tile rows -1 .. PH
-constexpr int CW = NROWW;                            // index of the column warp
-constexpr int NT = 32 * (NROWW + 1);                 // 608 threads
+constexpr int NT = 32 * (NROWW + 2);                 // + two column warps: 640 threads (17 .. 20 warps leave 96 registers each)
 constexpr unsigned ROWB = 8u * TW;                   // bytes per tile row
 constexpr unsigned OFF_X = 0;                        // x^l: row slots for rows -2 .. PH+1
 constexpr unsigned OFF_B = (PH + 4) * ROWB;          // b: row slots for rows -1 .. PH
@@ -95,11 +95,13 @@ __global__ void __launch_bounds__(NT, 1) k_march_pair(const __grid_constant__ De
     const unsigned sb = stage0 + slot * SB, bar = sbase + 8u * slot;
     const int kz = zw(k0 - 1 + s), kb = zw(k0 - 2 + s);
     const bool bd = s > tb;
-    const unsigned rows_x = PH + (loRow ? 2u : 0u) + (hiRow ? 2u : 0u), rows_b = PH + (loRow ? 1u : 0u) + (hiRow ? 1u : 0u);
+    const unsigned rows_x = PH + 4u, rows_b = PH + (loRow ? 1u : 0u) + (hiRow ? 1u : 0u);
     mbar_expect_tx(bar, ROWB * (rows_x + (bd ? 2u * rows_b : 0u)));
     tma_load_3d(sb + OFF_X + 2 * ROWB, mC, 2 * i0, j0, kz, bar);
-    if (loRow) tma_load_3d(sb + OFF_X, mR, 2 * i0, jlo - 1, kz, bar);
-    if (hiRow) tma_load_3d(sb + OFF_X + (PH + 2) * ROWB, mR, 2 * i0, jhi, kz, bar);
+    // the two rows below / above the tile: real or wrapped rows, or -- at an open y face -- the rows whose mirror
+    // images they are (P:483 with U_y = 1: row -1 = row 1, row ny = row ny - 2), so that "row +- 1" is always one slot away
+    tma_load_3d(sb + OFF_X, mR, 2 * i0, loRow ? jlo - 1 : 0, kz, bar);
+    tma_load_3d(sb + OFF_X + (PH + 2) * ROWB, mR, 2 * i0, hiRow ? jhi : ny - 2, kz, bar);
     if (bd) {
       tma_load_3d(sb + OFF_B + ROWB, &pm.bC, 2 * i0, j0, kb, bar);
       tma_load_3d(sb + OFF_D + ROWB, &pm.dC, 2 * i0, j0, kb, bar);
@@ -123,7 +125,7 @@ __global__ void __launch_bounds__(NT, 1) k_march_pair(const __grid_constant__ De
     *reinterpret_cast<unsigned *>(smem_raw + 68) = 0u;
   }
   __syncthreads();
-  if (tid == CW * 32) { issue(tb); issue(tb + 1); }
+  if (tid == 0) { issue(tb); issue(tb + 1); }
 
   const float2 *__restrict__ xin = dv.psi[xb];
   float2 *__restrict__ xout = dv.psi[xb ^ 1];
@@ -139,120 +141,154 @@ __global__ void __launch_bounds__(NT, 1) k_march_pair(const __grid_constant__ De
     const bool act1 = centre || (rr < 0 ? loRow : hiRow);            // this row takes part in stage 1
     const int jr = centre ? j0 + rr : (rr < 0 ? jlo : jhi);          // its row of the mesh
     const bool ylo = py && jr == 0, yhi = py && jr == ny - 1;        // quasi-periodic jump rows
-    const bool mlo = !py && jr == 0, mhi = !py && jr == ny - 1;      // open y faces: mirror (U_y = 1)
-    const unsigned oX = OFF_X + (unsigned)(rr + 2) * ROWB + 16u * lane;          // own sites, pair A (B: + 512)
-    const unsigned oN = mhi ? oX - ROWB : oX + ROWB, oS = mlo ? oX + ROWB : oX - ROWB;
-    const unsigned oBD = (unsigned)(rr + 1) * ROWB + 16u * lane;                 // within the b / d block
+    // open y faces: the x^{l+1} ghost rows of stage 2 are the mirror images of rows 1 and ny - 2, stored twice
+    const bool dupLo = !py && jr == 1, dupHi = !py && jr == ny - 2;
+    const unsigned oX = OFF_X + (unsigned)(rr + 2) * ROWB + 16u * lane;          // own sites in a stage, pair A (B: + 512);
+    constexpr unsigned DB = OFF_B - ROWB, DD = OFF_D - ROWB;                     //   b, d of the same sites at oX + DB, + DD
     const unsigned oY = (unsigned)(rr + 1) * YPITCH + 16u + 16u * lane;          // own sites in a Y plane
-    const unsigned oYN = mhi ? oY - YPITCH : oY + YPITCH, oYS = mlo ? oY + YPITCH : oY - YPITCH;
-    const unsigned oXrow = OFF_X + (unsigned)(rr + 2) * ROWB, oYrow = (unsigned)(rr + 1) * YPITCH;
     const unsigned oXH = (unsigned)(rr + 1) * 8u;                                // + side * NROWW * 8
-    const int iA = i0 + 2 * lane, iB = iA + 64;
-    const bool xloA = !px && iA == 0, xhiB = !px && iB + 1 == nx - 1;            // open x faces
+    const bool xloA = !px && i0 + 2 * lane == 0, xhiB = !px && i0 + 64 + 2 * lane + 1 == nx - 1;   // open x faces
     const float2 Uxj = dv.Ux[jr], Uzj = dv.Uz[jr];
     const Links L = make_links(make_float2(f * dv.cx * Uxj.x, f * dv.cx * Uxj.y),
                                make_float2(f * dv.cz * Uzj.x, f * dv.cz * Uzj.y), f * dv.cy);
     const float2 U2z = cmul(Uzj, Uzj);
-    const long long rowoff = (long long)jr * nx + iA;
-    long long idx2 = (long long)k0 * plane + rowoff;                 // stage 2 output index of pair A
+    const long long rowoff = (long long)jr * nx + i0 + 2 * lane;
+    float4 *out2 = reinterpret_cast<float4 *>(xout + (long long)k0 * plane + rowoff);   // stage 2 output, pair A
 
-    // The Jacobi update of this thread's four sites of plane `kp`; shared by both stages.  C = own values of that
-    // plane, T / B = own values of the planes above / below (registers); the in-plane neighbours and b, d are read
-    // from shared memory at the given addresses (x^l from a TMA stage or x^{l+1} from a Y plane; pair B at + 512):
-    // aN, aS = rows above / below, aW / aE = the sites left of site 0 / right of site 127 (lanes 0 / 31 only),
-    // aM = site 63 of the own row (sites 63 | 64 are the seam between the pairs of lanes 31 and 0).
-    // One half (pair) at a time keeps the live registers under the 96 of a 608-thread CTA.
-    auto update = [&](int kp, const float4 &CA, const float4 &CB, const float4 &TA, const float4 &TB, const float4 &BA,
-                      const float4 &BB, unsigned aN, unsigned aS, unsigned aW, unsigned aE, unsigned aM, unsigned ab,
-                      unsigned ad, float &rmax, float4 &outA, float4 &outB) {
-      float2 WA, EA, WB, EB;
-      WA.x = __shfl_up_sync(0xffffffffu, CA.z, 1);   WA.y = __shfl_up_sync(0xffffffffu, CA.w, 1);
-      EA.x = __shfl_down_sync(0xffffffffu, CA.x, 1); EA.y = __shfl_down_sync(0xffffffffu, CA.y, 1);
-      WB.x = __shfl_up_sync(0xffffffffu, CB.z, 1);   WB.y = __shfl_up_sync(0xffffffffu, CB.w, 1);
-      EB.x = __shfl_down_sync(0xffffffffu, CB.x, 1); EB.y = __shfl_down_sync(0xffffffffu, CB.y, 1);
-      if (lane == 0) { WA = lds64(aW); WB = lds64(aM); }
-      if (lane == 31) { EA = lds64(aM + 8u); EB = lds64(aE); }
-      if (xloA) WA = cmul(cmul(Uxj, Uxj), hi(CA));       // open x faces: W' = U^2 E, E' = U*^2 W
-      if (xhiB) EB = cmulc(cmul(Uxj, Uxj), lo(CB));
-      float rloc = 0.f;
-      auto half = [&](const float4 &C, const float4 &T, const float4 &B, float2 W, float2 E, unsigned o, int i, float4 &out) {
-        float4 Nn = lds128(aN + o), Ss = lds128(aS + o);
-        if (ylo || yhi) {                                // quasi-periodic jump in y, P_{i,k} = Pi[i] conj(Pk[k])
-          const float2 Pk = dv.Pk[kp];
-          const float4 Pi = *reinterpret_cast<const float4 *>(dv.Pi + i);
-          const float2 P0 = cmulc(Pk, lo(Pi)), P1 = cmulc(Pk, hi(Pi));
-          if (ylo) {                                     // psi_{i,-1,k} = P psi_{i,ny-1,k}
-            const float2 a = cmul(P0, lo(Ss)), b2 = cmul(P1, hi(Ss));
-            Ss = make_float4(a.x, a.y, b2.x, b2.y);
-          }
-          if (yhi) {                                     // psi_{i,ny,k} = P* psi_{i,0,k}
-            const float2 a = cmulc(P0, lo(Nn)), b2 = cmulc(P1, hi(Nn));
-            Nn = make_float4(a.x, a.y, b2.x, b2.y);
-          }
+    // The Jacobi update of ONE pair (two sites) of this thread in plane `kp`; shared by both stages.  C = own values
+    // of that plane, T / B = own values of the planes above / below; the in-plane neighbours are read from shared
+    // memory: aC = address of the own pair in that plane's buffer (x^l: TMA stage, row pitch ROWB; x^{l+1}: Y plane, row
+    // pitch YPITCH), W / E = the x neighbours of the pair's outer sites, ab / ad = b, d of the pair.  One pair at a
+    // time keeps the live registers under the 96 of a 608-thread CTA.
+    auto half = [&](auto fast_tag, int kp, const unsigned pitch, int col, const float4 &C, const float4 &T, const float4 &B,
+                    float2 W, float2 E, unsigned aC, unsigned ab, unsigned ad, float &rmax) -> float4 {
+      constexpr bool FAST = decltype(fast_tag)::value;      // no boundary role in this warp and plane: the checks vanish
+      float4 Nn = lds128(aC + pitch), Ss = lds128(aC - pitch);
+      if (!FAST && (ylo || yhi)) {                       // quasi-periodic jump in y, P_{i,k} = Pi[i] conj(Pk[k])
+        const float2 Pk = dv.Pk[kp];
+        const float4 Pi = *reinterpret_cast<const float4 *>(dv.Pi + col);
+        const float2 P0 = cmulc(Pk, lo(Pi)), P1 = cmulc(Pk, hi(Pi));
+        if (ylo) {                                       // psi_{i,-1,k} = P psi_{i,ny-1,k}
+          const float2 a = cmul(P0, lo(Ss)), b2 = cmul(P1, hi(Ss));
+          Ss = make_float4(a.x, a.y, b2.x, b2.y);
         }
-        const float4 b = lds128(ab + o);
-        float2 s0 = lo(b), s1 = hi(b);
-        nsum_pair(L, C, W, E, Nn, Ss, T, B, s0, s1);
-        out = divide_pair(s0, s1, lds128(ad + o), C, rloc);
-      };
-      half(CA, TA, BA, WA, EA, 0u, iA, outA);
-      half(CB, TB, BB, WB, EB, 512u, iB, outB);
+        if (yhi) {                                       // psi_{i,ny,k} = P* psi_{i,0,k}
+          const float2 a = cmulc(P0, lo(Nn)), b2 = cmulc(P1, hi(Nn));
+          Nn = make_float4(a.x, a.y, b2.x, b2.y);
+        }
+      }
+      const float4 b = lds128(ab);
+      float2 s0 = lo(b), s1 = hi(b);
+      nsum_pair(L, C, W, E, Nn, Ss, T, B, s0, s1);
+      float rloc = 0.f;
+      const float4 out = divide_pair(s0, s1, lds128(ad), C, rloc);
       rmax = fmaxf(rmax, rloc);
+      return out;
+    };
+    // x neighbours of pair A (sites 2 lane, 2 lane + 1) and pair B (64 + 2 lane, ...): shuffles, and for lanes 0 / 31
+    // the sites left of site 0 (aW) / right of site 127 (aE) and the seam 63 | 64 between the pairs of lanes 31 and 0
+    auto xnbA = [&](auto fast_tag, const float4 &CA, unsigned aC, unsigned aW, float2 &W, float2 &E) {
+      constexpr bool FAST = decltype(fast_tag)::value;
+      W.x = __shfl_up_sync(0xffffffffu, CA.z, 1);   W.y = __shfl_up_sync(0xffffffffu, CA.w, 1);
+      E.x = __shfl_down_sync(0xffffffffu, CA.x, 1); E.y = __shfl_down_sync(0xffffffffu, CA.y, 1);
+      const float2 e = lds64(lane == 0 ? aW : aC + 16u);            // (every lane loads: branch-free)
+      if (lane == 0) W = e;
+      if (lane == 31) E = e;
+      if (!FAST && xloA) W = cmul(cmul(Uxj, Uxj), hi(CA));          // open x face: W' = U^2 E
+    };
+    auto xnbB = [&](auto fast_tag, const float4 &CB, unsigned aC, unsigned aE, float2 &W, float2 &E) {
+      constexpr bool FAST = decltype(fast_tag)::value;
+      W.x = __shfl_up_sync(0xffffffffu, CB.z, 1);   W.y = __shfl_up_sync(0xffffffffu, CB.w, 1);
+      E.x = __shfl_down_sync(0xffffffffu, CB.x, 1); E.y = __shfl_down_sync(0xffffffffu, CB.y, 1);
+      const float2 e = lds64(lane == 31 ? aE : aC + 8u * 63u);      // aC = pair A's address
+      if (lane == 0) W = e;
+      if (lane == 31) E = e;
+      if (!FAST && xhiB) E = cmulc(cmul(Uxj, Uxj), lo(CB));         // open x face: E' = U*^2 W
     };
 
-    // x^l ring: this thread's values of planes p1 - 1, p1 stay in registers while plane p1 + 1 arrives
-    float4 xA[3], xB[3];
-    for (int q = 0; q < 3; ++q) xA[q] = xB[q] = make_float4(0.f, 0.f, 0.f, 0.f);
+    // x^l: this thread's values of plane p1 - 1 stay in registers (the stage that held them is being refilled);
+    // planes p1 and p1 + 1 are read from the two resident stages
+    float4 pA = make_float4(0.f, 0.f, 0.f, 0.f), pB = pA;
     if (act1) {
       const long long ob = (long long)zw(k0 - 2 + tb) * plane + rowoff;          // plane below the first stage-1 plane
-      xA[0] = __ldg(reinterpret_cast<const float4 *>(xin + ob));
-      xB[0] = __ldg(reinterpret_cast<const float4 *>(xin + ob + 64));
-      if (lo_ghost) { xA[0] = cmul4(U2z, xA[0]); xB[0] = cmul4(U2z, xB[0]); }   // psi_{-1} = U_z^2 psi_1
+      pA = __ldg(reinterpret_cast<const float4 *>(xin + ob));
+      pB = __ldg(reinterpret_cast<const float4 *>(xin + ob + 64));
+      if (lo_ghost) { pA = cmul4(U2z, pA); pB = cmul4(U2z, pB); }               // psi_{-1} = U_z^2 psi_1
     }
     wait_stage(tb);
-    if (act1) {
-      xA[1] = lds128(stage_of(tb) + oX);
-      xB[1] = lds128(stage_of(tb) + oX + 512u);
-    }
 
     float rdummy = 0.f;                                              // residuals of the halo rows belong to other tiles
-    auto iter = [&](int t, float4 &B1A, float4 &B1B, float4 &C1A, float4 &C1B, float4 &T1A, float4 &T1B) {
+    // B1 = plane p1 - 1 on entry, plane p1 on exit.
+    // FAST: a warp without boundary role (no jump / mirror row, no open x face) on a plane away from the z faces of the
+    // chunk runs a copy of the iteration from which every boundary check is compiled out.
+    auto iter = [&](auto fast_tag, int t, float4 &B1A, float4 &B1B) {
+      constexpr bool FAST = decltype(fast_tag)::value;
       __syncthreads();
-      const bool do1 = t <= te;
+      if (!FAST && tid == 0 && t + 2 <= te + 1) issue(t + 2);        // warp 0 (a halo row: half the work) is the producer
+      const bool do1 = FAST || t <= te;
       const unsigned prv = stage_of(t);
       const unsigned ym = (unsigned)t % NY;
       float4 T2A, T2B;                                               // x^{l+1} of plane p1: stage 1 -> stage 2
       if (do1) {
-        const int p1 = k0 - 1 + t;
+        const int p1 = k0 - 1 + t, kp = FAST ? p1 : zw(p1);
         const unsigned cur = stage_of(t + 1);
         wait_stage(t + 1);
-        if (act1) {
-          T1A = lds128(cur + oX);
-          T1B = lds128(cur + oX + 512u);
-          if (hi_ghost && t == nk) { T1A = cmulc4(U2z, T1A); T1B = cmulc4(U2z, T1B); }   // psi_{nz} = U_z*^2 psi_{nz-2}
+        if (FAST || act1) {
           const unsigned xh = xhbase + (unsigned)(t & 1) * XHPLANE + oXH;
-          update(zw(p1), C1A, C1B, T1A, T1B, B1A, B1B, prv + oN, prv + oS, xh, xh + NROWW * 8u, prv + oXrow + 8u * 63u,
-                 cur + OFF_B + oBD, cur + OFF_D + oBD, centre ? rmax1 : rdummy, T2A, T2B);
+          const bool top = !FAST && hi_ghost && t == nk;             // psi_{nz} = U_z*^2 psi_{nz-2}
+          float &r1 = centre ? rmax1 : rdummy;
+          float2 W, E;
+          {
+            const float4 C = lds128(prv + oX);
+            float4 T = lds128(cur + oX);
+            if (top) T = cmulc4(U2z, T);
+            xnbA(fast_tag, C, prv + oX, xh, W, E);
+            T2A = half(fast_tag, kp, ROWB, i0 + 2 * lane, C, T, B1A, W, E, prv + oX, cur + oX + DB, cur + oX + DD, r1);
+            B1A = C;
+          }
+          {
+            const float4 C = lds128(prv + oX + 512u);
+            float4 T = lds128(cur + oX + 512u);
+            if (top) T = cmulc4(U2z, T);
+            xnbB(fast_tag, C, prv + oX, xh + NROWW * 8u, W, E);
+            T2B = half(fast_tag, kp, ROWB, i0 + 64 + 2 * lane, C, T, B1B, W, E, prv + oX + 512u, cur + oX + DB + 512u,
+                       cur + oX + DD + 512u, r1);
+            B1B = C;
+          }
           const unsigned yw = ybase + ym * YPLANE + oY;
           sts128(yw, T2A);
           sts128(yw + 512u, T2B);
+          if (!FAST) {
+            if (dupLo) { sts128(yw - 2u * YPITCH, T2A); sts128(yw - 2u * YPITCH + 512u, T2B); }
+            if (dupHi) { sts128(yw + 2u * YPITCH, T2A); sts128(yw + 2u * YPITCH + 512u, T2B); }
+          }
         }
       }
-      if (centre && t >= 2) {
+      if (centre && (FAST || t >= 2)) {
         const int p2 = k0 - 2 + t;
-        const unsigned yr = ybase + ((ym + NY - 1) % NY) * YPLANE;     // plane p2
-        const unsigned yb = ybase + ((ym + NY - 2) % NY) * YPLANE;     // plane p2 - 1
-        const float4 C2A = lds128(yr + oY), C2B = lds128(yr + oY + 512u);
-        float4 B2A, B2B;
-        if (lo_ghost && t == 2) { B2A = cmul4(U2z, T2A); B2B = cmul4(U2z, T2B); }   // open bottom face
-        else { B2A = lds128(yb + oY); B2B = lds128(yb + oY + 512u); }
-        if (!do1) { T2A = cmulc4(U2z, B2A); T2B = cmulc4(U2z, B2B); }               // open top face, sweep l + 2
+        const unsigned yr = ybase + ((ym + NY - 1) % NY) * YPLANE + oY;     // own sites in plane p2
+        const unsigned yb = ybase + ((ym + NY - 2) % NY) * YPLANE + oY;     // ... in plane p2 - 1
+        const bool bot = !FAST && lo_ghost && t == 2, top = !FAST && !do1;  // open z faces, sweep l + 2
         float4 outA, outB;
-        update(p2, C2A, C2B, T2A, T2B, B2A, B2B, yr + oYN, yr + oYS, yr + oYrow + 8u, yr + oYrow + 8u * (TW + 2),
-               yr + oYrow + 8u * 65u, prv + OFF_B + oBD, prv + OFF_D + oBD, rmax2, outA, outB);
-        *reinterpret_cast<float4 *>(xout + idx2) = outA;
-        *reinterpret_cast<float4 *>(xout + idx2 + 64) = outB;
-        idx2 += plane;
+        float2 W, E;
+        {
+          const float4 C = lds128(yr);
+          float4 B = bot ? cmul4(U2z, T2A) : lds128(yb);
+          if (top) T2A = cmulc4(U2z, B);
+          xnbA(fast_tag, C, yr, yr - 8u, W, E);
+          outA = half(fast_tag, p2, YPITCH, i0 + 2 * lane, C, T2A, B, W, E, yr, prv + oX + DB, prv + oX + DD, rmax2);
+        }
+        {
+          const float4 C = lds128(yr + 512u);
+          float4 B = bot ? cmul4(U2z, T2B) : lds128(yb + 512u);
+          if (top) T2B = cmulc4(U2z, B);
+          xnbB(fast_tag, C, yr, yr + 512u + 16u, W, E);
+          outB = half(fast_tag, p2, YPITCH, i0 + 64 + 2 * lane, C, T2B, B, W, E, yr + 512u, prv + oX + DB + 512u,
+                      prv + oX + DD + 512u, rmax2);
+        }
+        out2[0] = outA;
+        out2[32] = outB;                                             // + 64 sites
+        out2 += plane / 2;
         if (jact) {
           // J_av (Eq. 35): x links of x^{l+2} inside the tile row, exactly as the plain sweep sums them
           const float nAx = __shfl_down_sync(0xffffffffu, outA.x, 1), nAy = __shfl_down_sync(0xffffffffu, outA.y, 1);
@@ -262,113 +298,93 @@ __global__ void __launch_bounds__(NT, 1) k_march_pair(const __grid_constant__ De
           tsum += jlink(Uxj, outA.x, outA.y, outA.z, outA.w);
           tsum += jlink(Uxj, outA.z, outA.w, nxA.x, nxA.y);
           tsum += jlink(Uxj, outB.x, outB.y, outB.z, outB.w);
-          if (lane < 31) tsum += jlink(Uxj, outB.z, outB.w, rBx, rBy);
+          const float last = jlink(Uxj, outB.z, outB.w, rBx, rBy);
+          tsum += (lane < 31) ? last : 0.f;                          // (adding +0 leaves the sum as it is)
           jacc += (double)tsum;
         }
       }
     };
-
-    // z march; the register ring rotates by renaming over three unrolled iterations
-    for (int t = tb; t <= nk + 1; t += 3) {
-      iter(t, xA[0], xB[0], xA[1], xB[1], xA[2], xB[2]);
-      if (t + 1 <= nk + 1) iter(t + 1, xA[1], xB[1], xA[2], xB[2], xA[0], xB[0]);
-      if (t + 2 <= nk + 1) iter(t + 2, xA[2], xB[2], xA[0], xB[0], xA[1], xB[1]);
+    // warps that may take the fast copy, and the iterations on which every warp may: both stages active, no z face
+    const bool xface = __any_sync(0xffffffffu, xloA || xhiB);
+    const bool wfast = w != 0 && act1 && !(ylo || yhi || dupLo || dupHi || xface);
+    const int tf0 = 3, tf1 = nk - 1;                                 // 3 <= t <= nk - 1
+    // z march
+    for (int t = tb; t <= nk + 1; ++t) {
+      if (wfast && t >= tf0 && t <= tf1) iter(std::true_type{}, t, pA, pB);
+      else iter(std::false_type{}, t, pA, pB);
     }
   } else {
-    // ======================================= column warp =========================================================
-    // lane q < 18 owns the halo sites of tile row q - 1: (row, i0 - 1) on the west side (second site of the pair
-    // loaded from xWp) and (row, i0 + 128) on the east side (first site of the pair loaded from xEp); rows -1 and 16
-    // only supply their x^l values (corners of the halo).
+    // ======================================= column warps ========================================================
+    // Warp 18 owns the halo column i0 - 1, warp 19 the column i0 + 128.  Lane q < 18 owns the halo site of tile row
+    // q - 1; rows -1 and 16 only supply their x^l values (corners of the halo).  The site is one of a 16-byte pair in
+    // HBM: (i0 - 2, i0 - 1) on the west side, (i0 + 128, i0 + 129) on the east side; the other site of the pair is its
+    // outer x neighbour, the inner one is in the TMA stage.  Plain 16-byte loads one plane ahead; the x^l values are
+    // handed to the row warps through the shared array XH.
+    const bool east = w != NROWW;                                    // warp-uniform
+    const bool sideon = east ? eCol : wCol;                          // no halo column beyond an open x face
     const int rr = lane - 1;
     const bool rowok = lane < NROWW && ((rr >= 0 && rr < PH) || (rr < 0 ? loRow : hiRow));
     const bool comp = lane < NROWW && rr >= 0 && rr < PH;
-    const int jr = (rr >= 0 && rr < PH) ? j0 + rr : (rr < 0 ? jlo : jhi);
+    const int jr = min(max((rr >= 0 && rr < PH) ? j0 + rr : (rr < 0 ? jlo : jhi), 0), ny - 1);
+    const bool ld = sideon && rowok, cp = sideon && comp;
     const bool ylo = py && jr == 0, yhi = py && jr == ny - 1, mlo = !py && jr == 0, mhi = !py && jr == ny - 1;
-    const bool ldW = rowok && wCol, ldE = rowok && eCol;
-    const int jc = min(max(jr, 0), ny - 1);
-    const float2 Uxj = dv.Ux[jc], Uzj = dv.Uz[jc];
+    const float2 *xpair = xin + (long long)jr * nx + (east ? xEp : xWp);          // the pair, plane 0
+    const long long bdoff = (long long)jr * nx + (east ? xEp : xWp + 1);         // the halo site itself
+    const unsigned oXin = OFF_X + (unsigned)(rr + 2) * ROWB + (east ? 8u * (TW - 1) : 0u);   // inner neighbour in a stage
+    const unsigned oYc = (unsigned)(rr + 1) * YPITCH + (east ? 8u * (TW + 2) : 8u);
+    const unsigned oXHc = (east ? NROWW * 8u : 0u) + (unsigned)(rr + 1) * 8u;
+    const float2 Uxj = dv.Ux[jr], Uzj = dv.Uz[jr];
     const Links L = make_links(make_float2(f * dv.cx * Uxj.x, f * dv.cx * Uxj.y),
                                make_float2(f * dv.cz * Uzj.x, f * dv.cz * Uzj.y), f * dv.cy);
     const float2 U2z = cmul(Uzj, Uzj);
-    const float2 PiW = dv.Pi[xWp + 1], PiE = dv.Pi[xEp];
-    const long long offW = (long long)jc * nx + xWp, offE = (long long)jc * nx + xEp;
-    const unsigned oXrow = OFF_X + (unsigned)(rr + 2) * ROWB;
-    const unsigned oXH = (unsigned)(rr + 1) * 8u, oYrow = (unsigned)(rr + 1) * YPITCH;
+    const float2 Pic = dv.Pi[east ? xEp : xWp + 1];
     const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
     const float2 z2 = make_float2(0.f, 0.f);
-    auto ldx = [&](int kp, bool on, long long off) -> float4 {
-      return on ? __ldg(reinterpret_cast<const float4 *>(xin + (long long)kp * plane + off)) : z4;
-    };
-    // rings of the two halo columns (pairs), planes p1 - 1, p1, p1 + 1
-    float4 cW[3], cE[3];
-    cW[0] = ldx(zw(k0 - 2 + tb), ldW, offW); cE[0] = ldx(zw(k0 - 2 + tb), ldE, offE);
-    if (lo_ghost) { cW[0] = cmul4(U2z, cW[0]); cE[0] = cmul4(U2z, cE[0]); }
-    cW[1] = ldx(zw(k0 - 1 + tb), ldW, offW); cE[1] = ldx(zw(k0 - 1 + tb), ldE, offE);
-    // the x^l halo columns of the first stage-1 plane for the row warps
-    if (ldW) sts64(xhbase + (unsigned)(tb & 1) * XHPLANE + oXH, hi(cW[1]));
-    if (ldE) sts64(xhbase + (unsigned)(tb & 1) * XHPLANE + NROWW * 8u + oXH, lo(cE[1]));
-    // prefetch: plane p1 + 1 of the first iteration and its b, d
-    float4 nW = ldx(zw(k0 + tb), ldW, offW), nE = ldx(zw(k0 + tb), ldE, offE);
-    auto ldbd = [&](const float2 *arr, int kp, bool on, long long off) -> float2 {
-      return on ? __ldg(arr + (long long)kp * plane + off) : z2;
-    };
-    const bool cpW = comp && wCol, cpE = comp && eCol;
-    float2 bW = ldbd(dv.b, zw(k0 - 1 + tb), cpW, offW + 1), dW = ldbd(dv.d, zw(k0 - 1 + tb), cpW, offW + 1);
-    float2 bE = ldbd(dv.b, zw(k0 - 1 + tb), cpE, offE), dE = ldbd(dv.d, zw(k0 - 1 + tb), cpE, offE);
-
-    auto site = [&](int kp, float2 C, float2 Wn, float2 En, float2 T, float2 B, float2 Pi, float2 b, float2 d) -> float2 {
-      float2 Nn = make_float2(__shfl_down_sync(0xffffffffu, C.x, 1), __shfl_down_sync(0xffffffffu, C.y, 1));
-      float2 Sn = make_float2(__shfl_up_sync(0xffffffffu, C.x, 1), __shfl_up_sync(0xffffffffu, C.y, 1));
-      if (mlo) Sn = Nn;
-      if (mhi) Nn = Sn;
-      if (ylo || yhi) {
-        const float2 P = cmulc(dv.Pk[kp], Pi);
-        if (ylo) Sn = cmul(P, Sn);
-        if (yhi) Nn = cmulc(P, Nn);
-      }
-      const float2 s = nsum_site(L, b, Wn, En, Nn, Sn, T, B);
-      float r = 0.f;
-      const float4 o = divide_pair(s, s, make_float4(d.x, d.y, d.x, d.y), make_float4(C.x, C.y, C.x, C.y), r);
-      return lo(o);
-    };
-
-    auto iter = [&](int t, float4 &BW, float4 &BE, float4 &CWv, float4 &CEv, float4 &TW_, float4 &TE_) {
+    auto ldx = [&](int kp) -> float4 { return ld ? __ldg(reinterpret_cast<const float4 *>(xpair + (long long)kp * plane)) : z4; };
+    auto ldbd = [&](const float2 *arr, int kp) -> float2 { return cp ? __ldg(arr + (long long)kp * plane + bdoff) : z2; };
+    auto own = [&](const float4 &v) -> float2 { return east ? lo(v) : hi(v); };
+    auto outer = [&](const float4 &v) -> float2 { return east ? hi(v) : lo(v); };
+    float4 cB = ldx(zw(k0 - 2 + tb));                                // planes p1 - 1, p1 and (prefetched) p1 + 1
+    if (lo_ghost) cB = cmul4(U2z, cB);
+    float4 cC = ldx(zw(k0 - 1 + tb));
+    if (ld) sts64(xhbase + (unsigned)(tb & 1) * XHPLANE + oXHc, own(cC));       // x^l halo column of the first plane
+    float4 cN = ldx(zw(k0 + tb));
+    float2 cb = ldbd(dv.b, zw(k0 - 1 + tb)), cd = ldbd(dv.d, zw(k0 - 1 + tb)); // b, d of plane p1 (prefetched)
+    for (int t = tb; t <= nk + 1; ++t) {
       __syncthreads();
-      if (lane == 0 && t + 2 <= te + 1) issue(t + 2);
-      if (t <= te) {
-        const int p1 = k0 - 1 + t;
-        const unsigned prv = stage_of(t);
-        wait_stage(t);                                                  // (complete since the last iteration: visibility only)
-        TW_ = nW; TE_ = nE;
-        const float2 b_w = bW, d_w = dW, b_e = bE, d_e = dE;
-        if (t + 1 <= te) {                                              // next plane's loads in flight during this one
-          nW = ldx(zw(p1 + 2), ldW, offW); nE = ldx(zw(p1 + 2), ldE, offE);
-          bW = ldbd(dv.b, zw(p1 + 1), cpW, offW + 1); dW = ldbd(dv.d, zw(p1 + 1), cpW, offW + 1);
-          bE = ldbd(dv.b, zw(p1 + 1), cpE, offE); dE = ldbd(dv.d, zw(p1 + 1), cpE, offE);
-        }
-        if (hi_ghost && t == nk) { TW_ = cmulc4(U2z, TW_); TE_ = cmulc4(U2z, TE_); }
-        // hand the x^l halo columns of plane p1 + 1 to the row warps of the next iteration
-        const unsigned xh = xhbase + (unsigned)((t + 1) & 1) * XHPLANE + oXH;
-        if (ldW) sts64(xh, hi(TW_));
-        if (ldE) sts64(xh + NROWW * 8u, lo(TE_));
-        // stage 1 on the halo sites (tile rows 0 .. PH-1); neighbours inside the tile come from the TMA stage
-        const unsigned yw = ybase + ((unsigned)t % NY) * YPLANE + oYrow;
-        if (wCol) {                                                     // warp-uniform
-          const float2 En = comp ? lds64(prv + oXrow) : z2;
-          const float2 o = site(zw(p1), hi(CWv), lo(CWv), En, hi(TW_), hi(BW), PiW, b_w, d_w);
-          if (comp) sts64(yw + 8u, o);
-        }
-        if (eCol) {
-          const float2 Wn = comp ? lds64(prv + oXrow + 8u * (TW - 1)) : z2;
-          const float2 o = site(zw(p1), lo(CEv), Wn, hi(CEv), lo(TE_), lo(BE), PiE, b_e, d_e);
-          if (comp) sts64(yw + 8u * (TW + 2), o);
-        }
+      if (t > te) continue;
+      const int p1 = k0 - 1 + t;
+      const unsigned prv = stage_of(t);
+      wait_stage(t);                                                  // (complete since the last iteration: visibility only)
+      float4 cT = cN;
+      const float2 b_ = cb, d_ = cd;
+      if (t + 1 <= te) {                                              // next plane's loads in flight during this one
+        cN = ldx(zw(p1 + 2));
+        cb = ldbd(dv.b, zw(p1 + 1));
+        cd = ldbd(dv.d, zw(p1 + 1));
       }
-    };
-    for (int t = tb; t <= nk + 1; t += 3) {
-      iter(t, cW[0], cE[0], cW[1], cE[1], cW[2], cE[2]);
-      if (t + 1 <= nk + 1) iter(t + 1, cW[1], cE[1], cW[2], cE[2], cW[0], cE[0]);
-      if (t + 2 <= nk + 1) iter(t + 2, cW[2], cE[2], cW[0], cE[0], cW[1], cE[1]);
+      if (hi_ghost && t == nk) cT = cmulc4(U2z, cT);
+      if (ld) sts64(xhbase + (unsigned)((t + 1) & 1) * XHPLANE + oXHc, own(cT));   // for the row warps' next iteration
+      if (sideon) {
+        // stage 1 on the halo sites; N / S neighbours are the lanes above / below
+        const float2 C = own(cC);
+        float2 Nn = make_float2(__shfl_down_sync(0xffffffffu, C.x, 1), __shfl_down_sync(0xffffffffu, C.y, 1));
+        float2 Sn = make_float2(__shfl_up_sync(0xffffffffu, C.x, 1), __shfl_up_sync(0xffffffffu, C.y, 1));
+        if (mlo) Sn = Nn;                                              // open y faces: mirror (U_y = 1)
+        if (mhi) Nn = Sn;
+        if (ylo || yhi) {
+          const float2 P = cmulc(dv.Pk[zw(p1)], Pic);
+          if (ylo) Sn = cmul(P, Sn);
+          if (yhi) Nn = cmulc(P, Nn);
+        }
+        const float2 inner = comp ? lds64(prv + oXin) : z2;
+        const float2 sm = nsum_site(L, b_, east ? inner : outer(cC), east ? outer(cC) : inner, Nn, Sn, own(cT), own(cB));
+        float r = 0.f;
+        const float4 o = divide_pair(sm, sm, make_float4(d_.x, d_.y, d_.x, d_.y), make_float4(C.x, C.y, C.x, C.y), r);
+        if (comp) sts64(ybase + ((unsigned)t % NY) * YPLANE + oYc, lo(o));
+      }
+      cB = cC;
+      cC = cT;
     }
   }
 
