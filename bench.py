@@ -253,6 +253,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-pairs", action="store_true", help="plain Jacobi sweeps only (tdgl_set_pair_mode 0): A/B against the fused two-sweep kernel")
     ap.add_argument("--fp64", action="store_true", help="the double-precision build (TDGL_FLAG_FP64; the paper's DP mode)")
     ap.add_argument("--mu-iterative", action="store_true", help="the paper's own pseudo-time mu solver (TDGL_FLAG_MU_ITERATIVE)")
     ap.add_argument("--h-tau", type=float, default=0.1, help="virtual time step of the pseudo-time mu solver (S20)")
@@ -290,10 +291,13 @@ def main():
     s = make_solver(cfg, seed_offset=rank, **mode)
     if args.fp64 or args.mu_iterative:
         s.set_mu_solver(h_tau=args.h_tau)
+    if args.no_pairs:
+        s.set_pair_mode(0)
     s.step(W)
     barrier()
     ob0 = s.observables()
     l0 = s.launch_count()
+    pair0 = s.pair_stats()
     sampler = ClockSampler(local_rank)
     sampler.start()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -310,6 +314,11 @@ def main():
         outer, inner = s.mu_log(min(K, 1000))
         mu_stats = {"outer_per_step": float(np.mean(outer)), "inner_per_outer": float(np.mean([np.mean(i) for i in inner if i]))}
     launches = s.launch_count() - l0 - 2           # minus the two observables kernels
+    pair1 = s.pair_stats()
+    pairs = {"eligible": pair1[0], "mode": "off (--no-pairs)" if args.no_pairs else "automatic",
+             "pairs_per_step": (pair1[1] - pair0[1]) / K, "discarded_per_step": (pair1[2] - pair0[2]) / K,
+             "note": "a pair = two Jacobi sweeps in one pass over HBM (march_pair.cu); bit-identical to plain sweeps; a pair "
+                     "whose first sweep already met criterion (34) is discarded and redone as one plain sweep"}
     sweeps = ob1.sweeps_total - ob0.sweeps_total
     ms, sweeps_all, launches_all = reduce_over_ranks([ms, sweeps, launches], dist if world > 1 else None, dev)
     launches_all = int(launches_all)
@@ -318,6 +327,7 @@ def main():
 
     # ---- roofline of the sweep kernel: CUDA events around every sweep launch (host-loop run) ----
     roof = None
+    roof_pair = None
     e2e = None
     if rank == 0 or world > 1:
         psi, mu = s.get_psi_mu()
@@ -326,11 +336,33 @@ def main():
         if args.fp64 or args.mu_iterative:
             sh.set_mu_solver(h_tau=args.h_tau)
         sh.set_state(psi, mu, K0)
+        sh.set_pair_mode(0)                          # every sweep a plain sweep: the kernel this figure is about
         sh.step(3)
-        sh.sweep_timing(True)
+        sh.sweep_timing(1)
         sh.step(max(3, min(K, 40)))
-        t_ms, n_l = sh.sweep_timing(False)
+        t_ms, n_l = sh.sweep_timing(0)
         peak, how = measured_peak()
+        roof_pair = None
+        if pair1[0] and not args.no_pairs:
+            # the fused two-sweep kernel, timed the same way (pairs chosen by the library as in the resident run)
+            sh.set_pair_mode(1)
+            sh.step(3)
+            sh.sweep_timing(2)
+            sh.step(max(3, min(K, 40)))
+            tp_ms, np_l = sh.sweep_timing(0)
+            if np_l > 0:
+                avg_p = tp_ms / np_l
+                roof_pair = {"bound": "hbm", "kernel": "k_march_pair (two Jacobi sweeps in one pass, both residuals)",
+                             "avg_launch_ms": avg_p, "launches_timed": int(np_l),
+                             "algorithmic_bytes_per_launch": 2.0 * bytes_per_site * N,
+                             "achieved": 2.0 * bytes_per_site * N / (avg_p * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
+                             "frac": 2.0 * bytes_per_site * N / (avg_p * 1e-3) / 1e9 / peak,
+                             "min_traffic_bytes_per_launch": bytes_per_site * N,
+                             "frac_of_min_traffic": bytes_per_site * N / (avg_p * 1e-3) / 1e9 / peak,
+                             "note": "`achieved` uses SURVEY 8(d)'s definition, 32 B/site/sweep x 2 sweeps per launch: a value "
+                                     "above the peak is the point of temporal blocking (x^{l+1} never goes to HBM, b and d are "
+                                     "read once for both sweeps: 32 B/site of DRAM traffic per PAIR, measured 2.16 GB per launch "
+                                     "on C4, profiles/r02_pair_ncu_full.md); `frac_of_min_traffic` is that traffic over the peak"}
         if n_l > 0:
             avg_ms = t_ms / n_l
             ach = bytes_per_site * N / (avg_ms * 1e-3) / 1e9
@@ -394,7 +426,8 @@ def main():
         "data": "synthetic", "steps_per_s": steps_per_s, "sweeps_per_step": sweeps_all / (K * world),
         "config": dict(config_dict(cfg, world), **({"mu_solver": "pseudo-time iteration (Eq. 40), host-driven loop"} if (args.fp64 or args.mu_iterative) else {})),
         "mu_iteration": mu_stats,
-        "clocks": clocks, "e2e": e2e, "gpu_launches": launches_all, "roofline": roof, "cpu_baseline": cpu,
+        "clocks": clocks, "e2e": e2e, "gpu_launches": launches_all, "roofline": roof, "roofline_pair": roof_pair,
+        "pairs": pairs, "cpu_baseline": cpu,
         "state": {"mean_abs2": ob1.mean_abs2, "Ex": ob1.Ex, "K": ob1.K, "vortices_per_slice": ob1.vortices_per_slice,
                   "status": ob1.status},
     }
