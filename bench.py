@@ -253,6 +253,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--pair-mode", type=int, default=1, help="tdgl_set_pair_mode: 1 automatic (default), 2 whenever the cap allows")
     ap.add_argument("--no-pairs", action="store_true", help="plain Jacobi sweeps only (tdgl_set_pair_mode 0): A/B against the fused two-sweep kernel")
     ap.add_argument("--fp64", action="store_true", help="the double-precision build (TDGL_FLAG_FP64; the paper's DP mode)")
     ap.add_argument("--mu-iterative", action="store_true", help="the paper's own pseudo-time mu solver (TDGL_FLAG_MU_ITERATIVE)")
@@ -291,8 +292,8 @@ def main():
     s = make_solver(cfg, seed_offset=rank, **mode)
     if args.fp64 or args.mu_iterative:
         s.set_mu_solver(h_tau=args.h_tau)
-    if args.no_pairs:
-        s.set_pair_mode(0)
+    if args.no_pairs or args.pair_mode != 1:
+        s.set_pair_mode(0 if args.no_pairs else args.pair_mode)
     s.step(W)
     barrier()
     ob0 = s.observables()

@@ -141,10 +141,14 @@ __device__ __forceinline__ void choose_next(const Dev &dv, Ctl *c, int sweeps, i
     if (target > 0) up = target - sweeps >= 2;
     else if (sweeps + 2 <= c->max_sweeps) {
       if (c->pair_mode == 2) up = 1;
-      else if (r_prev > 0.f) {                           // geometric decay: next residual ~ r_last * (r_last / r_prev)
-        const float q = fminf(1.f, r_last / r_prev);
-        up = r_last * q >= 3.f * c->eps_tol;
-      } else up = c->sweeps_last >= sweeps + 2;           // first decision of a step: the previous step's count
+      else {
+        // Two more sweeps are needed iff the NEXT residual is still >= eps.  Two predictors: geometric decay of the last two
+        // residuals (trusted alone when it says "far above eps"), and the previous time step, whose sweep count the
+        // present one rarely undercuts (a pair that ends at or before that count is taken unless the decay says the next
+        // sweep converges).  A wrong guess costs one discarded pair, never a wrong result.
+        const float next = r_prev > 0.f ? r_last * fminf(1.f, r_last / r_prev) : r_last;
+        up = next >= 10.f * c->eps_tol || (sweeps + 2 <= c->sweeps_last && next >= c->eps_tol);
+      }
     }
   }
   c->use_pair = up;

@@ -191,7 +191,8 @@ __global__ void __launch_bounds__(NT, 1) k_march_pair(const __grid_constant__ De
       constexpr bool FAST = decltype(fast_tag)::value;
       W.x = __shfl_up_sync(0xffffffffu, CA.z, 1);   W.y = __shfl_up_sync(0xffffffffu, CA.w, 1);
       E.x = __shfl_down_sync(0xffffffffu, CA.x, 1); E.y = __shfl_down_sync(0xffffffffu, CA.y, 1);
-      const float2 e = lds64(lane == 0 ? aW : aC + 16u);            // (every lane loads: branch-free)
+      const float2 e = lds64(lane == 0 ? aW : (lane == 31 ? aC + 16u : xhbase));   // every lane loads (branch-free); the
+                                                                                    // idle lanes share one address (broadcast)
       if (lane == 0) W = e;
       if (lane == 31) E = e;
       if (!FAST && xloA) W = cmul(cmul(Uxj, Uxj), hi(CA));          // open x face: W' = U^2 E
@@ -200,7 +201,7 @@ __global__ void __launch_bounds__(NT, 1) k_march_pair(const __grid_constant__ De
       constexpr bool FAST = decltype(fast_tag)::value;
       W.x = __shfl_up_sync(0xffffffffu, CB.z, 1);   W.y = __shfl_up_sync(0xffffffffu, CB.w, 1);
       E.x = __shfl_down_sync(0xffffffffu, CB.x, 1); E.y = __shfl_down_sync(0xffffffffu, CB.y, 1);
-      const float2 e = lds64(lane == 31 ? aE : aC + 8u * 63u);      // aC = pair A's address
+      const float2 e = lds64(lane == 31 ? aE : (lane == 0 ? aC + 8u * 63u : xhbase));   // aC = pair A's address
       if (lane == 0) W = e;
       if (lane == 31) E = e;
       if (!FAST && xhiB) E = cmulc(cmul(Uxj, Uxj), lo(CB));         // open x face: E' = U*^2 W
