@@ -223,7 +223,8 @@ int tdgl_sweep_timing(tdgl_t *h, int32_t enable, double *ms_total_host, int64_t 
  * (prescribed counts) or predicted from the residual history.  Criterion (34) stays exact: both residuals are reduced,
  * and a pair whose first sweep already met the criterion is discarded and redone as a plain sweep, so psi, the sweep
  * counts, the residual log and J_av are bit-identical to plain sweeps.  mode: 0 never, 1 automatic (default), 2 whenever
- * the cap max_sweeps allows (tests: forces the redo path).  tdgl_get_pair_stats: whether the mesh is eligible, pairs
+ * the cap max_sweeps allows (tests: forces the redo path), 3 as 2 and a pair never sums the J_av links of its output (tests:
+ * forces the separate pass k_jav_tiles, which otherwise runs only when a pair predicted not to end the step did end it).  tdgl_get_pair_stats: whether the mesh is eligible, pairs
  * launched, pairs discarded since create. */
 int tdgl_set_pair_mode(tdgl_t *h, int32_t mode);
 int tdgl_get_pair_stats(tdgl_t *h, int32_t *eligible_host, int64_t *pairs_host, int64_t *redone_host);

@@ -21,7 +21,7 @@ __global__ void k_ctl_reset(const __grid_constant__ Dev dv, float eps_tol, int m
   Ctl *c = dv.ctl;
   c->K = 0.0; c->Ex = 0.0; c->Jav = 0.0; c->Ex_sum = 0.0; c->Ex_cnt = 0; c->n = 0; c->sweeps_total = 0;
   c->sweeps = 0; c->done = 0; c->xbuf = 0; c->status = 0; c->sweeps_last = 0; c->resid_last = 0.f;
-  c->ticket = 0u; c->ticket2 = 0u; c->use_pair = 0; c->pair_mode = 1; c->r_hist = 0.f;
+  c->ticket = 0u; c->ticket2 = 0u; c->use_pair = 0; c->pair_mode = 1; c->pair_jav = 1; c->need_jav = 0; c->r_hist = 0.f;
   c->pair_launches = 0; c->pair_redone = 0; c->body_launches = 0;
   c->eps_tol = eps_tol; c->max_sweeps = max_sweeps; c->fixed_sweeps = fixed_sweeps;
   c->sched_n = 0; c->sched_pos = 0; c->Jext = 0.0; c->Bx = 0.0; c->Bz = 0.0;

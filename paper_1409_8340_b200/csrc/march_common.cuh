@@ -139,22 +139,31 @@ __device__ __forceinline__ float jlink(float2 U, float ar, float ai, float br, f
 // (prescribed counts) or predicted from the residual history (criterion (34) stays exact either way: a pair whose
 // FIRST sweep already met it is discarded and redone as a plain sweep, see pair_decide).
 __device__ __forceinline__ void choose_next(const Dev &dv, Ctl *c, int sweeps, int target, float r_last, float r_prev) {
-  int up = 0;
+  int up = 0, jav = 1;
   if (dv.pair_ok && c->pair_mode > 0) {
-    if (target > 0) up = target - sweeps >= 2;
-    else if (sweeps + 2 <= c->max_sweeps) {
-      if (c->pair_mode == 2) up = 1;
-      else {
-        // Two more sweeps are needed iff the NEXT residual is still >= eps.  Two predictors: geometric decay of the last two
-        // residuals (trusted alone when it says "far above eps"), and the previous time step, whose sweep count the
-        // present one rarely undercuts (a pair that ends at or before that count is taken unless the decay says the next
-        // sweep converges).  A wrong guess costs one discarded pair, never a wrong result.
-        const float next = r_prev > 0.f ? r_last * fminf(1.f, r_last / r_prev) : r_last;
-        up = next >= 10.f * c->eps_tol || (sweeps + 2 <= c->sweeps_last && next >= c->eps_tol);
-      }
+    if (target > 0) {
+      up = target - sweeps >= 2;
+      jav = sweeps + 2 >= target;                          // only the last sweep's J_av is used
+    } else if (sweeps + 2 <= c->max_sweeps) {
+      // Two more sweeps are needed iff the NEXT residual is still >= eps.  Two predictors: geometric decay of the last two
+      // residuals (trusted alone when it says "far above eps"), and the previous time step, whose sweep count the
+      // present one rarely undercuts (a pair that ends at or before that count is taken unless the decay says the next
+      // sweep converges).  A wrong guess costs one discarded pair, never a wrong result.
+      const float q = r_prev > 0.f ? fminf(1.f, r_last / r_prev) : 1.f;
+      const float next = r_last * q, next2 = next * q;
+      up = next >= 10.f * c->eps_tol || (sweeps + 2 <= c->sweeps_last && next >= c->eps_tol);
+      // The J_av link sums of a pair's output (17 % of its time on C4) are needed only if its second sweep ends the
+      // step: skipped when the residual after the pair is predicted far above eps, or when the previous step needed
+      // more sweeps than the pair reaches.  A wrong guess costs one pass of k_jav_tiles.
+      jav = !(r_prev > 0.f ? (next2 >= 10.f * c->eps_tol || (sweeps + 2 < c->sweeps_last && next2 >= c->eps_tol))
+                           : sweeps + 2 < c->sweeps_last);
+      if (sweeps + 2 >= c->max_sweeps) jav = 1;          // the cap would end the step with this pair
+      if (c->pair_mode >= 2) up = 1;
+      if (c->pair_mode == 3) jav = 0;
     }
   }
   c->use_pair = up;
+  c->pair_jav = jav;
 }
 
 __device__ __noinline__ void sweep_decide(const Dev &dv, int l) {
@@ -177,6 +186,7 @@ __device__ __noinline__ void sweep_decide(const Dev &dv, int l) {
   if (done) {
     c->done = 1;
     c->use_pair = 0;
+    c->need_jav = 0;                                    // a plain sweep always sums its J_av links
     c->sweeps_last = sweeps;
     c->resid_last = r2;
   }
@@ -208,6 +218,7 @@ __device__ __noinline__ void pair_decide(const Dev &dv, int l) {
       done = (r2 < c->eps_tol) || sweeps >= c->max_sweeps;
       if (!(r2 < c->eps_tol) && sweeps >= c->max_sweeps) c->status = 1;
     }
+    const int had_jav = c->pair_jav;                    // (read before choose_next overwrites it)
     choose_next(dv, c, sweeps, target, r2, r1);
     c->r_hist = r2;
     if (done) {
@@ -215,6 +226,7 @@ __device__ __noinline__ void pair_decide(const Dev &dv, int l) {
       c->use_pair = 0;
       c->sweeps_last = sweeps;
       c->resid_last = r2;
+      c->need_jav = !had_jav;                           // the last sweep did not sum its J_av links: k_jav_tiles will
     }
   }
   if (dv.use_cond) cudaGraphSetConditional((cudaGraphConditionalHandle)dv.cond_handle, done ? 0u : 1u);

@@ -132,7 +132,7 @@ __global__ void __launch_bounds__(NT, 1) k_march_pair(const __grid_constant__ De
   const float f = dv.ht2;
   float rmax1 = 0.f, rmax2 = 0.f;
   double jacc = 0.0;
-  const bool jact = dv.solve_mu && px;
+  const bool jact = dv.solve_mu && px && ctl->pair_jav;   // J_av link sums only if this pair may end the step (choose_next)
 
   if (w < NROWW) {
     // ======================================= row warps ===========================================================
@@ -424,6 +424,44 @@ __global__ void __launch_bounds__(NT, 1) k_march_pair(const __grid_constant__ De
   }
 }
 
+// J_av link sums of the current iterate per 128 x 8 tile and z chunk of the plain sweep's grid, exactly as the sweep
+// kernels form them on their own output (same lane layout, same order: bit-identical partial sums).  Acts only when the
+// step ended with a fused pair that had been told to skip them (ctl->need_jav, choose_next): one 8 B/site pass.
+__global__ void __launch_bounds__(256) k_jav_tiles(const __grid_constant__ Dev dv) {
+  Ctl *ctl = dv.ctl;
+  if (!ctl->need_jav) return;
+  __shared__ double s_j[8];
+  const int lane = threadIdx.x & 31, row = threadIdx.x >> 5;
+  const int j = blockIdx.y * 8 + row;
+  const int k0 = blockIdx.z * dv.zc, k1 = min(dv.nz, k0 + dv.zc);
+  const long long plane = (long long)dv.nx * dv.ny;
+  const float4 *x = reinterpret_cast<const float4 *>(dv.psi[ctl->xbuf] + (long long)k0 * plane + (long long)j * dv.nx +
+                                                      blockIdx.x * TW + 2 * lane);
+  const float2 Uxj = dv.Ux[j];
+  double jacc = 0.0;
+  for (int k = k0; k < k1; ++k, x += plane / 2) {
+    const float4 outA = __ldcs(x), outB = __ldcs(x + 32);
+    const float nAx = __shfl_down_sync(0xffffffffu, outA.x, 1), nAy = __shfl_down_sync(0xffffffffu, outA.y, 1);
+    const float rBx = __shfl_sync(0xffffffffu, outB.x, (lane + 1) & 31), rBy = __shfl_sync(0xffffffffu, outB.y, (lane + 1) & 31);
+    const float2 nxA = (lane == 31) ? make_float2(rBx, rBy) : make_float2(nAx, nAy);
+    float tsum = 0.f;
+    tsum += jlink(Uxj, outA.x, outA.y, outA.z, outA.w);
+    tsum += jlink(Uxj, outA.z, outA.w, nxA.x, nxA.y);
+    tsum += jlink(Uxj, outB.x, outB.y, outB.z, outB.w);
+    const float last = jlink(Uxj, outB.z, outB.w, rBx, rBy);
+    tsum += (lane < 31) ? last : 0.f;
+    jacc += (double)tsum;
+  }
+  for (int o = 16; o > 0; o >>= 1) jacc += __shfl_down_sync(0xffffffffu, jacc, o);
+  if (lane == 0) s_j[row] = jacc;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double sj = 0.0;
+    for (int q = 0; q < 8; ++q) sj += s_j[q];
+    dv.jpart[blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z)] = sj;
+  }
+}
+
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
                                   const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -474,4 +512,10 @@ cudaError_t march_pair_configure() {
 void launch_march_pair(const Dev &dv, const PairMaps &pm, cudaStream_t st) {
   const dim3 grid((unsigned)(dv.nx / TW), (unsigned)(dv.ny / PH), (unsigned)((dv.nz + dv.zc - 1) / dv.zc));
   k_march_pair<<<grid, NT, SMEM, st>>>(dv, pm);
+}
+
+// grid of the plain sweep (128 x 8 tiles, dv.zc planes): one partial sum per CTA, where k_step_finish expects it
+void launch_jav_tiles(const Dev &dv, cudaStream_t st) {
+  const dim3 grid((unsigned)(dv.nx / TW), (unsigned)(dv.ny / 8), (unsigned)((dv.nz + dv.zc - 1) / dv.zc));
+  k_jav_tiles<<<grid, 256, 0, st>>>(dv);
 }

@@ -15,3 +15,4 @@ bool march_pair_ok(int nx, int ny, int nz, bool gauge_yz);
 int march_pair_build_maps(const Dev &dv, PairMaps *pm);
 cudaError_t march_pair_configure();
 void launch_march_pair(const Dev &dv, const PairMaps &pm, cudaStream_t st);
+void launch_jav_tiles(const Dev &dv, cudaStream_t st);

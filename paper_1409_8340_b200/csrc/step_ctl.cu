@@ -59,6 +59,8 @@ __global__ void k_step_begin(const __grid_constant__ Dev dv) {
     c->sweeps = 0;
     c->done = 0;
     c->use_pair = 0;
+    c->pair_jav = 1;
+    c->need_jav = 0;
     c->ticket = 0u;
   }
   write_Ux(dv, c->K, tid, blockDim.x);

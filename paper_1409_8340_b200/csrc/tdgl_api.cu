@@ -342,6 +342,7 @@ static int enqueue_after_solve(tdgl_t *h, cudaStream_t st) {
   } else {
     // J_av: the in-tile x links were summed by the last sweep (one partial per CTA); the links that cross a
     // tile edge are summed here
+    if (kact && h->dv.pair_ok) { launch_jav_tiles(h->dv, st); ++n; }   // (acts only after a pair that skipped its J_av sums)
     if (kact) { launch_jav_edges(h->dv, march_tma_tile_w(), h->jav_blocks, st); ++n; }
     launch_step_finish(h->dv, (int)(h->mgrid.x * h->mgrid.y * h->mgrid.z), h->jav_blocks, st); ++n;
   }
@@ -946,7 +947,7 @@ extern "C" int64_t tdgl_launch_count(const tdgl_t *h) {
 }
 
 extern "C" int tdgl_set_pair_mode(tdgl_t *h, int32_t mode) {
-  if (!h || mode < 0 || mode > 2) return TDGL_EINVAL;
+  if (!h || mode < 0 || mode > 3) return TDGL_EINVAL;
   launch_ctl_pair_mode(h->dv, mode, h->stream);
   h->launches += 1;
   CKL();

@@ -27,8 +27,11 @@ struct Ctl {
   unsigned int ticket;      // last-block election of the sweep kernel
   unsigned int ticket2;     // ... of the reduction kernels
   // fused sweep pairs (march_pair.cu): 0 never, 1 when the residual history predicts that both sweeps are needed,
-  // 2 whenever the cap allows (tests: exercises the redo path); residual of the previous sweep; statistics
+  // 2 whenever the cap allows (tests: exercises the redo path), 3 as 2 and never summing J_av inside a pair (tests:
+  // exercises k_jav_tiles); residual of the previous sweep; statistics
   int pair_mode;
+  int pair_jav;             // the next pair sums the J_av links of its output (it may be the last sweep of the step)
+  int need_jav;             // the last sweep was a pair that did not: k_jav_tiles sums them
   float r_hist;
   long long pair_launches, pair_redone, body_launches;
   // solver controls (changed by tdgl_set_solver / tdgl_set_sweep_schedule)

@@ -4,7 +4,7 @@ Two gates.  (1) Against the fp64 oracle, with the tolerances of the plain path (
 plain sweep kernel: x^{l+1}, x^{l+2}, both residuals and the J_av partial sums use the same arithmetic in the same
 order, and criterion (34) is kept exact by discarding a pair whose first sweep already met it, so psi, mu, K, the sweep
 counts and the residual log must be BIT-identical whether pairs are never used (mode 0), used when predicted (mode 1) or
-forced (mode 2, which exercises the discard-and-redo path).
+forced (mode 2, which exercises the discard-and-redo path; mode 3 also forces the separate J_av pass k_jav_tiles).
 """
 import numpy as np
 import pytest
@@ -83,7 +83,7 @@ def test_tolerance_runs_are_bit_identical_in_all_pair_modes(bc, shape, host_loop
                  temperature=1e-3, incl_fraction=0.15, incl_rmin=1.0, incl_rmax=2.0, seed=5)
     nsteps = 25
     out = []
-    for mode in (0, 1, 2):
+    for mode in (0, 1, 2, 3):                                         # 3: forced pairs that never sum J_av (k_jav_tiles does)
         p, st, eps, (Bx, Bz), s = setup_pair(cfg, host_loop=host_loop)
         s.set_pair_mode(mode)
         s.step(nsteps)
@@ -94,7 +94,8 @@ def test_tolerance_runs_are_bit_identical_in_all_pair_modes(bc, shape, host_loop
     ref = out[0]
     assert ref[5][1] == 0
     assert out[1][5][1] > 0                                           # the prediction did launch pairs
-    assert out[2][5][1] > out[1][5][1] and out[2][5][2] > 0           # forced: more pairs, some discarded and redone
+    assert out[2][5][1] >= out[1][5][1] and out[2][5][2] > 0          # forced: some pairs discarded and redone
+    assert out[3][5][1:] == out[2][5][1:]
     for o in out[1:]:
         assert o[3] == ref[3] and o[4] == ref[4]
         assert np.array_equal(o[0].view(np.float32), ref[0].view(np.float32)) and np.array_equal(o[1], ref[1])
