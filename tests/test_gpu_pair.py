@@ -135,3 +135,27 @@ def test_schedule_and_cap_with_pairs():
         s.close()
     assert np.array_equal(res[0][0].view(np.float32), res[2][0].view(np.float32))
     assert np.array_equal(res[1][0].view(np.float32), res[3][0].view(np.float32))
+
+
+@pytest.mark.parametrize("shape", [(128, 32, 4), (128, 32, 33), (384, 32, 5), (128, 96, 17)])
+@pytest.mark.parametrize("bc", [(P_, P_, P_), (O_, P_, O_), (P_, O_, P_)])
+def test_smallest_and_ragged_meshes_forced_pairs(shape, bc):
+    """The smallest eligible mesh (nz = 4, ny = 32), one-plane and ragged last z chunks (nz = 33, 17, 5), three tiles in x:
+    forced pairs (incl. the discard-and-redo path and k_jav_tiles) against plain sweeps, bit for bit, 12 noisy steps."""
+    nx, ny, nz = shape
+    cfg = cfg_of(nx, ny, nz, bc, Bx=0.03, Bz=0.3, Jx=0.02 if bc[0] == P_ else 0.0, temperature=1e-3, incl_fraction=0.1,
+                 incl_rmin=1.0, incl_rmax=2.0, seed=11)
+    out = []
+    for mode in (0, 3):
+        p, st, eps, (Bx, Bz), s = setup_pair(cfg)
+        s.set_pair_mode(mode)
+        s.step(12)
+        psi, mu, ob = state_of(s)
+        out.append((psi, mu, ob, list(s.sweep_log(12)[0]), s.pair_stats()))
+        s.close()
+    a, b = out
+    assert b[4][1] > 0 and a[3] == b[3]
+    assert np.array_equal(a[0].view(np.float32), b[0].view(np.float32)) and np.array_equal(a[1], b[1])
+    assert a[2].K == b[2].K and a[2].Jav == b[2].Jav
+    O.run(p, st, eps, Bx, Bz, f32(cfg.Jx), 12, sweep_counts=a[3])
+    assert np.max(np.abs(b[0] - st.psi)) <= 1e-4 and rel_l2(b[0], st.psi) <= 1e-5
