@@ -143,11 +143,11 @@ def config_dict(cfg: I.Config, world: int = 1):
             "loop": "CUDA graph per step, WHILE node around the sweep, no host sync"}
 
 
-def make_solver(cfg: I.Config, host_loop=False, seed_offset=0, fp64=False, mu_iterative=False):
+def make_solver(cfg: I.Config, host_loop=False, seed_offset=0, fp64=False, mu_iterative=False, mu_direct=False):
     from paper_1409_8340_b200 import Solver
     s = Solver(cfg.nx, cfg.ny, cfg.nz, bc=cfg.bc, h=cfg.h, dt=cfg.dt, eps_tol=1e-6, max_sweeps=100,
                temperature=cfg.temperature, seed=replica_seed(cfg, seed_offset), init_amp=cfg.init_amp, solve_mu=True,
-               host_loop=host_loop, fp64=fp64, mu_iterative=mu_iterative)
+               host_loop=host_loop, fp64=fp64, mu_iterative=mu_iterative, mu_direct=mu_direct)
     s.set_pinning(I.sphere_list(cfg), cfg.eps_in, cfg.eps_out)
     bx, bz = cfg.requested_field()
     s.set_field_current(Bx=bx, Bz=bz, Jx=cfg.Jx)
@@ -256,6 +256,7 @@ def main():
     ap.add_argument("--pair-mode", type=int, default=1, help="tdgl_set_pair_mode: 1 automatic (default), 2 whenever the cap allows")
     ap.add_argument("--no-pairs", action="store_true", help="plain Jacobi sweeps only (tdgl_set_pair_mode 0): A/B against the fused two-sweep kernel")
     ap.add_argument("--fp64", action="store_true", help="the double-precision build (TDGL_FLAG_FP64; the paper's DP mode)")
+    ap.add_argument("--mu-direct", action="store_true", help="with --fp64: direct mu solver (fp32 transforms inside fp64 iterative refinement, TDGL_FLAG_MU_DIRECT)")
     ap.add_argument("--mu-iterative", action="store_true", help="the paper's own pseudo-time mu solver (TDGL_FLAG_MU_ITERATIVE)")
     ap.add_argument("--h-tau", type=float, default=0.1, help="virtual time step of the pseudo-time mu solver (S20)")
     args = ap.parse_args()
@@ -287,10 +288,11 @@ def main():
             torch.cuda.synchronize()
 
     # ---- resident run (graph mode) --------------------------------------------------------------
-    mode = dict(fp64=args.fp64, mu_iterative=args.mu_iterative)
+    mode = dict(fp64=args.fp64, mu_iterative=args.mu_iterative, mu_direct=args.mu_direct)
+    iter_mu = (args.fp64 or args.mu_iterative) and not args.mu_direct
     bytes_per_site = SWEEP_BYTES_PER_SITE * (2.0 if args.fp64 else 1.0)
     s = make_solver(cfg, seed_offset=rank, **mode)
-    if args.fp64 or args.mu_iterative:
+    if iter_mu:
         s.set_mu_solver(h_tau=args.h_tau)
     if args.no_pairs or args.pair_mode != 1:
         s.set_pair_mode(0 if args.no_pairs else args.pair_mode)
@@ -311,7 +313,10 @@ def main():
     clocks = sampler.stop()
     ob1 = s.observables()
     mu_stats = None
-    if args.fp64 or args.mu_iterative:
+    if args.mu_direct:
+        sv, ps, rl = s.mu_direct_stats()
+        mu_stats = {"refinement_passes_per_solve": ps / max(sv, 1), "last_max_residual": rl}
+    elif iter_mu:
         outer, inner = s.mu_log(min(K, 1000))
         mu_stats = {"outer_per_step": float(np.mean(outer)), "inner_per_outer": float(np.mean([np.mean(i) for i in inner if i]))}
     launches = s.launch_count() - l0 - 2           # minus the two observables kernels
@@ -334,7 +339,7 @@ def main():
         psi, mu = s.get_psi_mu()
         K0 = s.observables().K
         sh = make_solver(cfg, host_loop=True, seed_offset=rank, **mode)
-        if args.fp64 or args.mu_iterative:
+        if iter_mu:
             sh.set_mu_solver(h_tau=args.h_tau)
         sh.set_state(psi, mu, K0)
         sh.set_pair_mode(0)                          # every sweep a plain sweep: the kernel this figure is about
@@ -425,7 +430,8 @@ def main():
         "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64" if args.fp64 else "f32",
         "data": "synthetic", "steps_per_s": steps_per_s, "sweeps_per_step": sweeps_all / (K * world),
-        "config": dict(config_dict(cfg, world), **({"mu_solver": "pseudo-time iteration (Eq. 40), host-driven loop"} if (args.fp64 or args.mu_iterative) else {})),
+        "config": dict(config_dict(cfg, world), **({"mu_solver": "pseudo-time iteration (Eq. 40), host-driven loop"} if iter_mu else
+                                                   ({"mu_solver": "direct: fp32 transform solver inside fp64 iterative refinement"} if args.mu_direct else {}))),
         "mu_iteration": mu_stats,
         "clocks": clocks, "e2e": e2e, "gpu_launches": launches_all, "roofline": roof, "roofline_pair": roof_pair,
         "pairs": pairs, "cpu_baseline": cpu,

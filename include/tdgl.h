@@ -57,6 +57,10 @@ extern "C" {
                                    site ("no-current boundary conditions across internal grid edges").  Needs
                                    TDGL_FLAG_FP64 (the cut links are implemented in the precision-generic kernels; mu is
                                    then solved by the pseudo-time iteration, the transform solver does not apply). */
+#define TDGL_FLAG_MU_DIRECT 256u /* with TDGL_FLAG_FP64: solve Delta_h mu = rho DIRECTLY in double precision -- the fp32 transform
+                                   solver as an approximate inverse inside fp64 iterative refinement (residual rho - Delta_h mu
+                                   in fp64; 3-4 passes reach its rounding floor) -- instead of the paper's pseudo-time iteration.
+                                   Not with TDGL_FLAG_MU_ITERATIVE, TDGL_FLAG_MU_REFINE or TDGL_FLAG_INSULATORS. */
 #define TDGL_FLAG_HOST_LOOP 2u  /* test/diagnostic: host-driven sweep loop instead of the CUDA-graph
                                    WHILE node (identical arithmetic)                                     */
 
@@ -217,6 +221,10 @@ int64_t tdgl_launch_count(const tdgl_t *h);
  * at a time while timing is on.  The call returns the milliseconds and launches accumulated so far and, with enable > 0,
  * clears them.  Used by bench.py for the roofline figures. */
 int tdgl_sweep_timing(tdgl_t *h, int32_t enable, double *ms_total_host, int64_t *launches_host);
+
+/* TDGL_FLAG_MU_DIRECT: solves since create, refinement passes since create (each pass = one fp32 transform solve + one
+ * fp64 residual), max |rho - Delta_h mu| of the last solve. */
+int tdgl_get_mu_direct_stats(tdgl_t *h, int64_t *solves_host, int64_t *passes_host, double *resid_last_host);
 
 /* Fused sweep pairs (temporal blocking of Eq. 33; march_pair.cu).  On meshes that admit it (xz gauge, fp32, nx % 128 == 0,
  * ny % 16 == 0, ny >= 32, nz >= 4) two Jacobi sweeps run as ONE pass over HBM whenever two more sweeps are certain

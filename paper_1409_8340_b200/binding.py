@@ -13,14 +13,14 @@ _LIB_PATH = os.environ.get("TDGL_LIB") or os.path.join(_HERE, "libtdgl.so")     
 TDGL_OK, TDGL_EINVAL, TDGL_ENOMEM, TDGL_EINCOMPAT, TDGL_ECUDA, TDGL_WMAXSWEEPS = 0, -1, -2, -3, -4, 1
 TDGL_BC_PERIODIC, TDGL_BC_OPEN = 0, 1
 TDGL_FLAG_SOLVE_MU, TDGL_FLAG_HOST_LOOP, TDGL_FLAG_GAUGE_YZ, TDGL_FLAG_MU_REFINE, TDGL_FLAG_MU_NOREFINE = 1, 2, 4, 8, 16
-TDGL_FLAG_MU_ITERATIVE, TDGL_FLAG_FP64, TDGL_FLAG_INSULATORS = 32, 64, 128
+TDGL_FLAG_MU_ITERATIVE, TDGL_FLAG_FP64, TDGL_FLAG_INSULATORS, TDGL_FLAG_MU_DIRECT = 32, 64, 128, 256
 
 EXPORTS = (
     "tdgl_workspace_bytes", "tdgl_create", "tdgl_destroy", "tdgl_set_pinning", "tdgl_set_field_current", "tdgl_step",
     "tdgl_get_psi_mu", "tdgl_observables", "tdgl_strerror", "tdgl_last_cuda_error", "tdgl_set_state", "tdgl_set_solver",
     "tdgl_set_sweep_schedule", "tdgl_get_sweep_log", "tdgl_get_eps", "tdgl_debug_noise", "tdgl_debug_poisson",
     "tdgl_debug_rho", "tdgl_launch_count", "tdgl_sweep_timing", "tdgl_mu_gain", "tdgl_mu_refine_enabled",
-    "tdgl_set_mu_solver", "tdgl_get_mu_log", "tdgl_set_insulators", "tdgl_set_pinning_shapes", "tdgl_set_insulator_shapes", "tdgl_set_pair_mode", "tdgl_get_pair_stats",
+    "tdgl_set_mu_solver", "tdgl_get_mu_log", "tdgl_set_insulators", "tdgl_set_pinning_shapes", "tdgl_set_insulator_shapes", "tdgl_set_pair_mode", "tdgl_get_pair_stats", "tdgl_get_mu_direct_stats",
 )
 
 
@@ -97,6 +97,7 @@ def lib() -> C.CDLL:
     L.tdgl_set_insulators.argtypes = [vp, C.POINTER(TdglSphere), i64]
     L.tdgl_set_pinning_shapes.argtypes = [vp, vp, i64, f32, f32]
     L.tdgl_set_insulator_shapes.argtypes = [vp, vp, i64]
+    L.tdgl_get_mu_direct_stats.argtypes = [vp, C.POINTER(i64), C.POINTER(i64), C.POINTER(f64)]
     L.tdgl_set_pair_mode.argtypes = [vp, i32]
     L.tdgl_get_pair_stats.argtypes = [vp, C.POINTER(i32), C.POINTER(i64), C.POINTER(i64)]
     L.tdgl_get_mu_log.argtypes = [vp, i32, C.POINTER(i32), C.POINTER(i32), i32, C.POINTER(i32)]
@@ -177,7 +178,8 @@ class Solver:
                  u: float = 1.0, g: float = 1.0, eps_tol: float = 1e-6, max_sweeps: int = 100, fixed_sweeps: int = 0,
                  temperature: float = 0.0, seed: int = 0, init_amp: float = 0.01, solve_mu: bool = True,
                  host_loop: bool = False, hxyz: Optional[Sequence[float]] = None, device: Optional[str] = None,
-                 gauge_yz: bool = False, mu_refine: Optional[bool] = None, mu_iterative: bool = False, fp64: bool = False, insulators: bool = False):
+                 gauge_yz: bool = False, mu_refine: Optional[bool] = None, mu_iterative: bool = False, fp64: bool = False, insulators: bool = False,
+                 mu_direct: bool = False):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1409_8340_b200 needs a CUDA device (sm_100a); there is no CPU path")
@@ -196,7 +198,7 @@ class Solver:
                    | (TDGL_FLAG_GAUGE_YZ if gauge_yz else 0)
                    | (0 if mu_refine is None else (TDGL_FLAG_MU_REFINE if mu_refine else TDGL_FLAG_MU_NOREFINE))
                    | (TDGL_FLAG_MU_ITERATIVE if mu_iterative else 0) | (TDGL_FLAG_FP64 if fp64 else 0)
-                   | (TDGL_FLAG_INSULATORS if insulators else 0))
+                   | (TDGL_FLAG_INSULATORS if insulators else 0) | (TDGL_FLAG_MU_DIRECT if mu_direct else 0))
         self.fp64 = bool(fp64)
         nbytes = tdgl_workspace_bytes(p)
         if nbytes == 0:
@@ -338,6 +340,12 @@ class Solver:
 
     def launch_count(self) -> int:
         return int(lib().tdgl_launch_count(self.h))
+
+    def mu_direct_stats(self):
+        """TDGL_FLAG_MU_DIRECT: (solves, refinement passes, max |rho - Delta_h mu| of the last solve)."""
+        a, b, r = C.c_int64(), C.c_int64(), C.c_double()
+        _check(lib().tdgl_get_mu_direct_stats(self.h, C.byref(a), C.byref(b), C.byref(r)), "tdgl_get_mu_direct_stats", self.h)
+        return a.value, b.value, r.value
 
     def set_pair_mode(self, mode: int):
         """Fused sweep pairs: 0 never, 1 automatic (default), 2 whenever the cap allows (forces the redo path)."""

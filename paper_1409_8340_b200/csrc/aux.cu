@@ -29,6 +29,7 @@ __global__ void k_ctl_reset(const __grid_constant__ Dev dv, float eps_tol, int m
   c->mu_inner = 0; c->mu_inner_done = 0; c->mu_outer = 0; c->mu_done = 0; c->mu_sched_n = 0; c->mu_sched_pos = 0;
   c->mu_ticket = 0u; c->mu_r2bits = 0ull; c->mu_log_pos = 0; c->mu_solves = 0; c->mu_outer_total = 0; c->mu_inner_total = 0;
   c->mu_dt2_last = 0.0;
+  c->dref_rho_bits = 0ull; c->dref_r_bits = 0ull; c->dref_solves = 0; c->dref_passes = 0; c->dref_resid_last = 0.0;
 }
 __global__ void k_ctl_solver(const __grid_constant__ Dev dv, float eps_tol, int max_sweeps, int fixed_sweeps) {
   dv.ctl->eps_tol = eps_tol; dv.ctl->max_sweeps = max_sweeps; dv.ctl->fixed_sweeps = fixed_sweeps;

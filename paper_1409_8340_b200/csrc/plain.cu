@@ -500,6 +500,100 @@ __global__ void k_mu_controls(const __grid_constant__ Dev dv, float h_tau, float
 }
 __global__ void k_mu_sched(const __grid_constant__ Dev dv, int n) { dv.ctl->mu_sched_n = n; dv.ctl->mu_sched_pos = 0; }
 
+// ------------------------------------------------------------------------------------------------------------------
+// (1b) direct mu solver of the double-precision build (TDGL_FLAG_MU_DIRECT).  Delta_h mu = rho (the
+// fixed point of the paper's iteration) by mixed-precision iterative refinement: the fp32 transform solver S (poisson.cu)
+// is an approximate inverse with relative error ~1e-6 G (G = white-noise gain, refine.cu), so
+//     mu_0 = 0, r_0 = rho;   mu_{n+1} = mu_n + S(float(r_n)),   r_{n+1} = rho - Delta_h mu_{n+1}  (fp64)
+// gains six to seven digits per pass and reaches the fp64 rounding floor of the residual in 3-4 passes.
+// ------------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_dref_begin(const __grid_constant__ Dev dv) {
+  const double *__restrict__ rho = (const double *)dv.mu_rho;
+  double mx = 0.0;
+  for (long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x; m < dv.N; m += (long long)gridDim.x * blockDim.x) {
+    const double r = rho[m];
+    dv.resid[m] = (float)r;
+    dv.mu64[m] = 0.0;
+    mx = fmax(mx, fabs(r));
+  }
+  __shared__ double sh[8];
+  const double bm = block_max(mx, sh);
+  if (threadIdx.x == 0) atomicMax(&dv.ctl->dref_rho_bits, (unsigned long long)__double_as_longlong(bm));
+}
+// mu += S(r) (the solver worked in place on resid), then nothing else: the residual needs the updated neighbours
+__global__ void __launch_bounds__(256) k_dref_add(const __grid_constant__ Dev dv) {
+  for (long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x; m < dv.N; m += (long long)gridDim.x * blockDim.x)
+    dv.mu64[m] += (double)dv.resid[m];
+}
+// r = rho - Delta_h mu in fp64 (wrap / mirror ghost, S6), stored in fp32 for the next pass; max |r|
+__global__ void __launch_bounds__(128) k_dref_resid(const __grid_constant__ Dev dv) {
+  const double *__restrict__ rho = (const double *)dv.mu_rho;
+  const Chunk ch = chunk_of(dv);
+  const int i = ch.i;
+  double mx = 0.0;
+  if (i < dv.nx)
+  for (int k = ch.k0; k < ch.k1; ++k)
+  for (int j = ch.j0; j < ch.j1; ++j) {
+    const Site s = site_of(dv, i, j, k);
+    const long long m = (long long)i + (long long)dv.nx * (j + (long long)dv.ny * k);
+    double ctr;
+    const double ns = real_nsum(dv, dv.mu64, s, ctr, 63u);
+    const double r = rho[m] - (ns - link_diag(dv, 63u) * ctr);
+    dv.resid[m] = (float)r;
+    mx = fmax(mx, fabs(r));
+  }
+  __shared__ double sh[4];
+  const double bm = block_max(mx, sh);
+  if (threadIdx.x == 0) atomicMax(&dv.ctl->dref_r_bits, (unsigned long long)__double_as_longlong(bm));
+}
+// S7: the solution is fixed by sum_m w_m mu_m = 0 (w = 1/2 per open face).  Every fp32 solve removes its own weighted mean
+// only to fp32 accuracy and Delta_h cannot see a constant, so the accumulated mu carries an offset of ~1e-9: removed
+// here in fp64.  Partial sums per CTA in a fixed grid, summed in a fixed order by every CTA of the second kernel.
+#define DREF_NB 1024
+__global__ void __launch_bounds__(256) k_dref_wsum(const __grid_constant__ Dev dv) {
+  const int nx = dv.nx, ny = dv.ny, nz = dv.nz;
+  double acc = 0.0;
+  for (long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x; m < dv.N; m += (long long)gridDim.x * blockDim.x) {
+    const int i = (int)(m % nx);
+    const long long rest = m / nx;
+    const int j = (int)(rest % ny), k = (int)(rest / ny);
+    double w = 1.0;
+    if (dv.bcx && (i == 0 || i == nx - 1)) w *= 0.5;
+    if (dv.bcy && (j == 0 || j == ny - 1)) w *= 0.5;
+    if (nz > 1 && dv.bcz && (k == 0 || k == nz - 1)) w *= 0.5;
+    acc += w * dv.mu64[m];
+  }
+  __shared__ double sh[8];
+  for (int o = 16; o > 0; o >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, o);
+  if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = acc;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double t = 0.0;
+    for (int q = 0; q < 8; ++q) t += sh[q];
+    dv.part[blockIdx.x] = t;
+  }
+}
+__global__ void __launch_bounds__(256) k_dref_shift(const __grid_constant__ Dev dv) {
+  __shared__ double mean;
+  if (threadIdx.x == 0) {
+    double t = 0.0;
+    for (int q = 0; q < DREF_NB; ++q) t += dv.part[q];
+    const double wsum = (double)(dv.nx - (dv.bcx ? 1 : 0)) * (double)(dv.ny - (dv.bcy ? 1 : 0)) *
+                        (double)(dv.nz > 1 ? dv.nz - (dv.bcz ? 1 : 0) : 1);
+    mean = t / wsum;
+  }
+  __syncthreads();
+  const double mu0 = mean;
+  for (long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x; m < dv.N; m += (long long)gridDim.x * blockDim.x)
+    dv.mu64[m] -= mu0;
+}
+__global__ void k_dref_ctl(const __grid_constant__ Dev dv, int what) {
+  Ctl *c = dv.ctl;
+  if (what == 0) { c->dref_rho_bits = 0ull; c->dref_r_bits = 0ull; }           // start of a solve
+  else if (what == 1) c->dref_r_bits = 0ull;                                    // before a residual pass
+  else { c->dref_solves += 1; c->dref_resid_last = __longlong_as_double((long long)c->dref_r_bits); }   // end of a solve
+}
+
 // zero psi and mu on the removed sites (after tdgl_set_insulators / tdgl_set_state)
 __global__ void k_apply_mask64(const __grid_constant__ Dev dv) {
   double2 *x = dv.psi64[dv.ctl->xbuf & 1];
@@ -573,3 +667,12 @@ void launch_mu_controls(const Dev &dv, float h_tau, float eps_mu, float eps_in, 
   k_mu_controls<<<1, 1, 0, st>>>(dv, h_tau, eps_mu, eps_in, max_outer, max_inner);
 }
 void launch_mu_sched(const Dev &dv, int n, cudaStream_t st) { k_mu_sched<<<1, 1, 0, st>>>(dv, n); }
+
+void launch_dref_ctl(const Dev &dv, int what, cudaStream_t st) { k_dref_ctl<<<1, 1, 0, st>>>(dv, what); }
+void launch_dref_begin(const Dev &dv, cudaStream_t st) { k_dref_begin<<<148 * 8, 256, 0, st>>>(dv); }
+void launch_dref_add(const Dev &dv, cudaStream_t st) { k_dref_add<<<148 * 8, 256, 0, st>>>(dv); }
+void launch_dref_resid(const Dev &dv, cudaStream_t st) { k_dref_resid<<<grid3(dv), 128, 0, st>>>(dv); }
+void launch_dref_zero_mean(const Dev &dv, cudaStream_t st) {
+  k_dref_wsum<<<DREF_NB, 256, 0, st>>>(dv);
+  k_dref_shift<<<148 * 8, 256, 0, st>>>(dv);
+}

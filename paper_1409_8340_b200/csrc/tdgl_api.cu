@@ -56,6 +56,11 @@ void launch_mu_sweep(const Dev &dv, void *mu, cudaStream_t st);
 void launch_mu_finish(const Dev &dv, void *mu, cudaStream_t st);
 void launch_mu_controls(const Dev &dv, float h_tau, float eps_mu, float eps_in, int max_outer, int max_inner, cudaStream_t st);
 void launch_mu_sched(const Dev &dv, int n, cudaStream_t st);
+void launch_dref_ctl(const Dev &dv, int what, cudaStream_t st);
+void launch_dref_begin(const Dev &dv, cudaStream_t st);
+void launch_dref_add(const Dev &dv, cudaStream_t st);
+void launch_dref_resid(const Dev &dv, cudaStream_t st);
+void launch_dref_zero_mean(const Dev &dv, cudaStream_t st);
 void launch_spheres_mask(const Dev &dv, const float4 *sph, long long n, unsigned char *mask, cudaStream_t st);
 void launch_shapes(const Dev &dv, const float *shp, long long n, float eps_in, unsigned char *mask, cudaStream_t st);
 void launch_apply_mask64(const Dev &dv, cudaStream_t st);
@@ -90,6 +95,7 @@ struct tdgl {
   int *h_flag;                 // pinned: [0] done, [1] sweeps
   int pred_units;              // predicted iterations of the sweep loop (host loop: enqueued before the first flag read)
   int pred_mu_inner;           // pseudo-time mu iteration: predicted Jacobi sweeps per outer iteration
+  int64_t dref_passes;         // TDGL_FLAG_MU_DIRECT: refinement passes since create
   // sweep timing
   int timing;                  // 0 off, 1 plain sweeps, 2 fused pairs
   double t_ms;
@@ -148,6 +154,8 @@ static bool params_ok(const tdgl_params *p) {
   if ((p->flags & TDGL_FLAG_GAUGE_YZ) && p->nz == 1) return false;          // films use the xz gauge
   if ((p->flags & TDGL_FLAG_MU_REFINE) && (p->flags & (TDGL_FLAG_MU_ITERATIVE | TDGL_FLAG_FP64))) return false;
   if ((p->flags & TDGL_FLAG_INSULATORS) && !(p->flags & TDGL_FLAG_FP64)) return false;   // cut links: plain kernels only
+  if ((p->flags & TDGL_FLAG_MU_DIRECT) && (!(p->flags & TDGL_FLAG_FP64) || (p->flags & (TDGL_FLAG_MU_ITERATIVE | TDGL_FLAG_MU_REFINE |
+                                                                                      TDGL_FLAG_INSULATORS)))) return false;
   return true;
 }
 
@@ -184,8 +192,9 @@ static double mu_gain(const tdgl_params *p) {
 // automatic for meshes whose gain exceeds TDGL_MU_REFINE_GAIN (quasi-1D / thin long films; never the 3D BASELINE grids)
 static bool is_fp64(const tdgl_params *p) { return (p->flags & TDGL_FLAG_FP64) != 0; }
 // the pseudo-time iteration is the mu solver of the double-precision build (the direct solver is fp32 only)
+static bool is_mu_direct64(const tdgl_params *p) { return is_fp64(p) && (p->flags & TDGL_FLAG_SOLVE_MU) && (p->flags & TDGL_FLAG_MU_DIRECT); }
 static bool is_mu_iterative(const tdgl_params *p) {
-  return (p->flags & TDGL_FLAG_SOLVE_MU) && (p->flags & (TDGL_FLAG_MU_ITERATIVE | TDGL_FLAG_FP64));
+  return (p->flags & TDGL_FLAG_SOLVE_MU) && (p->flags & (TDGL_FLAG_MU_ITERATIVE | TDGL_FLAG_FP64)) && !is_mu_direct64(p);
 }
 static bool want_refine(const tdgl_params *p) {
   if (!(p->flags & TDGL_FLAG_SOLVE_MU) || (p->flags & TDGL_FLAG_MU_NOREFINE) || is_mu_iterative(p)) return false;
@@ -268,6 +277,10 @@ static size_t carve(const tdgl_params *p, char *base, Dev *dv) {
     q = take(N * es); if (dv) dv->mu_xb = q;
     if (dv) dv->mu_iterative = 1;
   }
+  if (is_mu_direct64(p)) {                     // rho in double, the residual / correction the fp32 solver works on
+    q = take(N * sizeof(double)); if (dv) dv->mu_rho = q;
+    q = take(N * sizeof(float)); if (dv) { dv->resid = (float *)q; dv->mu_direct64 = 1; }
+  }
   if (dv) dv->fp64 = f64 ? 1 : 0;
   return off;
 }
@@ -330,6 +343,35 @@ static int mu_iterative_solve(tdgl_t *h, void *mu) {
   return n;
 }
 
+// Direct mu solve of the double-precision build (TDGL_FLAG_MU_DIRECT; plain.cu (1b)): fp32 transform solves inside fp64
+// iterative refinement, host-driven: one 16-byte read per pass (max |rho|, max |r|).  Stops at max |r| <= 2e-15 max(1, max |rho|),
+// when a pass no longer halves the residual (its fp64 rounding floor), or after 8 passes.  rho is in dv.mu_rho.
+static int mu_direct64_solve(tdgl_t *h, const Dev &dv) {
+  cudaStream_t st = h->stream;
+  int n = 0;
+  launch_dref_ctl(dv, 0, st); ++n;
+  launch_dref_begin(dv, st); ++n;
+  double prev = -1.0;
+  for (int pass = 0; pass < 8; ++pass) {
+    n += poisson_solve(h->dvp, dv.resid, true, st);
+    launch_dref_add(dv, st); ++n;
+    launch_dref_ctl(dv, 1, st); ++n;
+    launch_dref_resid(dv, st); ++n;
+    unsigned long long bits[2];
+    if (cudaMemcpyAsync(bits, &dv.ctl->dref_rho_bits, sizeof(bits), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+        cudaStreamSynchronize(st) != cudaSuccess) return -1;
+    double rho_max, r_max;
+    memcpy(&rho_max, &bits[0], 8); memcpy(&r_max, &bits[1], 8);
+    h->dref_passes += 1;
+    if (r_max <= 2e-15 * (rho_max > 1.0 ? rho_max : 1.0)) break;
+    if (prev >= 0.0 && r_max > 0.5 * prev) break;
+    prev = r_max;
+  }
+  launch_dref_zero_mean(dv, st); n += 2;            // S7 in fp64 (the fp32 solves leave an offset of ~1e-9)
+  launch_dref_ctl(dv, 2, st); ++n;
+  return n;
+}
+
 // the kernels of one step after the psi solve: J_av + K (a5), rho (a6), mu (a7)
 static int enqueue_after_solve(tdgl_t *h, cudaStream_t st) {
   int n = 0;
@@ -346,7 +388,14 @@ static int enqueue_after_solve(tdgl_t *h, cudaStream_t st) {
     if (kact) { launch_jav_edges(h->dv, march_tma_tile_w(), h->jav_blocks, st); ++n; }
     launch_step_finish(h->dv, (int)(h->mgrid.x * h->mgrid.y * h->mgrid.z), h->jav_blocks, st); ++n;
   }
-  if (h->dv.solve_mu && h->dv.mu_iterative) {
+  if (h->dv.solve_mu && h->dv.mu_direct64) {
+    Dev d2 = h->dv;                               // the rho kernel writes where "mu" points: into the rho array
+    d2.mu64 = (double *)h->dv.mu_rho;
+    march(h, MODE_RHO, d2, st); ++n;
+    const int m = mu_direct64_solve(h, h->dv);
+    if (m < 0) return -1;
+    n += m;
+  } else if (h->dv.solve_mu && h->dv.mu_iterative) {
     Dev d2 = h->dv;                               // the rho kernel writes where "mu" points: into the iteration's rho array
     d2.mu = (float *)h->dv.mu_rho; d2.mu64 = (double *)h->dv.mu_rho;
     march(h, MODE_RHO, d2, st); ++n;
@@ -897,6 +946,16 @@ extern "C" int tdgl_debug_noise(tdgl_t *h, int64_t step, void *zeta_dev) {
 
 extern "C" int tdgl_debug_poisson(tdgl_t *h, const void *rho_dev, void *mu_dev) {
   if (!h || !rho_dev || !mu_dev) return TDGL_EINVAL;
+  if (h->dv.mu_direct64) {                        // rho, mu: N doubles; the state's own mu is left alone
+    CK(cudaMemcpyAsync(h->dv.mu_rho, rho_dev, (size_t)h->dv.N * sizeof(double), cudaMemcpyDeviceToDevice, h->stream));
+    Dev d2 = h->dv;
+    d2.mu64 = (double *)mu_dev;
+    const int m = mu_direct64_solve(h, d2);
+    if (m < 0) return cuda_fail(h, cudaGetLastError());
+    h->launches += m;
+    CKL();
+    return TDGL_OK;
+  }
   if (h->dv.mu_iterative) {                       // the pseudo-time iteration from mu = 0 on the given rho
     const size_t es = h->dv.fp64 ? sizeof(double) : sizeof(float);
     CK(cudaMemcpyAsync(h->dv.mu_rho, rho_dev, (size_t)h->dv.N * es, cudaMemcpyDeviceToDevice, h->stream));
@@ -944,6 +1003,19 @@ extern "C" int64_t tdgl_launch_count(const tdgl_t *h) {
     n += h->graph_steps * (int64_t)h->fixed_per_step + body;
   }
   return n;
+}
+
+extern "C" int tdgl_get_mu_direct_stats(tdgl_t *h, int64_t *solves, int64_t *passes, double *resid_last) {
+  if (!h) return TDGL_EINVAL;
+  if (!h->dv.mu_direct64) return TDGL_EINVAL;
+  long long sv = 0; double rl = 0.0;
+  CK(cudaMemcpyAsync(&sv, &h->dv.ctl->dref_solves, sizeof(sv), cudaMemcpyDeviceToHost, h->stream));
+  CK(cudaMemcpyAsync(&rl, &h->dv.ctl->dref_resid_last, sizeof(rl), cudaMemcpyDeviceToHost, h->stream));
+  CK(cudaStreamSynchronize(h->stream));
+  if (solves) *solves = sv;
+  if (passes) *passes = h->dref_passes;
+  if (resid_last) *resid_last = rl;
+  return TDGL_OK;
 }
 
 extern "C" int tdgl_set_pair_mode(tdgl_t *h, int32_t mode) {

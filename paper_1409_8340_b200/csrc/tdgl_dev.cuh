@@ -52,6 +52,10 @@ struct Ctl {
   unsigned long long mu_r2bits;
   long long mu_log_pos, mu_solves, mu_outer_total, mu_inner_total;
   double mu_dt2_last;
+  // direct mu solver of the double-precision build (TDGL_FLAG_MU_DIRECT: fp32 transform solver + fp64 iterative refinement)
+  unsigned long long dref_rho_bits, dref_r_bits;   // max |rho|, max |rho - Delta_h mu| as fp64 bit patterns
+  long long dref_solves, dref_passes;
+  double dref_resid_last;
 };
 
 struct Dev {
@@ -103,6 +107,7 @@ struct Dev {
   int mu_iterative;
   void *mu_rho, *mu_c, *mu_xa, *mu_xb;
   int *mu_log, *mu_outer_log, *mu_sched;
+  int mu_direct64;          // TDGL_FLAG_MU_DIRECT: rho in mu_rho (double), residual / correction in resid (float)
   int pair_ok;              // the mesh admits the fused two-sweep kernel (march_pair.cu)
   unsigned long long cond_handle;   // cudaGraphConditionalHandle of the WHILE node (graph mode)
   int use_cond;

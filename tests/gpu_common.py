@@ -14,21 +14,22 @@ def f32(x: float) -> float:
 
 
 def oracle_params(cfg: I.Config, eps_tol=1e-6, max_sweeps=100, solve_mu=True, temperature=None, hxyz=None, g=1.0, u=1.0,
-                  mu_iterative=False, fp64=False):
+                  mu_iterative=False, fp64=False, mu_direct=False):
     hx, hy, hz = hxyz if hxyz is not None else (cfg.h, cfg.h, cfg.h)
     return O.Params(cfg.nx, cfg.ny, cfg.nz, hx=f32(hx), hy=f32(hy), hz=f32(hz), dt=f32(cfg.dt), u=f32(u), g=f32(g),
                     bc=tuple(cfg.bc), eps_tol=f32(eps_tol), max_sweeps=max_sweeps,
                     temperature=f32(cfg.temperature if temperature is None else temperature), seed=cfg.seed,
-                    solve_mu=solve_mu, mu_solver="pseudotime" if (mu_iterative or fp64) else "direct",
+                    solve_mu=solve_mu, mu_solver="pseudotime" if ((mu_iterative or fp64) and not mu_direct) else "direct",
                     h_tau=f32(0.1), eps_mu=f32(1e-6), eps_mu_in=f32(1e-6))
 
 
 def make_solver(cfg: I.Config, eps_tol=1e-6, max_sweeps=100, solve_mu=True, temperature=None, host_loop=False,
-                fixed_sweeps=0, hxyz=None, g=1.0, u=1.0, mu_refine=None, mu_iterative=False, fp64=False):
+                fixed_sweeps=0, hxyz=None, g=1.0, u=1.0, mu_refine=None, mu_iterative=False, fp64=False, mu_direct=False):
     from paper_1409_8340_b200 import Solver
     return Solver(cfg.nx, cfg.ny, cfg.nz, bc=cfg.bc, h=cfg.h, dt=cfg.dt, g=g, u=u, eps_tol=eps_tol, max_sweeps=max_sweeps,
                   fixed_sweeps=fixed_sweeps, temperature=cfg.temperature if temperature is None else temperature,
-                  seed=cfg.seed, init_amp=cfg.init_amp, solve_mu=solve_mu, host_loop=host_loop, hxyz=hxyz, mu_refine=mu_refine, mu_iterative=mu_iterative, fp64=fp64)
+                  seed=cfg.seed, init_amp=cfg.init_amp, solve_mu=solve_mu, host_loop=host_loop, hxyz=hxyz, mu_refine=mu_refine, mu_iterative=mu_iterative, fp64=fp64,
+                  mu_direct=mu_direct)
 
 
 def setup_pair(cfg: I.Config, psi0=None, mu0=None, K0=0.0, with_pinning=True, **kw):

@@ -337,3 +337,87 @@ def test_insulators_need_the_flag():
     s.close()
     with pytest.raises(TdglError):
         Solver(16, 8, 4, insulators=True)                          # fp32 path has no cut links
+
+
+# ---------------------------------------------------------------------------------------------------
+# the direct mu solver of the double-precision build (TDGL_FLAG_MU_DIRECT): fp32 transform solver inside fp64
+# iterative refinement.  The oracle side is the DEFINITION Delta_h mu = rho solved in fp64 (O.solve_poisson).
+# ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("bc,shape", [((P_, P_, P_), (64, 32, 16)), ((P_, P_, O_), (128, 40, 9)), ((O_, O_, O_), (34, 13, 11)),
+                                      ((P_, O_, P_), (64, 20, 12)), ((O_, P_, O_), (1024, 6, 5)), ((P_, P_, P_), (256, 96, 1)),
+                                      ((O_, O_, P_), (130, 37, 1))])
+def test_fp64_direct_poisson(bc, shape):
+    nx, ny, nz = shape
+    cfg = cfg_of(nx, ny, nz, bc)
+    p = oracle_params(cfg, fp64=True, mu_direct=True)
+    s = make_solver(cfg, fp64=True, mu_direct=True)
+    rng = np.random.default_rng(8)
+    w = O.site_weights(p)
+    rho = rng.standard_normal(p.shape)
+    rho -= np.sum(w * rho) / np.sum(w)                       # solvable right side (S6)
+    mu = s.debug_poisson(torch.from_numpy(rho)).cpu().numpy()
+    ref = O.solve_poisson(p, rho)
+    scale = np.max(np.abs(ref))
+    assert mu.dtype == np.float64
+    assert np.max(np.abs(mu - ref)) < 1e-11 * scale
+    assert np.max(np.abs(O.laplacian_real(p, mu) - rho)) < 1e-11 * max(1.0, np.max(np.abs(rho)))
+    solves, passes, resid = s.mu_direct_stats()
+    # the residual bottoms out at the fp64 rounding of Delta_h mu itself: ~ 6 terms of size 4 |mu| each
+    assert solves == 1 and 2 <= passes <= 8 and resid < 1e-14 * max(1.0, 24.0 * scale)
+    s.close()
+
+
+@pytest.mark.parametrize("bc", ALL_BC)
+def test_fp64_direct_two_steps(bc):
+    cfg = cfg_of(36, 14, 10, bc, Bx=0.05, Bz=0.3, Jx=0.02 if bc[0] == P_ else 0.0, temperature=1e-3, incl_fraction=0.15,
+                 incl_rmin=1.0, incl_rmax=2.0, seed=2)
+    psi0, mu0 = I.random_state(cfg, seed=21, amp=0.8)
+    K0 = 0.11 if bc[0] == P_ else 0.0
+    p, st, eps, (Bx, Bz), s = setup_pair(cfg, psi0=psi0, mu0=mu0, K0=K0, fixed_sweeps=5, fp64=True, mu_direct=True)
+    assert p.mu_solver == "direct"
+    s.step(2)
+    psi, mu = s.get_psi_mu()
+    for _ in range(2):
+        O.step(p, st, eps, Bx, Bz, f32(cfg.Jx), fixed_sweeps=5)
+    ob = s.observables()
+    assert np.max(np.abs(psi.cpu().numpy() - st.psi)) < 1e-12
+    assert np.max(np.abs(mu.cpu().numpy() - st.mu)) < 1e-11 * max(1.0, np.max(np.abs(st.mu)))
+    assert abs(ob.K - st.K) < 1e-13 and abs(ob.Jav - st.Jav) < 1e-13
+    s.close()
+
+
+def test_fp64_direct_film_and_C1_run():
+    cfg = cfg_of(132, 22, 1, (P_, P_, P_), Bz=0.3, Jx=0.02, temperature=1e-3, incl_fraction=0.15, incl_rmin=1.0, incl_rmax=2.0, seed=3)
+    psi0, mu0 = I.random_state(cfg, seed=7, amp=0.8)
+    p, st, eps, (Bx, Bz), s = setup_pair(cfg, psi0=psi0, mu0=mu0, K0=0.2, fixed_sweeps=4, fp64=True, mu_direct=True)
+    s.step(3)
+    psi, mu = s.get_psi_mu()
+    for _ in range(3):
+        O.step(p, st, eps, Bx, Bz, f32(cfg.Jx), fixed_sweeps=4)
+    assert np.max(np.abs(psi.cpu().numpy() - st.psi)) < 1e-12
+    assert np.max(np.abs(mu.cpu().numpy() - st.mu)) < 1e-10 * max(1.0, np.max(np.abs(st.mu)))
+    s.close()
+    # BASELINE.json configs[0], 100 steps, both sides taking their own decisions
+    cfg = I.CONFIGS["C1"]
+    p, st, eps, (Bx, Bz), s = setup_pair(cfg, fp64=True, mu_direct=True)
+    s.step(100)
+    psi, mu = s.get_psi_mu()
+    counts, _ = s.sweep_log(100)
+    O.run(p, st, eps, Bx, Bz, 0.0, 100)
+    assert list(counts) == st.sweep_log
+    psi = psi.cpu().numpy()
+    # C1 spends its last ~65 steps in the single-sweep regime, which amplifies the checkerboard band by 1.186 per step (reading R3):
+    # fp64 rounding differences of 1e-16 (another summation order in mu) arrive at ~1e-10; measured 1.5e-10
+    assert np.max(np.abs(psi - st.psi)) <= 1e-9 and rel_l2(psi, st.psi) <= 1e-10
+    assert np.max(np.abs(mu.cpu().numpy() - st.mu)) <= 1e-10
+    solves, passes, _ = s.mu_direct_stats()
+    assert solves == 100 and passes <= 6 * solves
+    s.close()
+
+
+def test_mu_direct_flag_validation():
+    from paper_1409_8340_b200 import Solver
+    from paper_1409_8340_b200.binding import TdglError
+    for kw in (dict(mu_direct=True), dict(mu_direct=True, fp64=True, mu_iterative=True), dict(mu_direct=True, fp64=True, insulators=True)):
+        with pytest.raises(TdglError):
+            Solver(16, 8, 4, **kw)
