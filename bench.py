@@ -46,11 +46,11 @@ def measured_peak():
         return 6650.0, "fallback (B200_PROFILING.md)"
 
 
-def ncu_traffic():
-    """Per-launch DRAM bytes of the sweep kernel from the committed ncu capture (profiles/sweep_traffic.txt)."""
+def ncu_traffic(name="sweep_traffic.txt"):
+    """Per-launch DRAM bytes of a sweep kernel from the committed ncu capture (profiles/sweep_traffic.txt, pair_traffic.txt)."""
     try:
         d = {}
-        with open(os.path.join(ROOT, "profiles", "sweep_traffic.txt")) as f:
+        with open(os.path.join(ROOT, "profiles", name)) as f:
             for line in f:
                 if line.startswith("#") or not line.strip():
                     continue
@@ -364,6 +364,9 @@ def main():
                              "achieved": 2.0 * bytes_per_site * N / (avg_p * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
                              "frac": 2.0 * bytes_per_site * N / (avg_p * 1e-3) / 1e9 / peak,
                              "min_traffic_bytes_per_launch": bytes_per_site * N,
+                             "traffic": (ncu_traffic("pair_traffic.txt") or {}).get("dram_bytes_per_launch")
+                             if (ncu_traffic("pair_traffic.txt") or {}).get("sites") == N else None,
+                             "traffic_source": "profiles/pair_traffic.txt (one committed ncu --set full capture; not measured in this run)",
                              "frac_of_min_traffic": bytes_per_site * N / (avg_p * 1e-3) / 1e9 / peak,
                              "note": "`achieved` uses SURVEY 8(d)'s definition, 32 B/site/sweep x 2 sweeps per launch: a value "
                                      "above the peak is the point of temporal blocking (x^{l+1} never goes to HBM, b and d are "
