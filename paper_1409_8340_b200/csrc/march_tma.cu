@@ -31,12 +31,14 @@ constexpr unsigned OFF_XW = 10240;      // ghost column pair (i0-2, i0-1): TH x 
 constexpr unsigned OFF_XE = 10368;      // ghost column pair (i0+nv, i0+nv+1)
 constexpr unsigned OFF_B = 10496;       // b tile (sweep only)
 constexpr unsigned OFF_D = 18688;       // d tile (sweep only)
-constexpr unsigned STAGE_PSI = 10496, STAGE_SWEEP = 26880;
+constexpr unsigned OFF_MU = 10496;      // mu tile (init only, when the row pitch 4 nx is a multiple of 16 B): TH rows x 4 min(TW, nx) bytes
+constexpr unsigned OFF_EPS = 14592;     // eps tile (init only)
+constexpr unsigned STAGE_PSI = 10496, STAGE_INIT = 18688, STAGE_SWEEP = 26880;
 constexpr unsigned HDR = 256;           // mbarriers (8 B each) at 0, the CTA residual word at 64, 8 J_av warp sums at 128
 
 template <int MODE> struct Cfg {
   static constexpr int NS = (MODE == MODE_SWEEP) ? 4 : 6;                       // stages in the ring
-  static constexpr unsigned SB = (MODE == MODE_SWEEP) ? STAGE_SWEEP : STAGE_PSI; // bytes per stage
+  static constexpr unsigned SB = (MODE == MODE_SWEEP) ? STAGE_SWEEP : (MODE == MODE_INIT ? STAGE_INIT : STAGE_PSI); // bytes per stage
   static constexpr unsigned SMEM = HDR + NS * SB;
 };
 
@@ -109,6 +111,8 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_march_tma(const __grid_constant
   const int xE = 2 * ((i0 + nv < nx) ? i0 + nv : 0);
   const unsigned tx_psi = pitch * bh + 2u * pitch + 2u * 16u * bh;
   const unsigned tx_bd = 2u * pitch * bh;
+  const bool me_tma = (MODE == MODE_INIT) && mm.me_tma;             // mu, eps through the stage (else plain loads)
+  const unsigned tx_me = (pitch / 2u) * bh * (dv.solve_mu ? 2u : 1u);
   const CUtensorMap *mC = &mm.psiC[xb], *mR = &mm.psiR[xb], *mX = &mm.psiX[xb];
   // stage t holds psi plane k0 + t (the "k+1" plane of iteration k = k0 + t - 1) and b, d of plane k0 + t - 1
   auto issue = [&](int t) {
@@ -116,7 +120,8 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_march_tma(const __grid_constant
     const unsigned sb = stage0 + slot * SB, bar = sbase + 8u * slot;
     const int kz = zwrap(k0 + t);
     const bool bd = (MODE == MODE_SWEEP) && t >= 1;
-    mbar_expect_tx(bar, tx_psi + (bd ? tx_bd : 0u));
+    const bool me = (MODE == MODE_INIT) && me_tma && t >= 1;          // mu, eps of plane k0 + t - 1
+    mbar_expect_tx(bar, tx_psi + (bd ? tx_bd : 0u) + (me ? tx_me : 0u));
     tma_load_3d(sb + OFF_C, mC, cx0, j0, kz, bar);
     tma_load_3d(sb + OFF_RLO, mR, cx0, yLo, kz, bar);
     tma_load_3d(sb + OFF_RHI, mR, cx0, yHi, kz, bar);
@@ -125,6 +130,10 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_march_tma(const __grid_constant
     if (bd) {
       tma_load_3d(sb + OFF_B, &mm.bC, cx0, j0, k0 + t - 1, bar);
       tma_load_3d(sb + OFF_D, &mm.dC, cx0, j0, k0 + t - 1, bar);
+    }
+    if (me) {
+      if (dv.solve_mu) tma_load_3d(sb + OFF_MU, &mm.muC, i0, j0, k0 + t - 1, bar);
+      tma_load_3d(sb + OFF_EPS, &mm.epsC, i0, j0, k0 + t - 1, bar);
     }
   };
 
@@ -212,8 +221,8 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_march_tma(const __grid_constant
   rA[1] = lds128(stage0 + oA);
   rB[1] = lds128(stage0 + oB);
 
-  // INIT: mu and eps of plane k, prefetched one plane ahead with plain loads (4 B/site arrays whose row
-  // stride need not be a multiple of 16 B, which rules out TMA)
+  // INIT: mu and eps of plane k arrive with the stage when nx % 4 == 0 (me_tma); otherwise their row stride is not a
+  // multiple of 16 B, which rules out TMA, and they are prefetched one plane ahead with plain loads
   float2 muA = make_float2(0.f, 0.f), muB = muA, epA = make_float2(1.f, 1.f), epB = epA;
   auto load_mu_eps = [&](long long ix, float2 &ma, float2 &mb, float2 &ea, float2 &eb) {
     if (MODE == MODE_INIT) {
@@ -227,7 +236,8 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_march_tma(const __grid_constant
       }
     }
   };
-  load_mu_eps(idx, muA, muB, epA, epB);
+  if (!me_tma) load_mu_eps(idx, muA, muB, epA, epB);
+  const unsigned oME = (unsigned)row * (pitch / 2u) + 8u * lane;   // this thread's pair A in a mu / eps tile (pair B: + 256)
 
   // one plane: Bv, Cv = this thread's values of planes k-1, k; Tv receives plane k+1
   auto do_plane = [&](int t, float4 &BvA, float4 &BvB, float4 &CvA, float4 &CvB, float4 &TvA, float4 &TvB) {
@@ -250,7 +260,10 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_march_tma(const __grid_constant
     float2 nmuA, nmuB, nepA, nepB;
     if (MODE == MODE_INIT) {
       nmuA = muA; nmuB = muB; nepA = epA; nepB = epB;
-      if (t < nk) load_mu_eps(idx + plane, nmuA, nmuB, nepA, nepB);
+      if (me_tma) {                                    // mu, eps of THIS plane arrived with the stage
+        if (dv.solve_mu) { muA = lds64(cur + OFF_MU + oME); muB = lds64(cur + OFF_MU + oME + 256u); }
+        epA = lds64(cur + OFF_EPS + oME); epB = lds64(cur + OFF_EPS + oME + 256u);
+      } else if (t < nk) load_mu_eps(idx + plane, nmuA, nmuB, nepA, nepB);
     }
     float2 WA, EA, WB, EB;
     WA.x = __shfl_up_sync(0xffffffffu, CvA.z, 1);   WA.y = __shfl_up_sync(0xffffffffu, CvA.w, 1);
@@ -356,7 +369,7 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_march_tma(const __grid_constant
         };
         init_pair(CvA, muA, epA, idx, actA, sA0, sA1, nA0, nA1, dA);
         init_pair(CvB, muB, epB, idx + 64, actB, sB0, sB1, nB0, nB1, dB);
-        muA = nmuA; muB = nmuB; epA = nepA; epB = nepB;
+        if (!me_tma) { muA = nmuA; muB = nmuB; epA = nepA; epB = nepB; }
       }
       float rloc = 0.f;
       const float4 outA = divide_pair(nA0, nA1, dA, CvA, rloc);
@@ -456,6 +469,20 @@ int march_tma_build_maps(const Dev &dv, MarchMaps *mm) {
   }
   if (!rc) rc = mk(&mm->bC, dv.b, boxC);
   if (!rc) rc = mk(&mm->dC, dv.d, boxC);
+  mm->me_tma = 0;
+  if (!rc && dv.nx % 4 == 0) {                                      // row pitch of a 4-byte field: a multiple of 16 B
+    const cuuint64_t gdim1[3] = {(cuuint64_t)dv.nx, (cuuint64_t)dv.ny, (cuuint64_t)dv.nz};
+    const cuuint64_t gstr1[2] = {4ull * dv.nx, 4ull * dv.nx * dv.ny};
+    const cuuint32_t box1[3] = {(cuuint32_t)(dv.nx < TW ? dv.nx : TW), bh, 1};
+    auto mk1 = [&](CUtensorMap *m, void *base) -> int {
+      const CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, base, gdim1, gstr1, box1, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                             CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+      return r == CUDA_SUCCESS ? 0 : -(int)r;
+    };
+    rc = mk1(&mm->muC, dv.mu);
+    if (!rc) rc = mk1(&mm->epsC, dv.eps);
+    if (!rc) mm->me_tma = 1;
+  }
   return rc;
 }
 

@@ -9,6 +9,8 @@
 struct MarchMaps {
   CUtensorMap psiC[2], psiR[2], psiX[2];   // the two ping-pong psi buffers
   CUtensorMap bC, dC;                       // right side b and diagonal d of the linear system (Eq. 30-31)
+  CUtensorMap muC, epsC;                    // mu and eps as fp32 [nz][ny][nx], box 128 x 8 x 1 (init kernel; only if nx % 4 == 0)
+  int me_tma;                               // 1: the init kernel takes mu, eps through the TMA stage, 0: plain loads
 };
 
 int march_tma_build_maps(const Dev &dv, MarchMaps *mm);
