@@ -50,8 +50,9 @@ extern "C" {
                                    Host-driven loop.  Controls: tdgl_set_mu_solver.  Not with TDGL_FLAG_MU_REFINE. */
 #define TDGL_FLAG_FP64 64u      /* the DOUBLE-PRECISION build (the paper ships and times SP and DP):
                                    psi, b, d, mu in double (104 B/site of workspace), every kernel of the step in fp64;
-                                   mu is solved by the pseudo-time iteration (the direct solver is fp32 only).  psi / mu
-                                   buffers of tdgl_get_psi_mu, tdgl_set_state, tdgl_debug_* are then double (pairs). */
+                                   mu is solved by the pseudo-time iteration in double, or directly with TDGL_FLAG_MU_DIRECT (the
+                                   transform solver itself is fp32 only).  psi / mu buffers of tdgl_get_psi_mu, tdgl_set_state,
+                                   tdgl_debug_* are then double (pairs). */
 #define TDGL_FLAG_INSULATORS 128u /* insulating inclusions (P:511 (ii), reading S25): tdgl_set_insulators removes the sites
                                    inside a list of spheres and CUTS every link between a superconducting and a removed
                                    site ("no-current boundary conditions across internal grid edges").  Needs
