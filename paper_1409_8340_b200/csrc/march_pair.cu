@@ -6,14 +6,16 @@
 // A CTA of 20 warps owns a 128 x 16 tile of the xy plane and marches through a chunk of z planes, two pipeline
 // stages per iteration t:
 //   stage 1  x^{l+1} of plane p1 = k0 - 1 + t on the tile grown by one site (rows -1 .. 16: warps 0 .. 17, one row
-//            each; columns -1 and 128: one warp each, 18 and 19), from x^l planes p1 - 1, p1 (registers) and p1 + 1 (TMA
-//            stage), written to a three-plane shared-memory ring Y;
+//            each; columns -1 and 128: one warp each, 18 and 19), from x^l planes p1 - 1 (registers), p1 and p1 + 1 (the
+//            two resident TMA stages), written to a three-plane shared-memory ring Y;
 //   stage 2  x^{l+2} of plane p2 = p1 - 1 on the tile itself (warps 1 .. 16) from x^{l+1} planes p2 - 1, p2 and the
 //            in-plane neighbours (all in Y) and p2 + 1 (just computed, registers), written to HBM.
 // Both stages use the arithmetic of the plain sweep (nsum_pair / divide_pair, same operand order, contractions
 // spelled out), so x^{l+1}, x^{l+2}, both residuals and the J_av partial sums are bit-identical to two plain sweeps.
 // Criterion (34) stays exact: the residuals of BOTH sweeps are reduced; if the first one already meets it, the pair
 // is discarded (x^l is intact in its buffer) and the plain sweep recomputes x^{l+1} (pair_decide, march_common.cuh).
+// The J_av link sums of x^{l+2} are formed only if this pair may end the step (choose_next); k_jav_tiles below supplies
+// them, bit-identically, in the rare case that a pair that skipped them did end it.
 //
 // TMA: one stage = x^l rows -2 .. 17 of plane p1 + 1 (three boxes: centre 16 rows, two rows below, two above;
 // wrapped rows for tiles at a periodic seam) and the b, d rows -1 .. 16 of plane p1; ring of 3 stages (56 KB each).
