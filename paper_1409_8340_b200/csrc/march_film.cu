@@ -25,12 +25,14 @@ constexpr int NTHREADS = 32 * NW;
 constexpr unsigned OFF_ROW = 16;
 constexpr unsigned OFF_B = 8320;         // b segment (sweep only)
 constexpr unsigned OFF_D = 16512;        // d segment (sweep only)
-constexpr unsigned STAGE_PSI = 8320, STAGE_SWEEP = 24704;
+constexpr unsigned OFF_MU = 8320;        // mu segment (init only, when nx % 4 == 0: 16-byte aligned 4-byte rows)
+constexpr unsigned OFF_EPS = 12416;      // eps segment (init only)
+constexpr unsigned STAGE_PSI = 8320, STAGE_INIT = 16512, STAGE_SWEEP = 24704;
 constexpr unsigned HDR = 256;            // mbarriers at 0, CTA residual word at 64, 8 J_av warp sums at 128
 
 template <int MODE> struct FCfg {
   static constexpr int NS = (MODE == MODE_SWEEP) ? 4 : 6;
-  static constexpr unsigned SB = (MODE == MODE_SWEEP) ? STAGE_SWEEP : STAGE_PSI;
+  static constexpr unsigned SB = (MODE == MODE_SWEEP) ? STAGE_SWEEP : (MODE == MODE_INIT ? STAGE_INIT : STAGE_PSI);
   static constexpr unsigned SMEM = HDR + NS * SB;
 };
 
@@ -71,6 +73,9 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_march_film(const __grid_constan
   const unsigned sbase = smem_u32(smem_raw);
   const unsigned stage0 = sbase + HDR;
   const unsigned rowbytes = 8u * (unsigned)nvs;
+  // init: mu, eps of the row arrive with the stage when their row segments are 16-byte aligned multiples of 16 B
+  const bool me_bulk = (MODE == MODE_INIT) && (nx % 4 == 0) && (nvs % 4 == 0) &&
+                       ((reinterpret_cast<unsigned long long>(dv.mu) | reinterpret_cast<unsigned long long>(dv.eps)) & 15ull) == 0ull;
 
   auto ywrap = [&](int jp) -> int {                                 // row index with wrap / mirror
     if (jp < 0) return py ? ny - 1 : 1;
@@ -84,7 +89,8 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_march_film(const __grid_constan
     const unsigned sb = stage0 + slot * SB, bar = sbase + 8u * slot;
     const float2 *src = xin + (long long)ywrap(j0 + t) * nx;
     const bool bd = (MODE == MODE_SWEEP) && t >= 1;
-    mbar_expect_tx(bar, rowbytes + 32u + (bd ? 2u * rowbytes : 0u));
+    const bool me = (MODE == MODE_INIT) && me_bulk && t >= 1;         // mu, eps of row j0 + t - 1
+    mbar_expect_tx(bar, rowbytes + 32u + (bd ? 2u * rowbytes : 0u) + (me ? (dv.solve_mu ? rowbytes : rowbytes / 2u) : 0u));
     bulk_load_1d(sb + OFF_ROW, src + i0, rowbytes, bar);
     bulk_load_1d(sb, src + gW, 16u, bar);
     bulk_load_1d(sb + OFF_ROW + rowbytes, src + gE, 16u, bar);
@@ -92,6 +98,11 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_march_film(const __grid_constan
       const long long o = (long long)(j0 + t - 1) * nx + i0;
       bulk_load_1d(sb + OFF_B, dv.b + o, rowbytes, bar);
       bulk_load_1d(sb + OFF_D, dv.d + o, rowbytes, bar);
+    }
+    if (me) {
+      const long long o = (long long)(j0 + t - 1) * nx + i0;
+      if (dv.solve_mu) bulk_load_1d(sb + OFF_MU, dv.mu + o, rowbytes / 2u, bar);
+      bulk_load_1d(sb + OFF_EPS, dv.eps + o, rowbytes / 2u, bar);
     }
   };
 
@@ -150,7 +161,7 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_march_film(const __grid_constan
       }
     }
   };
-  load_mu_eps(idx, muA, muB, epA, epB);
+  if (!me_bulk) load_mu_eps(idx, muA, muB, epA, epB);
 
   // one row: Bv, Cv = this thread's values of rows j-1, j; Tv receives row j+1
   auto do_row = [&](int t, float4 &BvA, float4 &BvB, float4 &CvA, float4 &CvB, float4 &TvA, float4 &TvB) {
@@ -173,7 +184,11 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_march_film(const __grid_constan
     float2 nmuA, nmuB, nepA, nepB;
     if (MODE == MODE_INIT) {
       nmuA = muA; nmuB = muB; nepA = epA; nepB = epB;
-      if (t < nk) load_mu_eps(idx + nx, nmuA, nmuB, nepA, nepB);
+      if (me_bulk) {                                   // mu, eps of THIS row arrived with the stage
+        const unsigned om = 4u * (unsigned)sA;
+        if (dv.solve_mu) { muA = lds64(cur + OFF_MU + om); muB = lds64(cur + OFF_MU + om + 256u); }
+        epA = lds64(cur + OFF_EPS + om); epB = lds64(cur + OFF_EPS + om + 256u);
+      } else if (t < nk) load_mu_eps(idx + nx, nmuA, nmuB, nepA, nepB);
     }
     float2 WA, EA, WB, EB;
     WA.x = __shfl_up_sync(0xffffffffu, CvA.z, 1);   WA.y = __shfl_up_sync(0xffffffffu, CvA.w, 1);
@@ -256,7 +271,7 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_march_film(const __grid_constan
         };
         init_pair(CvA, muA, epA, idx, actA, sA0, sA1, nA0, nA1, dA);
         init_pair(CvB, muB, epB, idx + 64, actB, sB0, sB1, nB0, nB1, dB);
-        muA = nmuA; muB = nmuB; epA = nepA; epB = nepB;
+        if (!me_bulk) { muA = nmuA; muB = nmuB; epA = nepA; epB = nepB; }
       }
       float rloc = 0.f;
       const float4 outA = divide_pair(nA0, nA1, dA, CvA, rloc);
