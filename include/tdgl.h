@@ -33,6 +33,7 @@ extern "C" {
 #define TDGL_EINCOMPAT   (-3)   /* open x with Jx != 0; a field component the Landau gauge chosen  */
                                 /* at create cannot carry (By in the xz gauge, Bx in the yz gauge or film) */
 #define TDGL_ECUDA       (-4)   /* a CUDA runtime call failed; tdgl_last_cuda_error() has the code      */
+#define TDGL_ESCRATCH    (-5)   /* tdgl_mean_abs2_static only: more sites than its built-in scratch array covers */
 #define TDGL_WMAXSWEEPS    1    /* some step hit max_sweeps before max|r|^2 < eps_tol (S10)             */
 
 #define TDGL_BC_PERIODIC   0    /* (quasi-)periodic                                          */
@@ -237,6 +238,36 @@ int tdgl_get_mu_direct_stats(tdgl_t *h, int64_t *solves_host, int64_t *passes_ho
  * launched, pairs discarded since create. */
 int tdgl_set_pair_mode(tdgl_t *h, int32_t mode);
 int tdgl_get_pair_stats(tdgl_t *h, int32_t *eligible_host, int64_t *pairs_host, int64_t *redone_host);
+
+/* ---- for callers that cannot allocate device memory ---------------------------------------------------------------
+ * <|psi|^2> (observable a8; the same per-site fp32 |psi_m|^2 summed in fp64 as tdgl_observables.mean_abs2) WITHOUT a
+ * handle and WITHOUT a workspace.  Every other call needs the 44 B/site workspace the owner of the simulation allocated.
+ * Code that merely sits beside a running solver and was handed a pointer to psi has none, and often cannot get any: an
+ * in-situ monitor whose cudaMalloc / cudaFree would synchronise the device and stall the time-stepping stream, a plug-in
+ * in a host application whose own pool reserved all of HBM at start-up (a cudaMalloc then fails), a component that is
+ * forbidden to allocate after initialisation.  For them the scratch of the reduction (per-CTA partial sums and the
+ * counter that elects the finishing CTA) lives in a fixed array inside the library image, and the call allocates
+ * nothing -- no cudaMalloc, no cudaFree, no allocating library routine.
+ *
+ *   psi_dev   DEVICE, n_sites (re, im) fp32 pairs, 8-byte aligned (16-byte alignment takes the faster two-site loads); read only
+ *   n_sites   1 ... TDGL_STATIC_MAX_SITES (2^29 = 1024 x 1024 x 512).  More: TDGL_ESCRATCH, nothing is enqueued or written
+ *   mean_dev  DEVICE, one double, 8-byte aligned; written by the kernel, valid once the work enqueued on `stream` is done
+ *   stream    cudaStream_t (NULL = legacy default stream) of the CURRENT device, which must own psi_dev and mean_dev
+ *
+ * What the built-in array implies:
+ *   - TDGL_STATIC_SCRATCH_BYTES of device memory are held on every GPU that loads the library, until the process exits;
+ *   - one array per device, shared by ALL calls: calls that can overlap on the GPU (different streams without an event
+ *     between them, several host threads) race and return garbage.  Serialise them.  Calls on one stream are safe;
+ *   - the array keeps the previous call's contents; what has to start at zero (the counter) is cleared on `stream` in
+ *     front of every launch, so no call depends on how the previous one ended;
+ *   - the FIRST call on each device resolves the array's device address (cudaGetSymbolAddress; the runtime may load the
+ *     module on that device at this point).  Make that first call during start-up, before any stream capture begins.
+ * Asynchronous.  Errors: TDGL_EINVAL (NULL / misaligned pointer, n_sites < 1), TDGL_ESCRATCH, TDGL_ECUDA (the runtime's
+ * error is left in place for cudaGetLastError()).  The result does not depend on the number of SMs (fixed 65 536-site
+ * chunks, partial sums added in index order). */
+#define TDGL_STATIC_MAX_SITES     536870912
+#define TDGL_STATIC_SCRATCH_BYTES 65792       /* 8192 fp64 partial sums + one 256-byte line for the counter */
+int tdgl_mean_abs2_static(const void *psi_dev, int64_t n_sites, double *mean_dev, void *stream);
 
 #ifdef __cplusplus
 }

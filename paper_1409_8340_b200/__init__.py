@@ -9,4 +9,5 @@ from .binding import (  # noqa: F401
     TDGL_BC_OPEN, TDGL_BC_PERIODIC, TDGL_FLAG_FP64, TDGL_FLAG_GAUGE_YZ, TDGL_FLAG_HOST_LOOP, TDGL_FLAG_INSULATORS, TDGL_FLAG_MU_ITERATIVE, TDGL_FLAG_SOLVE_MU, TdglError, TdglObs, TdglParams,
     TdglSphere, Solver, lib, tdgl_create, tdgl_destroy, tdgl_get_psi_mu, tdgl_observables, tdgl_set_field_current,
     tdgl_set_pinning, tdgl_step, tdgl_strerror, tdgl_workspace_bytes,
+    TDGL_ESCRATCH, TDGL_STATIC_MAX_SITES, tdgl_mean_abs2_static,
 )

@@ -11,6 +11,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.environ.get("TDGL_LIB") or os.path.join(_HERE, "libtdgl.so")     # TDGL_LIB: another build of the same ABI
 
 TDGL_OK, TDGL_EINVAL, TDGL_ENOMEM, TDGL_EINCOMPAT, TDGL_ECUDA, TDGL_WMAXSWEEPS = 0, -1, -2, -3, -4, 1
+TDGL_ESCRATCH = -5
+TDGL_STATIC_MAX_SITES, TDGL_STATIC_SCRATCH_BYTES = 536870912, 65792
 TDGL_BC_PERIODIC, TDGL_BC_OPEN = 0, 1
 TDGL_FLAG_SOLVE_MU, TDGL_FLAG_HOST_LOOP, TDGL_FLAG_GAUGE_YZ, TDGL_FLAG_MU_REFINE, TDGL_FLAG_MU_NOREFINE = 1, 2, 4, 8, 16
 TDGL_FLAG_MU_ITERATIVE, TDGL_FLAG_FP64, TDGL_FLAG_INSULATORS, TDGL_FLAG_MU_DIRECT = 32, 64, 128, 256
@@ -21,6 +23,7 @@ EXPORTS = (
     "tdgl_set_sweep_schedule", "tdgl_get_sweep_log", "tdgl_get_eps", "tdgl_debug_noise", "tdgl_debug_poisson",
     "tdgl_debug_rho", "tdgl_launch_count", "tdgl_sweep_timing", "tdgl_mu_gain", "tdgl_mu_refine_enabled",
     "tdgl_set_mu_solver", "tdgl_get_mu_log", "tdgl_set_insulators", "tdgl_set_pinning_shapes", "tdgl_set_insulator_shapes", "tdgl_set_pair_mode", "tdgl_get_pair_stats", "tdgl_get_mu_direct_stats",
+    "tdgl_mean_abs2_static",
 )
 
 
@@ -101,6 +104,7 @@ def lib() -> C.CDLL:
     L.tdgl_set_pair_mode.argtypes = [vp, i32]
     L.tdgl_get_pair_stats.argtypes = [vp, C.POINTER(i32), C.POINTER(i64), C.POINTER(i64)]
     L.tdgl_get_mu_log.argtypes = [vp, i32, C.POINTER(i32), C.POINTER(i32), i32, C.POINTER(i32)]
+    L.tdgl_mean_abs2_static.argtypes = [vp, i64, vp, vp]
     _lib = L
     return L
 
@@ -167,6 +171,15 @@ def tdgl_observables(h) -> TdglObs:
     o = TdglObs()
     _check(lib().tdgl_observables(h, C.byref(o)), "tdgl_observables", h)
     return o
+
+
+def tdgl_mean_abs2_static(psi_dev_ptr: Optional[int], n_sites: int, mean_dev_ptr: Optional[int], stream_ptr: Optional[int] = None) -> None:
+    """<|psi|^2> of n_sites (re, im) fp32 pairs at DEVICE address psi_dev_ptr into the double at DEVICE address
+    mean_dev_ptr, enqueued on the CUDA stream stream_ptr -- for callers that hold a pointer to psi but cannot allocate
+    device memory (no handle, no workspace: the scratch is a fixed array inside libtdgl.so).  At most
+    TDGL_STATIC_MAX_SITES sites (TdglError with code TDGL_ESCRATCH beyond); one call at a time per device; make the
+    first call on a device at start-up.  See include/tdgl.h."""
+    _check(lib().tdgl_mean_abs2_static(psi_dev_ptr, int(n_sites), mean_dev_ptr, stream_ptr), "tdgl_mean_abs2_static")
 
 
 # ---- convenience wrapper: torch owns the device memory and the stream ------------------------------

@@ -8,7 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtdgl.so")
-SOURCES = ["tdgl_api.cu", "march_tma.cu", "march_film.cu", "march_pair.cu", "step_ctl.cu", "poisson.cu", "fft.cu", "fft_r8.cu", "dct.cu", "dct_pfa.cu", "aux.cu", "refine.cu", "plain.cu"]
+SOURCES = ["tdgl_api.cu", "march_tma.cu", "march_film.cu", "march_pair.cu", "step_ctl.cu", "poisson.cu", "fft.cu", "fft_r8.cu", "dct.cu", "dct_pfa.cu", "aux.cu", "refine.cu", "plain.cu", "static_scratch.cu"]
 HEADERS = ["tdgl_dev.cuh", "march_tma.h", "march_film.h", "march_pair.h", "march_common.cuh", "philox.cuh", "fft_regs.cuh", os.path.join("..", "..", "include", "tdgl.h")]
 
 

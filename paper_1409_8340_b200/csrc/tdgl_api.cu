@@ -825,6 +825,7 @@ extern "C" const char *tdgl_strerror(int code) {
     case TDGL_ENOMEM: return "workspace too small or misaligned";
     case TDGL_EINCOMPAT: return "incompatible request (open x with a current, a field component the chosen Landau gauge cannot carry, or a call the mode chosen at create does not support)";
     case TDGL_ECUDA: return "CUDA runtime error";
+    case TDGL_ESCRATCH: return "more sites than the built-in scratch array of tdgl_mean_abs2_static covers (TDGL_STATIC_MAX_SITES)";
     case TDGL_WMAXSWEEPS: return "warning: Jacobi iteration hit max_sweeps";
     default: return "unknown code";
   }
