@@ -35,6 +35,8 @@ extern "C" {
 #define TDGL_ECUDA       (-4)   /* a CUDA runtime call failed; tdgl_last_cuda_error() has the code      */
 #define TDGL_ESCRATCH    (-5)   /* tdgl_mean_abs2_static only: more sites than its built-in scratch array covers */
 #define TDGL_WMAXSWEEPS    1    /* some step hit max_sweeps before max|r|^2 < eps_tol (S10)             */
+#define TDGL_WMUCAP        2    /* TDGL_FLAG_MU_ITERATIVE / FP64: some mu solve stopped at max_outer or max_inner
+                                   (tdgl_set_mu_solver) before eps_mu / eps_in was met: mu is not converged          */
 
 #define TDGL_BC_PERIODIC   0    /* (quasi-)periodic                                          */
 #define TDGL_BC_OPEN       1    /* open: n.(grad - iA)psi = 0, n.grad(mu) = 0            */
@@ -109,7 +111,7 @@ typedef struct {
   int64_t steps;              /* steps taken since create                                              */
   int64_t sweeps_total;       /* Jacobi sweeps since create                                            */
   int32_t sweeps_last;        /* sweeps of the last step                                               */
-  int32_t status;             /* latched TDGL_WMAXSWEEPS, else 0                                       */
+  int32_t status;             /* latched warnings since create: TDGL_WMAXSWEEPS | TDGL_WMUCAP (bits), 0 = none */
 } tdgl_obs;
 
 /* Bytes of device workspace tdgl_create needs for these params (0 if the params are invalid).
@@ -169,7 +171,8 @@ int tdgl_step(tdgl_t *h, int32_t nsteps);
  * is current is device state; a copy kernel reads it on the device, the host never waits). */
 int tdgl_get_psi_mu(tdgl_t *h, void *psi_dev, void *mu_dev);
 
-/* Runs the reductions (a8) and fills *out_host.  Synchronises the stream. */
+/* Runs the reductions (a8) and fills *out_host.  Synchronises the stream.  Returns the latched warning, if any
+ * (TDGL_WMAXSWEEPS before TDGL_WMUCAP when both are set; out_host->status carries both bits). */
 int tdgl_observables(tdgl_t *h, tdgl_obs *out_host);
 
 const char *tdgl_strerror(int code);
@@ -190,7 +193,7 @@ double tdgl_mu_gain(const tdgl_params *p_host);
  * max|(mu - mu^-)/h_tau|^2 < eps_mu.  Defaults (S20): h_tau = 0.1, eps_mu = eps_in = 1e-6, max_outer = 1000,
  * max_inner = 100. */
 int tdgl_set_mu_solver(tdgl_t *h, float h_tau, float eps_mu, float eps_in, int32_t max_outer, int32_t max_inner);
-/* Log of the last `nsolves` mu solves (one per time step): outer_host[s] = outer iterations of solve s (oldest first);
+/* Log of the last `nsolves` mu solves (one per time step, and one per tdgl_debug_poisson call in this mode): outer_host[s] = outer iterations of solve s (oldest first);
  * inner_host = the Jacobi sweep counts of all those outer iterations in order (sum(outer_host) entries, at most
  * inner_cap, else TDGL_ENOMEM); *n_inner_host = that number.  Host arrays, any may be NULL.  Synchronises the stream. */
 int tdgl_get_mu_log(tdgl_t *h, int32_t nsolves, int32_t *outer_host, int32_t *inner_host, int32_t inner_cap, int32_t *n_inner_host);

@@ -10,4 +10,5 @@ from .binding import (  # noqa: F401
     TdglSphere, Solver, lib, tdgl_create, tdgl_destroy, tdgl_get_psi_mu, tdgl_observables, tdgl_set_field_current,
     tdgl_set_pinning, tdgl_step, tdgl_strerror, tdgl_workspace_bytes,
     TDGL_ESCRATCH, TDGL_STATIC_MAX_SITES, tdgl_mean_abs2_static,
+    TDGL_FLAG_MU_DIRECT, TDGL_FLAG_MU_REFINE, TDGL_FLAG_MU_NOREFINE, TDGL_WMAXSWEEPS, TDGL_WMUCAP,
 )

@@ -12,6 +12,7 @@ _LIB_PATH = os.environ.get("TDGL_LIB") or os.path.join(_HERE, "libtdgl.so")     
 
 TDGL_OK, TDGL_EINVAL, TDGL_ENOMEM, TDGL_EINCOMPAT, TDGL_ECUDA, TDGL_WMAXSWEEPS = 0, -1, -2, -3, -4, 1
 TDGL_ESCRATCH = -5
+TDGL_WMUCAP = 2
 TDGL_STATIC_MAX_SITES, TDGL_STATIC_SCRATCH_BYTES = 536870912, 65792
 TDGL_BC_PERIODIC, TDGL_BC_OPEN = 0, 1
 TDGL_FLAG_SOLVE_MU, TDGL_FLAG_HOST_LOOP, TDGL_FLAG_GAUGE_YZ, TDGL_FLAG_MU_REFINE, TDGL_FLAG_MU_NOREFINE = 1, 2, 4, 8, 16

@@ -353,14 +353,14 @@ static unsigned grid_for(long long n, int block, int cap) {
   long long g = (n + block - 1) / block;
   return (unsigned)(g < 1 ? 1 : (g > cap ? cap : g));
 }
-void launch_init_state(const Dev &dv, float amp, cudaStream_t st) { k_init_state<<<grid_for(dv.N, 256, 148 * 16), 256, 0, st>>>(dv, amp); }
+void launch_init_state(const Dev &dv, float amp, cudaStream_t st) { k_init_state<<<grid_for(dv.N, 256, tdgl_sm_count() * 16), 256, 0, st>>>(dv, amp); }
 void launch_ctl_reset(const Dev &dv, float tol, int maxs, int fixed, cudaStream_t st) { k_ctl_reset<<<1, 1, 0, st>>>(dv, tol, maxs, fixed); }
 void launch_ctl_solver(const Dev &dv, float tol, int maxs, int fixed, cudaStream_t st) { k_ctl_solver<<<1, 1, 0, st>>>(dv, tol, maxs, fixed); }
 void launch_ctl_sched(const Dev &dv, int n, cudaStream_t st) { k_ctl_sched<<<1, 1, 0, st>>>(dv, n); }
 void launch_ctl_pair_mode(const Dev &dv, int mode, cudaStream_t st) { k_ctl_pair_mode<<<1, 1, 0, st>>>(dv, mode); }
 void launch_ctl_state(const Dev &dv, double K, cudaStream_t st) { k_ctl_state<<<1, 1, 0, st>>>(dv, K); }
 void launch_set_field(const Dev &dv, double Bx, double Bz, double J, cudaStream_t st) { k_set_field<<<1, 256, 0, st>>>(dv, Bx, Bz, J); }
-void launch_fill(float *p, long long n, float v, cudaStream_t st) { k_fill_f32<<<grid_for(n, 256, 148 * 16), 256, 0, st>>>(p, n, v); }
+void launch_fill(float *p, long long n, float v, cudaStream_t st) { k_fill_f32<<<grid_for(n, 256, tdgl_sm_count() * 16), 256, 0, st>>>(p, n, v); }
 static void spheres_impl(const Dev &dv, const float4 *sph, long long n, float eps_in, cudaStream_t st, unsigned char *mask) {
   for (long long off = 0; off < n; off += 1 << 20) {
     const unsigned g = (unsigned)((n - off) < (1 << 20) ? (n - off) : (1 << 20));
@@ -377,8 +377,8 @@ void launch_shapes(const Dev &dv, const float *shp, long long n, float eps_in, u
     k_shapes<<<g, 128, 0, st>>>(dv, shp + 10 * off, eps_in, mask);
   }
 }
-void launch_copy_psi(const Dev &dv, float2 *out, cudaStream_t st) { k_copy_psi<<<grid_for(dv.N / 2, 256, 148 * 16), 256, 0, st>>>(dv, out); }
-void launch_noise(const Dev &dv, long long step, float2 *out, cudaStream_t st) { k_noise<<<grid_for(dv.N, 256, 148 * 16), 256, 0, st>>>(dv, step, out); }
+void launch_copy_psi(const Dev &dv, float2 *out, cudaStream_t st) { k_copy_psi<<<grid_for(dv.N / 2, 256, tdgl_sm_count() * 16), 256, 0, st>>>(dv, out); }
+void launch_noise(const Dev &dv, long long step, float2 *out, cudaStream_t st) { k_noise<<<grid_for(dv.N, 256, tdgl_sm_count() * 16), 256, 0, st>>>(dv, step, out); }
 void launch_obs_final(const Dev &dv, int npart, cudaStream_t st) { k_obs_final<<<1, 256, 0, st>>>(dv, npart); }
 int launch_obs(const Dev &dv, cudaStream_t st) {
   const long long nblk = (long long)((dv.ny + OBS_RB - 1) / OBS_RB) * dv.nz;

@@ -22,6 +22,7 @@
 //   V_k = v_0 + sum_j a_j cos(2 pi j k/R) - i sum_j b_j sin(2 pi j k/R),  V_{R-k} = conj-partner: (R-1)^2 real FMAs.
 // Work per line of 1024 points: 2 x (17 x 900 + 47 x 100 + 171 x 4) = 41 k FMAs (Bluestein: two 4096-point FFTs per
 // line pair, about 250 k flops per line and six times the shared-memory traffic).
+#include <mutex>
 #include "tdgl_dev.cuh"
 #include <vector>
 
@@ -359,19 +360,28 @@ void dct_pfa_build_table(int kind, bool xpass, unsigned short *host_out) {
   const std::vector<unsigned short> t = build_tables(kPlans[kind].R, plan_lp(kind), xpass);
   for (size_t i = 0; i < t.size(); ++i) host_out[i] = t[i];
 }
+// __constant__ memory and function attributes belong to a DEVICE, not to the process: the trig table is uploaded once per
+// device (the current one; tdgl_create runs with the caller's device current), and the attributes are set on every call.
 cudaError_t dct_pfa_configure(int kind) {
-  static bool trig_done = false;                              // cos / sin of every supported radix, fp64 -> fp32, once
-  if (!trig_done) {
-    float4 h[96];
-    for (int i = 0; i < 96; ++i) h[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-    for (int R : kRadices)
-      for (int t = 0; t < R; ++t) {
-        const double ang = 2.0 * 3.14159265358979323846 * t / R;
-        h[trig_off(R) + t] = make_float4((float)cos(ang), (float)cos(ang), (float)sin(ang), (float)sin(ang));
-      }
-    cudaError_t e = cudaMemcpyToSymbol(c_trig, h, sizeof(h));
-    if (e != cudaSuccess) return e;
-    trig_done = true;
+  static std::mutex lock;
+  static unsigned long long trig_done = 0;                    // bit d: cos / sin of every supported radix (fp64 -> fp32) are on device d
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  {
+    std::lock_guard<std::mutex> guard(lock);
+    if (dev < 0 || dev >= 64 || !((trig_done >> dev) & 1ull)) {
+      float4 h[96];
+      for (int i = 0; i < 96; ++i) h[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+      for (int R : kRadices)
+        for (int t = 0; t < R; ++t) {
+          const double ang = 2.0 * 3.14159265358979323846 * t / R;
+          h[trig_off(R) + t] = make_float4((float)cos(ang), (float)cos(ang), (float)sin(ang), (float)sin(ang));
+        }
+      e = cudaMemcpyToSymbol(c_trig, h, sizeof(h));
+      if (e != cudaSuccess) return e;
+      if (dev >= 0 && dev < 64) trig_done |= 1ull << dev;
+    }
   }
   switch (kind) {
     case 0: return L1024::configure();

@@ -114,6 +114,6 @@ cudaError_t dht_x_512_configure() {
 }
 void launch_dht_x_512(float *data, long long nrows, const float2 *tw, cudaStream_t st) {
   const long long npairs = (nrows + 1) / 2, ntiles = (npairs + LP - 1) / LP;
-  const long long grid = ntiles < 148 * 2 ? ntiles : 148 * 2;
+  const long long grid = ntiles < tdgl_sm_count() * 2 ? ntiles : tdgl_sm_count() * 2;
   k_dht_x_512<<<(unsigned)grid, NT, SMEM, st>>>(data, nrows, ntiles, tw);
 }

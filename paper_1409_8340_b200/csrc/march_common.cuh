@@ -179,7 +179,7 @@ __device__ __noinline__ void sweep_decide(const Dev &dv, int l) {
     done = sweeps >= target;
   } else {
     done = (r2 < c->eps_tol) || sweeps >= c->max_sweeps;
-    if (!(r2 < c->eps_tol) && sweeps >= c->max_sweeps) c->status = 1;
+    if (!(r2 < c->eps_tol) && sweeps >= c->max_sweeps) c->status |= 1;
   }
   choose_next(dv, c, sweeps, target, r2, l > 0 ? c->r_hist : 0.f);
   c->r_hist = r2;
@@ -216,7 +216,7 @@ __device__ __noinline__ void pair_decide(const Dev &dv, int l) {
       done = sweeps >= target;
     } else {
       done = (r2 < c->eps_tol) || sweeps >= c->max_sweeps;
-      if (!(r2 < c->eps_tol) && sweeps >= c->max_sweeps) c->status = 1;
+      if (!(r2 < c->eps_tol) && sweeps >= c->max_sweeps) c->status |= 1;
     }
     const int had_jav = c->pair_jav;                    // (read before choose_next overwrites it)
     choose_next(dv, c, sweeps, target, r2, r1);

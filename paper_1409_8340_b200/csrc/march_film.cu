@@ -55,6 +55,7 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_march_film(const __grid_constan
   extern __shared__ __align__(128) unsigned char smem_raw[];
   Ctl *ctl = dv.ctl;
   int l = 0;
+  if (MODE == MODE_SWEEP && (blockIdx.x | blockIdx.y | blockIdx.z | threadIdx.x) == 0) ctl->body_launches += 1;   // as march_tma.cu: tdgl_launch_count in graph mode
   if (MODE != MODE_RHO) {
     if (ctl->done) return;
     l = ctl->sweeps;

@@ -433,7 +433,10 @@ __global__ void __launch_bounds__(128) k_mu_sweep(const __grid_constant__ Dev dv
       ctl->mu_inner = sweeps;
       bool done;
       if (ctl->mu_sched_pos < ctl->mu_sched_n) done = sweeps >= dv.mu_sched[ctl->mu_sched_pos];
-      else done = r2max < (double)ctl->eps_mu_in || sweeps >= ctl->mu_max_inner;
+      else {
+        done = r2max < (double)ctl->eps_mu_in || sweeps >= ctl->mu_max_inner;
+        if (!(r2max < (double)ctl->eps_mu_in) && sweeps >= ctl->mu_max_inner) ctl->status |= 2;   // TDGL_WMUCAP: the cap, not the test, ended it
+      }
       if (done) ctl->mu_inner_done = 1;
       __threadfence();
     }
@@ -475,7 +478,10 @@ __global__ void __launch_bounds__(128) k_mu_finish(const __grid_constant__ Dev d
       ctl->mu_dt2_last = dt2;
       bool done;
       if (ctl->mu_sched_pos < ctl->mu_sched_n) { ctl->mu_sched_pos += 1; done = ctl->mu_sched_pos >= ctl->mu_sched_n; }
-      else done = dt2 < (double)ctl->eps_mu || ctl->mu_outer >= ctl->mu_max_outer;
+      else {
+        done = dt2 < (double)ctl->eps_mu || ctl->mu_outer >= ctl->mu_max_outer;
+        if (!(dt2 < (double)ctl->eps_mu) && ctl->mu_outer >= ctl->mu_max_outer) ctl->status |= 2;   // TDGL_WMUCAP
+      }
       if (done) ctl->mu_done = 1;
       __threadfence();
     }
@@ -636,17 +642,17 @@ int launch_jav64(const Dev &dv, cudaStream_t st) {                 // returns th
   k_jav64<<<g, 256, 0, st>>>(dv);
   return (int)g;
 }
-void launch_init_state64(const Dev &dv, double amp, cudaStream_t st) { k_init_state64<<<grid1(dv.N, 256, 148 * 16), 256, 0, st>>>(dv, amp); }
-void launch_noise64(const Dev &dv, long long step, double2 *out, cudaStream_t st) { k_noise64<<<grid1(dv.N, 256, 148 * 16), 256, 0, st>>>(dv, step, out); }
-void launch_copy_psi64(const Dev &dv, double2 *out, cudaStream_t st) { k_copy_psi64<<<grid1(dv.N, 256, 148 * 16), 256, 0, st>>>(dv, out); }
+void launch_init_state64(const Dev &dv, double amp, cudaStream_t st) { k_init_state64<<<grid1(dv.N, 256, tdgl_sm_count() * 16), 256, 0, st>>>(dv, amp); }
+void launch_noise64(const Dev &dv, long long step, double2 *out, cudaStream_t st) { k_noise64<<<grid1(dv.N, 256, tdgl_sm_count() * 16), 256, 0, st>>>(dv, step, out); }
+void launch_copy_psi64(const Dev &dv, double2 *out, cudaStream_t st) { k_copy_psi64<<<grid1(dv.N, 256, tdgl_sm_count() * 16), 256, 0, st>>>(dv, out); }
 int launch_obs64(const Dev &dv, cudaStream_t st) {                 // followed by k_obs_final (aux.cu): returns the partial count
   const unsigned g = grid1(dv.N, 256, TDGL_NPART);
   k_obs64<<<g, 256, 0, st>>>(dv);
   return (int)g;
 }
-void launch_apply_mask64(const Dev &dv, cudaStream_t st) { k_apply_mask64<<<grid1(dv.N, 256, 148 * 16), 256, 0, st>>>(dv); }
-void launch_fill_u8(unsigned char *p, long long n, unsigned char v, cudaStream_t st) { k_fill_u8<<<grid1(n, 256, 148 * 16), 256, 0, st>>>(p, n, v); }
-void launch_fill64(double *p, long long n, double v, cudaStream_t st) { k_fill_t<double><<<grid1(n, 256, 148 * 16), 256, 0, st>>>(p, n, v); }
+void launch_apply_mask64(const Dev &dv, cudaStream_t st) { k_apply_mask64<<<grid1(dv.N, 256, tdgl_sm_count() * 16), 256, 0, st>>>(dv); }
+void launch_fill_u8(unsigned char *p, long long n, unsigned char v, cudaStream_t st) { k_fill_u8<<<grid1(n, 256, tdgl_sm_count() * 16), 256, 0, st>>>(p, n, v); }
+void launch_fill64(double *p, long long n, double v, cudaStream_t st) { k_fill_t<double><<<grid1(n, 256, tdgl_sm_count() * 16), 256, 0, st>>>(p, n, v); }
 
 // the pieces of one pseudo-time solve; `mu` = the array that holds mu^- and receives mu (T = double iff dv.fp64)
 void launch_mu_begin(const Dev &dv, cudaStream_t st) { k_mu_begin<<<1, 1, 0, st>>>(dv); }
@@ -669,10 +675,10 @@ void launch_mu_controls(const Dev &dv, float h_tau, float eps_mu, float eps_in, 
 void launch_mu_sched(const Dev &dv, int n, cudaStream_t st) { k_mu_sched<<<1, 1, 0, st>>>(dv, n); }
 
 void launch_dref_ctl(const Dev &dv, int what, cudaStream_t st) { k_dref_ctl<<<1, 1, 0, st>>>(dv, what); }
-void launch_dref_begin(const Dev &dv, cudaStream_t st) { k_dref_begin<<<148 * 8, 256, 0, st>>>(dv); }
-void launch_dref_add(const Dev &dv, cudaStream_t st) { k_dref_add<<<148 * 8, 256, 0, st>>>(dv); }
+void launch_dref_begin(const Dev &dv, cudaStream_t st) { k_dref_begin<<<tdgl_sm_count() * 8, 256, 0, st>>>(dv); }
+void launch_dref_add(const Dev &dv, cudaStream_t st) { k_dref_add<<<tdgl_sm_count() * 8, 256, 0, st>>>(dv); }
 void launch_dref_resid(const Dev &dv, cudaStream_t st) { k_dref_resid<<<grid3(dv), 128, 0, st>>>(dv); }
 void launch_dref_zero_mean(const Dev &dv, cudaStream_t st) {
   k_dref_wsum<<<DREF_NB, 256, 0, st>>>(dv);
-  k_dref_shift<<<148 * 8, 256, 0, st>>>(dv);
+  k_dref_shift<<<tdgl_sm_count() * 8, 256, 0, st>>>(dv);
 }

@@ -28,8 +28,11 @@ __device__ __forceinline__ c64 ldd(const double2 *p) { const double2 v = __ldg(p
 // the neighbour operators of SURVEY 8(c) (wrap / quasi-periodic jump / open-face rule S- := S+), link variables
 // from the fp64 tables; otherwise rho is read from `rho` (kernel-level test entry tdgl_debug_poisson).
 template <bool FROM_PSI>
-__global__ void __launch_bounds__(256) k_mu_residual(const __grid_constant__ Dev dv, const float *__restrict__ rho,
-                                                     const float *__restrict__ mu, float *__restrict__ out) {
+// `rho` and `out` MAY be the same array (tdgl_debug_poisson keeps rho in the residual buffer and overwrites it in place:
+// each thread reads rho[m] before it writes out[m], and no other thread touches element m), so neither is __restrict__
+// and rho is read with a plain load, not through the read-only path.
+__global__ void __launch_bounds__(256) k_mu_residual(const __grid_constant__ Dev dv, const float *rho,
+                                                     const float *__restrict__ mu, float *out) {
   const int nx = dv.nx, ny = dv.ny, nz = dv.nz;
   const bool px = dv.bcx == 0, py = dv.bcy == 0, pz = dv.bcz == 0, film = nz == 1, yz = dv.gauge_yz != 0;
   const long long plane = (long long)nx * ny;
@@ -86,7 +89,7 @@ __global__ void __launch_bounds__(256) k_mu_residual(const __grid_constant__ Dev
       }
       r = c.x * s.y - c.y * s.x;                            // Im[psi* s]
     } else {
-      r = (double)__ldg(rho + m);
+      r = (double)rho[m];
     }
     // (Delta_h mu)_m with wrap / mirror ghost
     const double m0 = (double)__ldg(mu + m);
@@ -121,10 +124,10 @@ unsigned grid_for(long long n, int block, int cap) {
 
 // r = rho_64(psi, K) - Delta_h mu  ->  out      (rho == nullptr: rho from psi)
 void launch_mu_residual(const Dev &dv, const float *rho, const float *mu, float *out, cudaStream_t st) {
-  const unsigned g = grid_for(dv.N, 256, 148 * 32);
+  const unsigned g = grid_for(dv.N, 256, tdgl_sm_count() * 32);
   if (rho) k_mu_residual<false><<<g, 256, 0, st>>>(dv, rho, mu, out);
   else k_mu_residual<true><<<g, 256, 0, st>>>(dv, nullptr, mu, out);
 }
 void launch_mu_add(const Dev &dv, float *mu, const float *delta, cudaStream_t st) {
-  k_mu_add<<<grid_for(dv.N / 4, 256, 148 * 16), 256, 0, st>>>(mu, delta, dv.N / 4, dv.N);
+  k_mu_add<<<grid_for(dv.N / 4, 256, tdgl_sm_count() * 16), 256, 0, st>>>(mu, delta, dv.N / 4, dv.N);
 }

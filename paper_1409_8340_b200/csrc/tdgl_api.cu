@@ -1,5 +1,6 @@
 // C ABI of libtdgl (include/tdgl.h): parameter validation, workspace carving, the per-step launch
 // sequence (host loop or CUDA graph with a WHILE node around the Jacobi sweep), read-back.
+#include <atomic>
 #include "../../include/tdgl.h"
 #include "tdgl_dev.cuh"
 #include "march_tma.h"
@@ -105,16 +106,17 @@ struct tdgl {
 
 static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
-// SMs of the current device (B200: 148), queried once; the launch geometry is sized in multiples of it
-static int sm_count() {
-  static int n = 0;
-  if (n <= 0) {
-    int dev = 0, v = 0;
-    if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0) n = v;
-    else { cudaGetLastError(); return 148; }
-  }
-  return n;
+// SMs of the CURRENT device (B200: 148), queried once per device; the launch geometry is sized in multiples of it
+int tdgl_sm_count() {
+  static std::atomic<int> cached[64];
+  int dev = 0, v = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return 148; }
+  if (dev >= 0 && dev < 64 && (v = cached[dev].load(std::memory_order_relaxed)) > 0) return v;
+  if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || v <= 0) { cudaGetLastError(); return 148; }
+  if (dev >= 0 && dev < 64) cached[dev].store(v, std::memory_order_relaxed);
+  return v;
 }
+static int sm_count() { return tdgl_sm_count(); }
 
 // launch geometry of the marching kernels (march_tma.cu): 128 x 8 tiles, one warp per row; z chunks chosen
 // so that there are enough CTAs for ~4 waves of 2 CTAs/SM, chunks of at least 8 planes
@@ -814,8 +816,8 @@ extern "C" int tdgl_observables(tdgl_t *h, tdgl_obs *out) {
   out->max_resid2 = c.resid_last;
   out->Bx_eff = (float)h->Bx_eff; out->Bz_eff = (float)h->Bz_eff;
   out->steps = c.n; out->sweeps_total = c.sweeps_total; out->sweeps_last = c.sweeps_last;
-  out->status = c.status ? TDGL_WMAXSWEEPS : 0;
-  return c.status ? TDGL_WMAXSWEEPS : TDGL_OK;
+  out->status = ((c.status & 1) ? TDGL_WMAXSWEEPS : 0) | ((c.status & 2) ? TDGL_WMUCAP : 0);
+  return (c.status & 1) ? TDGL_WMAXSWEEPS : ((c.status & 2) ? TDGL_WMUCAP : TDGL_OK);
 }
 
 extern "C" const char *tdgl_strerror(int code) {
@@ -827,6 +829,7 @@ extern "C" const char *tdgl_strerror(int code) {
     case TDGL_ECUDA: return "CUDA runtime error";
     case TDGL_ESCRATCH: return "more sites than the built-in scratch array of tdgl_mean_abs2_static covers (TDGL_STATIC_MAX_SITES)";
     case TDGL_WMAXSWEEPS: return "warning: Jacobi iteration hit max_sweeps";
+    case TDGL_WMUCAP: return "warning: the pseudo-time mu iteration stopped at max_outer / max_inner before its tolerance was met";
     default: return "unknown code";
   }
 }

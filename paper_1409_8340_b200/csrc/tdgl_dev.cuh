@@ -21,7 +21,7 @@ struct Ctl {
   int done;                 // psi solve of the current step finished
   int use_pair;             // the next loop-body kernel to act is the fused two-sweep kernel (march_pair.cu), else the plain sweep
   int xbuf;                 // which psi buffer holds the latest iterate
-  int status;               // latched TDGL_WMAXSWEEPS
+  int status;               // latched warnings: bit 0 TDGL_WMAXSWEEPS, bit 1 TDGL_WMUCAP
   int sweeps_last;
   float resid_last;
   unsigned int ticket;      // last-block election of the sweep kernel
@@ -112,6 +112,9 @@ struct Dev {
   unsigned long long cond_handle;   // cudaGraphConditionalHandle of the WHILE node (graph mode)
   int use_cond;
 };
+
+// SMs of the current device, cached per device (tdgl_api.cu): grid caps are multiples of it
+int tdgl_sm_count();
 
 // complex products with the contraction spelled out (one product, one FMA per component): the plain sweep and the
 // fused pair kernel must round identically, whatever the compiler would choose in either context

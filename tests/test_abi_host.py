@@ -129,15 +129,15 @@ def test_null_handles_are_rejected(L):
 def test_strerror_covers_every_code(L):
     from paper_1409_8340_b200 import binding as Bd
     seen = set()
-    for code in (Bd.TDGL_OK, Bd.TDGL_EINVAL, Bd.TDGL_ENOMEM, Bd.TDGL_EINCOMPAT, Bd.TDGL_ECUDA, Bd.TDGL_ESCRATCH, Bd.TDGL_WMAXSWEEPS):
+    for code in (Bd.TDGL_OK, Bd.TDGL_EINVAL, Bd.TDGL_ENOMEM, Bd.TDGL_EINCOMPAT, Bd.TDGL_ECUDA, Bd.TDGL_ESCRATCH, Bd.TDGL_WMAXSWEEPS, Bd.TDGL_WMUCAP):
         s = Bd.tdgl_strerror(code)
         assert s and s != "unknown code"
         seen.add(s)
-    assert len(seen) == 7
+    assert len(seen) == 8
     assert Bd.tdgl_strerror(12345) == "unknown code"
     # the header's numeric values
     src = open(HEADER).read()
-    for name in ("TDGL_OK", "TDGL_EINVAL", "TDGL_ENOMEM", "TDGL_EINCOMPAT", "TDGL_ECUDA", "TDGL_ESCRATCH", "TDGL_WMAXSWEEPS"):
+    for name in ("TDGL_OK", "TDGL_EINVAL", "TDGL_ENOMEM", "TDGL_EINCOMPAT", "TDGL_ECUDA", "TDGL_ESCRATCH", "TDGL_WMAXSWEEPS", "TDGL_WMUCAP"):
         m = re.search(r"#define\s+%s\s+\(?(-?\d+)\)?" % name, src)
         assert m and int(m.group(1)) == getattr(Bd, name), name
 
