@@ -43,6 +43,34 @@ def test_noise_bit_exact(seed, step):
     s.close()
 
 
+@pytest.mark.parametrize("shape,bc", [((34, 10, 6), (P_, P_, P_)), ((130, 12, 9), (P_, O_, O_)), ((256, 32, 8), (P_, P_, O_)),
+                                      ((66, 20, 1), (P_, P_, P_)), ((2050, 9, 1), (O_, P_, P_))])
+@pytest.mark.parametrize("seed,nsteps", [(0, 1), ((1 << 40) + 99, 3)])
+def test_fused_noise_draw_is_the_oracles(shape, bc, seed, nsteps):
+    """The draw INSIDE the init kernels (k_march_tma<INIT>, k_march_film<INIT>; test_noise_bit_exact above exercises the copy
+    in k_noise).  From psi = 0 with eps = 0, mu = 0, B = 0 and one sweep per step, Eq. (31) leaves b = h_t zeta and the
+    sweep returns psi+ = h_t zeta / d with a constant real d: the new state IS the noise field, site by site.  A wrong
+    word, counter, pair assignment or step index anywhere shows as an O(0.1) difference; agreement is asked to 1e-7
+    (a few fp32 roundings of |psi+| ~ 0.02).  Several steps: the step index enters the counter (after step one psi is no longer zero, so this
+    part is ordinary parity with the noise as the only source)."""
+    nx, ny, nz = shape
+    cfg = cfg_of(nx, ny, nz, bc, temperature=1e-3, seed=seed)
+    psi0 = np.zeros((nz, ny, nx), np.complex64)
+    p, st, eps, (Bx, Bz), s = setup_pair(cfg, psi0=psi0, with_pinning=False, solve_mu=False, fixed_sweeps=1)
+    s.set_pinning(np.zeros((0, 4), np.float32), 0.0, 0.0)
+    eps = np.zeros_like(eps)
+    for n in range(nsteps):
+        s.step(1)
+        O.step(p, st, eps, Bx, Bz, 0.0, fixed_sweeps=1)
+        psi = s.get_psi_mu()[0].cpu().numpy()
+        if n == 0:
+            zeta = O.langevin_noise(p, 0)
+            ratio = st.psi / zeta                                     # h_t / d: one real constant over the whole mesh
+            assert np.max(np.abs(ratio - ratio.flat[0])) < 1e-12 and abs(ratio.flat[0].imag) < 1e-15
+        assert np.max(np.abs(psi - st.psi)) < 1e-7, (n, np.max(np.abs(psi - st.psi)))
+    s.close()
+
+
 def test_initial_state_matches_oracle_box_muller():
     cfg = cfg_of(32, 12, 6, (P_, P_, P_), seed=3)
     p = oracle_params(cfg)

@@ -138,6 +138,38 @@ def test_C2_with_noise_statistics():
     s.close()
 
 
+def test_C2_protocol_length_1000_noisy_steps():
+    """C2 exactly as BASELINE.json configs[1] writes it: 64^3, inclusions, J = 0.01, T = 1e-3, 1000 steps, the same Philox
+    stream on both sides, the oracle replaying the GPU's per-step sweep counts (S9).  north_star: "vortex count plus
+    mean |psi|^2 must agree within 1e-3 over the run" -- checked at steps 100, 250, 500 and 1000.  The decisions are
+    validated over the first 100 steps (where the two trajectories still agree pointwise to 1e-4); the pointwise deviation
+    at the later checkpoints is reported, not gated: nothing in the paper bounds it for a noisy vortex liquid."""
+    cfg = I.CONFIGS["C2"]
+    assert (cfg.nx, cfg.ny, cfg.nz, cfg.steps) == (64, 64, 64, 1000) and cfg.temperature > 0
+    p, st, eps, (Bx, Bz), s = setup_pair(cfg)
+    done, dev = 0, []
+    for upto in (100, 250, 500, 1000):
+        n = upto - done
+        s.step(n)
+        counts, _ = s.sweep_log(n)
+        O.run(p, st, eps, Bx, Bz, f32(cfg.Jx), n, sweep_counts=counts)
+        done = upto
+        if upto == 100:
+            check_decisions(p, st, counts)
+        ob = s.observables()
+        psi, _ = s.get_psi_mu()
+        links = O.paper_links(p, st.K, Bx, Bz)
+        dev.append(float(np.max(np.abs(psi.cpu().numpy() - st.psi))))
+        assert ob.steps == upto
+        assert abs(ob.mean_abs2 - O.mean_abs2(st.psi)) <= 1e-3, (upto, ob.mean_abs2, O.mean_abs2(st.psi), dev)
+        assert abs(ob.vortices_per_slice - O.vortices_per_slice(p, st.psi, links, Bz)) <= 1e-3, (upto, dev)
+        assert ob.vortices_per_slice == 16.0                  # n_z flux quanta per slice, P:467
+        assert abs(ob.K - st.K) < 1e-3 and ob.status == 0
+    assert dev[0] <= 1e-4, dev
+    print("C2 1000 noisy steps: max|dpsi| at 100/250/500/1000 =", dev)
+    s.close()
+
+
 @pytest.mark.parametrize("name,shape,nsteps", [("C3", (64, 64, 32), 30), ("C4", (64, 64, 32), 30),
                                                 ("C5a", (48, 40, 24), 20), ("C5b", (48, 40, 24), 20)])
 def test_replicas_of_large_configs(name, shape, nsteps):
@@ -187,4 +219,33 @@ def test_C3_current_sweep_iv_replica():
     psi, mu = s.get_psi_mu()
     assert np.max(np.abs(psi.cpu().numpy() - st.psi)) <= 1e-4
     assert rel_l2(psi.cpu().numpy(), st.psi) <= 1e-5
+    s.close()
+
+
+def test_C3_full_current_sweep_ten_legs():
+    """C3's whole I-V protocol (BASELINE.json configs[2]) on the 64 x 64 x 32 replica: all ten currents of
+    tdgl_inputs.C3_CURRENTS, 200 steps per leg, E_x averaged per leg against the oracle driven the same way (replaying the
+    GPU's sweep counts), noise off."""
+    cfg = I.CONFIGS["C3"].scaled(64, 64, 32)
+    p, st, eps, (Bx, Bz), s = setup_pair(cfg, temperature=0.0)
+    bx_req, bz_req = cfg.requested_field()
+    assert len(I.C3_CURRENTS) == 10
+    nsteps, done, curve = 200, 0, []
+    for J in I.C3_CURRENTS:
+        s.set_field_current(Bx=bx_req, Bz=bz_req, Jx=J)
+        s.step(nsteps)
+        counts, _ = s.sweep_log(nsteps)
+        ex = []
+        for n in range(nsteps):
+            O.step(p, st, eps, Bx, Bz, f32(J), fixed_sweeps=int(counts[n]))
+            ex.append(st.Ex)
+        done += nsteps
+        ob = s.observables()
+        curve.append((J, ob.Ex_mean, float(np.mean(ex))))
+        assert ob.steps == done and ob.status == 0
+        assert abs(ob.Ex_mean - float(np.mean(ex))) < 1e-6, curve
+        assert abs(ob.K - st.K) < 1e-4, (J, ob.K, st.K)
+    psi, _ = s.get_psi_mu()
+    assert abs(s.observables().mean_abs2 - O.mean_abs2(st.psi)) <= 1e-3
+    print("C3 replica I-V (J, <Ex> gpu, <Ex> oracle):", curve, "max|dpsi| =", float(np.max(np.abs(psi.cpu().numpy() - st.psi))))
     s.close()
