@@ -9,8 +9,11 @@ sweeps to criterion (34), J_av/K, rho, Poisson solve.  Prints ONE JSON line (ran
              resident in HBM (CUDA events on the launching stream, max over ranks)
   e2e        the same metric with, every step, the state uploaded from pinned host memory
              (tdgl_set_state), one tdgl_step, and psi, mu and the observables read back to the host
-  roofline   the Jacobi sweep kernel: 32 B/site algorithmic bytes / mean launch duration (CUDA events
-             around every sweep launch of a host-loop run of the same workload) vs the measured HBM peak
+  roofline   the sweep kernel with the largest share of the timed step (on C4 the fused two-sweep kernel k_march_pair,
+             else the plain sweep): 32 B/site/sweep algorithmic bytes / mean launch duration (CUDA events around every
+             launch of a host-loop run of the same workload) vs the measured HBM peak; `frac_of_min_traffic` for the
+             pair kernel; both kernels also under roofline_sweep / roofline_pair; step_traffic = the whole step
+  c5a        (C4 run only) a short resident leg on 1024x1024x512, open on all faces: steps/s at the largest grid
   cpu_baseline  the fp64 oracle (oracle/, numpy) timed on this box's host cores on a bounded sample
 N > 1 (torchrun): independent replicas, one per GPU ("replicas only"); no collective on the
 data path.  `--impl reference` times the oracle alone (rank 0).
@@ -214,6 +217,7 @@ def oracle_sample(cfg: I.Config, budget_s: float = 20.0, cores: int = 0):
             res = pool.map(_oracle_worker, [(cfg.name, w, budget_s) for w in range(cores)])
     wall = time.perf_counter() - t0
     n_sites = res[0][0]
+    steps_per_worker = max(r[1] for r in res)
     steps = sum(r[1] for r in res)
     sweeps = sum(r[2] for r in res)
     dt = max(r[3] for r in res)
@@ -221,6 +225,7 @@ def oracle_sample(cfg: I.Config, budget_s: float = 20.0, cores: int = 0):
             "sample": f"{sub.name} (C-order numpy fp64 oracle as it stands), {cores} independent replicas on {cores} "
                       f"host cores, {steps} steps and {sweeps} sweeps in {dt:.1f} s",
             "steps_per_s_on_sample": steps / dt, "ms_per_step_sample": 1e3 * dt * cores / steps,
+            "steps_per_worker": steps_per_worker, "ms_per_worker_step": 1e3 * dt / steps_per_worker,
             "host_cores_available": host_cores(), "wall_s": wall}
 
 
@@ -233,8 +238,13 @@ def run_reference(args, cfg):
     t_all = time.perf_counter()
     res = oracle_sample(cfg, budget_s=min(60.0, max(10.0, 2.0 * args.steps)))
     v = res["value"]
-    out = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-           "warmup": args.warmup, "ms_per_step": res["ms_per_step_sample"], "higher_is_better": True,
+    # `steps` / `ms_per_step` describe what was EXECUTED: every host core advanced its own replica of the slab sample by
+    # `steps` oracle steps (the slowest worker's count) in parallel, `ms_per_step` wall milliseconds each, after one
+    # untimed step; ms_per_step x steps is the timed wall time.  The K of the command line (`steps_requested`) only sizes
+    # the time budget: K = 200 oracle steps of this slab would take half an hour.
+    out = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": res["steps_per_worker"],
+           "steps_requested": args.steps, "warmup": 1, "warmup_requested": args.warmup,
+           "ms_per_step": res["ms_per_worker_step"], "ms_per_slab_step_per_core": res["ms_per_step_sample"], "higher_is_better": True,
            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
            "config": dict(config_dict(cfg), parallelism="%d host cores" % res["cores"], l2="n/a (host)",
                           loop="oracle.step on a bounded slab sample per bench step; " + res["sample"]),
@@ -253,6 +263,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-c5a", action="store_true", help="skip the short 1024x1024x512 leg that follows the C4 run")
     ap.add_argument("--pair-mode", type=int, default=1, help="tdgl_set_pair_mode: 1 automatic (default), 2 whenever the cap allows")
     ap.add_argument("--no-pairs", action="store_true", help="plain Jacobi sweeps only (tdgl_set_pair_mode 0): A/B against the fused two-sweep kernel")
     ap.add_argument("--fp64", action="store_true", help="the double-precision build (TDGL_FLAG_FP64; the paper's DP mode)")
@@ -457,7 +468,63 @@ def main():
                    "how": "per step: state uploaded from pinned host memory, tdgl_set_state + tdgl_step + tdgl_get_psi_mu + "
                           "tdgl_observables, state downloaded to pinned host memory; uploads / downloads on their own streams "
                           "(double-buffered: the copies of neighbouring steps overlap this step's kernels)"}
+    # ---- which kernel dominates the timed step: that one is `roofline` (the other stays under its own key) ------------
+    step_ms = ms / K
+    pps = (pair1[1] - pair0[1]) / K
+    sweeps_ps = sweeps / K
+    plain_ps = max(0.0, sweeps_ps - 1.0 - 2.0 * pps)          # sweep 1 is fused into the init kernel
+    roofline, step_traffic = roof, None
+    if roof is not None:
+        roof["launches_per_step"] = plain_ps
+        roof["share_of_step"] = plain_ps * roof["avg_launch_ms"] / step_ms
+    if roof_pair is not None:
+        roof_pair["peak_source"] = how
+        roof_pair["launches_per_step"] = pps
+        roof_pair["share_of_step"] = pps * roof_pair["avg_launch_ms"] / step_ms
+        if roof is None or roof_pair["share_of_step"] > roof["share_of_step"]:
+            roofline = roof_pair
+    if roofline is not None:
+        roofline = dict(roofline, dominant="largest share of the timed step among the kernels timed here; the other sweep "
+                                          "kernel is under roofline_sweep / roofline_pair")
+    if roof is not None and cfg.nz > 1 and not args.fp64 and not iter_mu:
+        # minimum DRAM bytes of the step AS EXECUTED: init + first sweep 40 B/site, every fused pair 32, every
+        # plain sweep 32, rho + J_av 12, the direct mu solve 56 (five passes over 4-8 B), over the time of the whole step
+        per_site = 40.0 + 32.0 * pps + 32.0 * plain_ps + 12.0 + 56.0
+        step_traffic = {"min_bytes_per_site": per_site, "achieved": per_site * N / (step_ms * 1e-3) / 1e9, "peak": peak,
+                        "unit": "GB/s", "frac": per_site * N / (step_ms * 1e-3) / 1e9 / peak,
+                        "note": "whole time step in graph mode: minimum real traffic of the kernels executed / ms_per_step / peak"}
     s.close()
+    del s
+    torch.cuda.empty_cache()
+
+    # ---- steps/s at the largest BASELINE grid (C5a: 1024 x 1024 x 512, open on all faces), a short resident leg -----------
+    c5a = None
+    if args.config == "C4" and world == 1 and not args.no_c5a and not (args.fp64 or args.mu_iterative):
+        c5 = I.CONFIGS["C5a"]
+        if torch.cuda.mem_get_info()[0] > 60 * c5.n_sites:
+            s5 = make_solver(c5)
+            W5, K5 = 20, 30
+            s5.step(W5)
+            torch.cuda.synchronize()
+            o0 = s5.observables()
+            l5 = s5.launch_count()
+            f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            f0.record()
+            s5.step(K5)
+            f1.record()
+            torch.cuda.synchronize()
+            ms5 = f0.elapsed_time(f1)
+            l5 = s5.launch_count() - l5
+            o1 = s5.observables()
+            v5, sps5 = throughput(c5.n_sites, o1.sweeps_total - o0.sweeps_total, K5, 1, ms5)
+            c5a = {"workload": "C5a", "grid": [c5.nx, c5.ny, c5.nz], "bc": list(c5.bc), "steps": K5, "warmup": W5,
+                   "ms_per_step": ms5 / K5, "steps_per_s": sps5, "value": v5, "unit": UNIT,
+                   "sweeps_per_step": (o1.sweeps_total - o0.sweeps_total) / K5, "gpu_launches": int(l5),
+                   "state": {"mean_abs2": o1.mean_abs2, "status": o1.status},
+                   "note": "north_star: steps/s up to 1024x1024x512; the literal all-open configs[4] with Jx = 0 (reading S14); the "
+                           "run starts from the random initial state (protocol length is 500 steps: BASELINE.md section 4)"}
+            s5.close()
+            del s5
 
     if rank != 0:
         if world > 1:
@@ -475,7 +542,8 @@ def main():
         "config": dict(config_dict(cfg, world), **({"mu_solver": "pseudo-time iteration (Eq. 40), host-driven loop"} if iter_mu else
                                                    ({"mu_solver": "direct: fp32 transform solver inside fp64 iterative refinement"} if args.mu_direct else {}))),
         "mu_iteration": mu_stats,
-        "clocks": clocks, "e2e": e2e, "gpu_launches": launches_all, "roofline": roof, "roofline_pair": roof_pair,
+        "clocks": clocks, "e2e": e2e, "gpu_launches": launches_all, "roofline": roofline, "roofline_sweep": roof,
+        "roofline_pair": roof_pair, "step_traffic": step_traffic, "c5a": c5a,
         "pairs": pairs, "cpu_baseline": cpu,
         "state": {"mean_abs2": ob1.mean_abs2, "Ex": ob1.Ex, "K": ob1.K, "vortices_per_slice": ob1.vortices_per_slice,
                   "status": ob1.status},
