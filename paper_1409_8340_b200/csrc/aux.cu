@@ -325,14 +325,24 @@ __global__ void __launch_bounds__(256, 4) k_obs_partial(const __grid_constant__ 
     float gx0;
     { const float2 g = cmulc(c, e); gx0 = obs_arg(g.y, g.x); }
     float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
+    // the three loads of a row are issued one row ahead (the walk is otherwise a chain of load -> use: 69 % of the stall
+    // samples were long_scoreboard)
+    int jn = (jb + 1 == ny) ? 0 : jb + 1;
+    const float2 *pn = prow0 + (long long)nx * jn;                              // psi(col, j + 1, k)
+    float2 nr = *pn, tz = *ptop;
+    float ep = *erow;
     for (int j = jb; j < je; ++j) {
-      const int jp = (j + 1 == ny) ? 0 : j + 1;
+      const int jp = jn;
+      float2 nr2 = nr, tz2 = tz;
+      float ep2 = ep;
+      if (j + 1 < je) {                                                         // (warp-uniform)
+        jn = (jp + 1 == ny) ? 0 : jp + 1;
+        pn = (jn == 0) ? prow0 : pn + nx;
+        ptop += nx; erow += nx;
+        nr2 = *pn; tz2 = *ptop; ep2 = *erow;
+      }
       const bool hasy = py || j + 1 < ny;
       const float wy = face_w(j, ny, dv.bcy);
-      const float2 nr = (jp == 0) ? *prow0 : prow[nx];
-      const float2 tz = *ptop;
-      const float ep = *erow;
-      prow += nx; ptop += nx; erow += nx;
       const float2 ner = make_float2(__shfl_down_sync(0xffffffffu, nr.x, 1), __shfl_down_sync(0xffffffffu, nr.y, 1));
       const float2 t = cmul(YZ ? Uzc : dv.Uz[j], tz);
       const float2 nn = ylink(j, nr);
@@ -354,6 +364,7 @@ __global__ void __launch_bounds__(256, 4) k_obs_partial(const __grid_constant__ 
         if (hasx && hasy) s3 += rintf((gx0 + gy1 - gx1 - gy0 + flux) * inv2pi);
       }
       c = nr; er = ner; e = en; gx0 = gx1;
+      nr = nr2; tz = tz2; ep = ep2;
     }
     a0 += (double)s0; a1 += (double)s1; a2 += (double)s2; a3 += (double)s3;
   }
